@@ -1,0 +1,139 @@
+"""ctypes loader for the plain-C CPU oracle (``dpi_oracle.c``).
+
+TEST INFRASTRUCTURE ONLY. May be imported by ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs; never by ``paper_2606_21101_b200``. It imports nothing from
+the CUDA path. Argument marshalling only: every number comes out of ``dpi_oracle.c``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+from typing import Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "dpi_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lock = threading.Lock()
+_lib = None
+
+F32, F16, BF16 = 0, 1, 2
+SUM, MEAN = 0, 1
+_STATUS = {0: "ok", 1: "bad argument", 2: "index out of range", 3: "offset overflow (N >= 2^31)",
+           4: "seg_bag capacity too small"}
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+def build(force: bool = False) -> str:
+    """Compile dpi_oracle.c -> liboracle.so with gcc (-O2, no fast-math, no FMA contraction)."""
+    with _lock:
+        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+            tmp = _LIB + f".tmp{os.getpid()}"
+            subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared",
+                                   "-Wall", "-Wextra", "-o", tmp, _SRC])
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        lib.oracle_alg1_onehot.argtypes = [i32, i32, i32, ctypes.c_int, vp, vp, vp, vp]
+        lib.oracle_alg1_onehot.restype = ctypes.c_int
+        lib.oracle_lookup.argtypes = [i32, i32, i32, ctypes.c_int, vp, vp, vp, vp, vp, vp]
+        lib.oracle_lookup.restype = ctypes.c_int
+        lib.oracle_plan.argtypes = [vp, i64, i32, vp, vp, i64, vp]
+        lib.oracle_plan.restype = ctypes.c_int
+        lib.oracle_decode_f16.argtypes = [ctypes.c_uint16]
+        lib.oracle_decode_f16.restype = ctypes.c_double
+        lib.oracle_decode_bf16.argtypes = [ctypes.c_uint16]
+        lib.oracle_decode_bf16.restype = ctypes.c_double
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise OracleError(_STATUS.get(rc, f"status {rc}"))
+
+
+_STORAGE = {F32: np.float32, F16: np.float16, BF16: np.uint16}
+
+
+def _table_ptrs(tables: Sequence[np.ndarray], dtype: int, D: int):
+    keep = []
+    for t in tables:
+        a = np.ascontiguousarray(t)
+        if dtype == F16 and a.dtype == np.uint16:
+            pass  # raw binary16 bits are accepted as well
+        elif a.dtype != _STORAGE[dtype]:
+            raise TypeError(f"table dtype {a.dtype} does not match oracle dtype code {dtype}")
+        if a.ndim != 2 or a.shape[1] != D:
+            raise ValueError("table must be [rows, D]")
+        keep.append(a)
+    arr = (ctypes.c_void_p * len(keep))(*[a.ctypes.data for a in keep])
+    rows = np.asarray([a.shape[0] for a in keep], dtype=np.int64)
+    return arr, rows, keep
+
+
+def alg1_onehot(tables: Sequence[np.ndarray], dtype: int, ids: np.ndarray) -> np.ndarray:
+    """Algorithm 1. ids int32[b, k] -> float64[b, k*d]."""
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    b, k = ids.shape
+    d = int(np.asarray(tables[0]).shape[1])
+    ptrs, rows, keep = _table_ptrs(tables, dtype, d)
+    out = np.empty((b, k * d), dtype=np.float64)
+    _check(_load().oracle_alg1_onehot(b, k, d, dtype, ctypes.cast(ptrs, ctypes.c_void_p), rows.ctypes.data,
+                                      ids.ctypes.data, out.ctypes.data))
+    del keep
+    return out
+
+
+def lookup(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray, offsets: np.ndarray,
+           pooling: np.ndarray) -> np.ndarray:
+    """Pooled multi-hot lookup. Returns the unrounded float64 reference [B, T*D]."""
+    T = len(tables)
+    D = int(np.asarray(tables[0]).shape[1])
+    indices = np.ascontiguousarray(indices, dtype=np.int32)
+    offsets = np.ascontiguousarray(offsets, dtype=np.int32)
+    pooling = np.ascontiguousarray(pooling, dtype=np.uint8)
+    if offsets.shape[0] != B * T + 1 or pooling.shape[0] != T:
+        raise ValueError("offsets must be [B*T+1], pooling [T]")
+    if int(offsets[-1]) > indices.shape[0]:
+        raise ValueError("offsets[-1] exceeds len(indices)")
+    ptrs, rows, keep = _table_ptrs(tables, dtype, D)
+    ref = np.empty((B, T * D), dtype=np.float64)
+    _check(_load().oracle_lookup(T, B, D, dtype, ctypes.cast(ptrs, ctypes.c_void_p), rows.ctypes.data,
+                                 indices.ctypes.data, offsets.ctypes.data, pooling.ctypes.data,
+                                 ref.ctypes.data))
+    del keep
+    return ref
+
+
+def plan(lengths: np.ndarray, K: int):
+    """Workload plan. Returns (offsets int32[G+1], seg_bag int32[S+1], S)."""
+    lengths = np.ascontiguousarray(lengths, dtype=np.int32)
+    G = lengths.shape[0]
+    cap = (int(lengths.astype(np.int64).sum()) + G) // max(K, 1) + 3  # upper bound on S+1 (C[G] <= N + G)
+    offsets = np.empty(G + 1, dtype=np.int32)
+    seg_bag = np.empty(cap, dtype=np.int32)
+    S = ctypes.c_int32(0)
+    _check(_load().oracle_plan(lengths.ctypes.data, G, K, offsets.ctypes.data, seg_bag.ctypes.data, cap,
+                               ctypes.byref(S)))
+    return offsets, seg_bag[: S.value + 1].copy(), int(S.value)
+
+
+def decode_f16(bits: int) -> float:
+    return float(_load().oracle_decode_f16(int(bits)))
+
+
+def decode_bf16(bits: int) -> float:
+    return float(_load().oracle_decode_bf16(int(bits)))
