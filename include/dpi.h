@@ -1,0 +1,179 @@
+/*
+ * dpi.h -- C ABI of the B200-native fused multi-table embedding lookup (DPIFrame, arxiv 2606.21101).
+ *
+ * The path (citations are /root/reference/PAPER.md line numbers; DESIGN.md has the full readings):
+ *
+ *   a1  plan: offset scan        "the overall embedding workload is deterministic and known in advance"
+ *                                (PAPER.md:109), sizes computed before the traversal (Alg. 1 lines 1-2,
+ *                                PAPER.md:150-151); multi-hot "by marking offset information"
+ *   a2  plan: balanced segments  workload allocation across threads, output-first: adjacent workers own
+ *                                adjacent output addresses (§IV-C)
+ *   a3  fused gather-and-pool    Algorithm 1 "Multi-table Lookup" generalised to bags:
+ *                                one pass writes the concatenated EmbedOut[b x (k*d)]
+ *
+ * Notation: T tables (the paper's k), B samples (b), D embedding dim (d), G = B*T bags,
+ * bag id g = b*T + t (sample-major, Alg. 1 line 7 "IDs[row*k + table_id]"),
+ * len[g] bag length, N = sum len, K = cost quantum of a segment.
+ *
+ * Plan definition (integer, one correct answer; checked bit for bit against oracle/):
+ *   offsets[0] = 0, offsets[g+1] = offsets[g] + len[g]
+ *   C[0] = 0,       C[g+1] = C[g] + max(len[g], 1)
+ *   S = ceil(C[G] / K)
+ *   seg_bag[s] = min(G, min{ g in [0,G] : C[g] >= s*K })   for s = 0..S
+ *   warp-task s owns bags [seg_bag[s], seg_bag[s+1]).
+ *
+ * Lookup definition: for every bag g = (b,t), c < D
+ *   acc[c] = sum_{j in [offsets[g], offsets[g+1])} float(table_t[indices[j]][c])     (fp32 accumulate)
+ *   if pooling[t] == MEAN and len > 0: acc[c] /= len;   empty bag -> +0.0
+ *   out[b, t*D + c] = cast_to_table_dtype(acc[c])       (one RNE cast at the store)
+ *
+ * Conventions for every entry point
+ *   - extern "C"; nothing throws across the boundary; every call returns dpi_status_t.
+ *   - "host" pointers are ordinary CPU memory; "device" pointers are CUDA device memory of the current
+ *     device. The library never takes torch types.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Caller owns tables, table_ptrs, lengths, indices, out. The library owns everything inside dpi_plan_t.
+ *   - Asynchronous calls (dpi_plan_build, dpi_lookup, dpi_check_indices without result read) only enqueue
+ *     work; device-side faults surface at the caller's next synchronisation.
+ *   - There is NO CPU fallback: without a CUDA device every call that needs one returns DPI_ERR_CUDA.
+ *   - A plan is not thread-safe; distinct plans are independent.
+ */
+#ifndef DPI_H_
+#define DPI_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DPI_VERSION 100       /* 0.1.0 */
+#define DPI_MAX_TABLES 2048   /* pooling modes travel to the kernel as a by-value bit mask */
+
+typedef struct dpi_plan_s dpi_plan_t; /* opaque, library-owned */
+
+typedef enum {
+    DPI_OK = 0,
+    DPI_ERR_INVALID_ARG = 1,  /* NULL, non-positive sizes, misaligned pointers, capacity exceeded */
+    DPI_ERR_UNSUPPORTED = 2,  /* mixed dims, row size not a multiple of 16 B or > 512 B, T > DPI_MAX_TABLES */
+    DPI_ERR_ALLOC = 3,        /* host or device allocation failed */
+    DPI_ERR_CUDA = 4,         /* CUDA runtime error (text in dpi_last_error) */
+    DPI_ERR_INDEX_RANGE = 5   /* dpi_check_indices found indices outside [0, table_rows[t]) */
+} dpi_status_t;
+
+typedef enum { DPI_F32 = 0, DPI_F16 = 1, DPI_BF16 = 2 } dpi_dtype_t;
+typedef enum { DPI_POOL_SUM = 0, DPI_POOL_MEAN = 1 } dpi_pool_t;
+
+/* Tuning knobs for dpi_plan_set_option (all kernel-internal; none changes a result). */
+typedef enum {
+    DPI_OPT_UNROLL = 0,         /* independent 128-bit row loads in flight per lane: 2, 4, 8 or 16; 0 = auto */
+    DPI_OPT_BLOCK_THREADS = 1,  /* lookup CTA size: 128, 256 or 512; 0 = auto */
+    DPI_OPT_BLOCKS_PER_SM = 2,  /* persistent grid = SMs * this; 0 = auto (occupancy) */
+    DPI_OPT_MODE = 3,           /* 0 auto per segment, 1 sub-warp per bag, 2 whole warp per bag */
+    DPI_OPT_ROW_L1_NO_ALLOC = 4,/* 1: table rows bypass L1 (ld.global.nc.L1::no_allocate); 0: default; -1 auto */
+    DPI_OPT_PDL = 5,            /* 1: lookup is launched with programmatic dependent launch after the planner */
+    DPI_OPT_COUNT_
+} dpi_option_t;
+
+/*
+ * dpi_plan_create -- host side. Validates the shape and allocates the plan's device buffers once; the plan
+ * is reusable for any batch of the same (T, B, dims, dtype) whose N <= max_indices.
+ *   T            number of tables, 1..DPI_MAX_TABLES
+ *   table_rows   host int64[T], heights n_t >= 1; copied
+ *   dims         host int32[T], embedding dim of each table; v1 requires all equal (R10) and
+ *                D*sizeof(dtype) a multiple of 16 B and <= 512 B, else DPI_ERR_UNSUPPORTED
+ *   dtype        storage type of tables AND of the output
+ *   B            samples per batch >= 1;  G = B*T must be < 2^31
+ *   max_indices  upper bound on N for any batch built with this plan, 0 <= max_indices < 2^31
+ *   plan         receives the handle; destroy with dpi_plan_destroy
+ */
+dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t* dims, dpi_dtype_t dtype,
+                             int32_t B, int64_t max_indices, dpi_plan_t** plan);
+
+/* Cost quantum K >= 1 of the balanced segments (0 = library default for this row size). Takes effect at the
+ * next dpi_plan_build. DPI_ERR_INVALID_ARG if K < 0. */
+dpi_status_t dpi_plan_set_quantum(dpi_plan_t* plan, int32_t K);
+
+/* Kernel-internal tuning (see dpi_option_t). Unknown option or unsupported value -> DPI_ERR_INVALID_ARG. */
+dpi_status_t dpi_plan_set_option(dpi_plan_t* plan, dpi_option_t opt, int32_t value);
+dpi_status_t dpi_plan_get_option(const dpi_plan_t* plan, dpi_option_t opt, int32_t* value);
+
+/*
+ * dpi_plan_build -- steps a1 + a2 on the device, asynchronous on `stream`, ONE kernel launch for all
+ * (sample, table) bags (no per-table launches, no host synchronisation):
+ *   lengths_dev  device int32[G], len[g] >= 0, g = b*T + t, 4-byte aligned
+ * Writes the plan's offsets[G+1], seg_bag[S+1] and S (device memory). If the batch has N > max_indices
+ * the device sets an overflow flag that dpi_plan_export / dpi_plan_stats report (DPI_ERR_INVALID_ARG);
+ * seg_bag writes beyond the capacity are suppressed, never out of bounds.
+ */
+dpi_status_t dpi_plan_build(dpi_plan_t* plan, const int32_t* lengths_dev, void* stream);
+
+/* north_star spelling: dpi_plan(table_rows[T], dims, lengths, B) = create (max_indices given) + build. */
+dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims, dpi_dtype_t dtype,
+                      const int32_t* lengths_dev, int32_t B, int64_t max_indices, void* stream,
+                      dpi_plan_t** plan);
+
+/* Borrowed device pointers into the plan, valid until the next build/destroy. Any out-pointer may be NULL.
+ *   offsets_dev int32[G+1]; seg_bag_dev int32[seg_capacity]; meta_dev int32[8] = {S, N, C[G] low 32 bits,
+ *   overflow flag, K, G, 0, 0}. */
+dpi_status_t dpi_plan_device_views(const dpi_plan_t* plan, const int32_t** offsets_dev,
+                                   const int32_t** seg_bag_dev, const int32_t** meta_dev);
+
+/* Static facts about a plan (host only, no synchronisation). Any out-pointer may be NULL. */
+dpi_status_t dpi_plan_info(const dpi_plan_t* plan, int32_t* T, int32_t* B, int32_t* D, int32_t* dtype,
+                           int64_t* G, int32_t* K, int64_t* seg_capacity);
+
+/* Parity/debug: synchronises `stream`, copies the plan to caller-owned host arrays.
+ *   offsets_host int32[G+1] (may be NULL); seg_bag_host int32[seg_cap] receives S+1 entries (may be NULL);
+ *   S, N receive the segment count and total index count (may be NULL).
+ * DPI_ERR_INVALID_ARG if seg_cap < S+1 or the last build overflowed max_indices. */
+dpi_status_t dpi_plan_export(const dpi_plan_t* plan, int32_t* offsets_host, int32_t* seg_bag_host,
+                             int64_t seg_cap, int32_t* S, int64_t* N, void* stream);
+
+/*
+ * dpi_lookup -- step a3, asynchronous on `stream`, ONE kernel launch for all tables and samples.
+ *   table_ptrs_dev device array of T device pointers; table t is row-major [table_rows[t], D] of the
+ *                  plan's dtype, 16-byte aligned ("Embs", per-table local ids PAPER.md:162)
+ *   indices_dev    device int32[N], per-table local row ids, bag-contiguous in bag order g
+ *   offsets_dev    NULL (use the plan's own offsets) or a device int32[G+1] equal to them
+ *   plan           a built plan (same stream, or ordered after dpi_plan_build by an event)
+ *   pooling        host uint8[T] of dpi_pool_t (NULL = all SUM)
+ *   out_dev        device [B, T*D] row-major in the plan's dtype, 16-byte aligned; table t at columns
+ *                  [t*D, (t+1)*D); every element is written exactly once
+ * Out-of-range indices are a precondition violation (the paper is silent, R12): use
+ * dpi_check_indices in tests.
+ */
+dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indices_dev,
+                        const int32_t* offsets_dev, const dpi_plan_t* plan, const uint8_t* pooling,
+                        void* out_dev, void* stream);
+
+/*
+ * dpi_forward_host -- the whole path (a1+a2+a3) for callers whose sparse inputs live in HOST memory
+ * (the end-to-end number of bench.py): copies lengths and indices host->device into plan-owned staging,
+ * builds the plan, runs the lookup and copies the [B, T*D] block back, then synchronises `stream`.
+ * Tables stay resident on the device (they are the model, not a per-batch input).
+ *   lengths_host int32[G]; indices_host int32[n_indices] (n_indices <= max_indices); out_host [B,T*D].
+ *   Pinned (page-locked) host buffers make the copies asynchronous and faster but are not required.
+ */
+dpi_status_t dpi_forward_host(dpi_plan_t* plan, const void* const* table_ptrs_dev,
+                              const int32_t* lengths_host, const int32_t* indices_host, int64_t n_indices,
+                              const uint8_t* pooling, void* out_host, void* stream);
+
+/* Off the hot path: counts indices outside [0, table_rows[t]) for the last built batch; synchronises.
+ * Returns DPI_ERR_INDEX_RANGE (and *n_bad > 0) if any. */
+dpi_status_t dpi_check_indices(const dpi_plan_t* plan, const int32_t* indices_dev, int64_t* n_bad,
+                               void* stream);
+
+dpi_status_t dpi_plan_destroy(dpi_plan_t* plan);
+
+/* Number of kernels this library has launched in this process (for bench.py's gpu_launches claim). */
+int64_t dpi_launch_count(void);
+
+int32_t dpi_version(void);
+const char* dpi_status_string(dpi_status_t status);
+const char* dpi_last_error(void); /* thread-local detail of the last failing call on this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DPI_H_ */

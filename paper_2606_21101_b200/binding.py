@@ -1,0 +1,237 @@
+"""Thin ctypes binding over ``libdpi.so`` (include/dpi.h). Argument marshalling only: every step of the
+path runs in the CUDA library. PyTorch appears here only as the owner of device memory and streams.
+
+There is no CPU fallback: if the library is missing, import-time use raises ``DpiLibraryMissing``; if no
+CUDA device is present the library itself returns ``DPI_ERR_CUDA``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+DPI_OK = 0
+STATUS_NAMES = {0: "DPI_OK", 1: "DPI_ERR_INVALID_ARG", 2: "DPI_ERR_UNSUPPORTED", 3: "DPI_ERR_ALLOC",
+                4: "DPI_ERR_CUDA", 5: "DPI_ERR_INDEX_RANGE"}
+DPI_F32, DPI_F16, DPI_BF16 = 0, 1, 2
+DPI_POOL_SUM, DPI_POOL_MEAN = 0, 1
+OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL = range(6)
+
+# every symbol include/dpi.h declares (tests check the .so exports each one)
+EXPORTS = ["dpi_plan_create", "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
+           "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export",
+           "dpi_lookup", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
+           "dpi_version", "dpi_status_string", "dpi_last_error"]
+
+
+class DpiLibraryMissing(RuntimeError):
+    pass
+
+
+class DpiError(RuntimeError):
+    def __init__(self, status: int, detail: str):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {detail}")
+        self.status = status
+        self.detail = detail
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None) -> ctypes.CDLL:
+    """dlopen libdpi.so (built in-tree by ``python -m paper_2606_21101_b200.build``)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or _build.lib_path("libdpi.so")
+    if not os.path.exists(path):
+        raise DpiLibraryMissing(f"{path} not found: run `python -m paper_2606_21101_b200.build` "
+                                "(the CUDA library is the only implementation; there is no fallback)")
+    lib = ctypes.CDLL(path)
+    vp, i32, i64, st = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int
+    sig = {
+        "dpi_plan_create": (st, [i32, vp, vp, ctypes.c_int, i32, i64, vp]),
+        "dpi_plan_set_quantum": (st, [vp, i32]),
+        "dpi_plan_set_option": (st, [vp, ctypes.c_int, i32]),
+        "dpi_plan_get_option": (st, [vp, ctypes.c_int, vp]),
+        "dpi_plan_build": (st, [vp, vp, vp]),
+        "dpi_plan": (st, [vp, i32, vp, ctypes.c_int, vp, i32, i64, vp, vp]),
+        "dpi_plan_device_views": (st, [vp, vp, vp, vp]),
+        "dpi_plan_info": (st, [vp, vp, vp, vp, vp, vp, vp, vp]),
+        "dpi_plan_export": (st, [vp, vp, vp, i64, vp, vp, vp]),
+        "dpi_lookup": (st, [vp, vp, vp, vp, vp, vp, vp]),
+        "dpi_forward_host": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
+        "dpi_check_indices": (st, [vp, vp, vp, vp]),
+        "dpi_plan_destroy": (st, [vp]),
+        "dpi_launch_count": (i64, []),
+        "dpi_version": (i32, []),
+        "dpi_status_string": (ctypes.c_char_p, [ctypes.c_int]),
+        "dpi_last_error": (ctypes.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _check(status: int):
+    if status != DPI_OK:
+        raise DpiError(status, load_library().dpi_last_error().decode(errors="replace"))
+
+
+def _ptr(x) -> int:
+    """Device/host address of a torch tensor, numpy array, int or None."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return x.data_ptr()  # torch.Tensor
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def launch_count() -> int:
+    return int(load_library().dpi_launch_count())
+
+
+def version() -> int:
+    return int(load_library().dpi_version())
+
+
+class Plan:
+    """Owner of a ``dpi_plan_t*``. Method names mirror the C entry points."""
+
+    def __init__(self, table_rows: Sequence[int], dims, dtype: int, B: int, max_indices: int):
+        lib = load_library()
+        self._lib = lib
+        rows = np.ascontiguousarray(table_rows, dtype=np.int64)
+        T = rows.shape[0]
+        dims = np.ascontiguousarray(np.broadcast_to(np.asarray(dims, dtype=np.int32), (T,)))
+        handle = ctypes.c_void_p()
+        _check(lib.dpi_plan_create(T, rows.ctypes.data, dims.ctypes.data, int(dtype), int(B), int(max_indices),
+                                   ctypes.byref(handle)))
+        self._h = handle
+        self.T, self.B, self.D, self.dtype = T, int(B), int(dims[0]), int(dtype)
+        self.G = self.T * self.B
+        self.max_indices = int(max_indices)
+
+    # -- lifetime --------------------------------------------------------------------------------------
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.dpi_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # -- dpi_plan_set_quantum / options ---------------------------------------------------------------------
+    def set_quantum(self, K: int):
+        _check(self._lib.dpi_plan_set_quantum(self._h, int(K)))
+
+    def set_option(self, opt: int, value: int):
+        _check(self._lib.dpi_plan_set_option(self._h, int(opt), int(value)))
+
+    def get_option(self, opt: int) -> int:
+        v = ctypes.c_int32()
+        _check(self._lib.dpi_plan_get_option(self._h, int(opt), ctypes.byref(v)))
+        return v.value
+
+    def info(self) -> dict:
+        T, B, D, dt, K = (ctypes.c_int32() for _ in range(5))
+        G, cap = ctypes.c_int64(), ctypes.c_int64()
+        _check(self._lib.dpi_plan_info(self._h, ctypes.byref(T), ctypes.byref(B), ctypes.byref(D), ctypes.byref(dt),
+                                       ctypes.byref(G), ctypes.byref(K), ctypes.byref(cap)))
+        return {"T": T.value, "B": B.value, "D": D.value, "dtype": dt.value, "G": G.value, "K": K.value,
+                "seg_capacity": cap.value}
+
+    # -- dpi_plan_build -------------------------------------------------------------------------------------
+    def build(self, lengths_dev, stream=None):
+        _check(self._lib.dpi_plan_build(self._h, _ptr(lengths_dev), _stream_handle(stream)))
+
+    # -- dpi_plan_device_views ------------------------------------------------------------------------------
+    def device_views(self):
+        o, s, m = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
+        _check(self._lib.dpi_plan_device_views(self._h, ctypes.byref(o), ctypes.byref(s), ctypes.byref(m)))
+        return o.value, s.value, m.value
+
+    # -- dpi_plan_export ------------------------------------------------------------------------------------
+    def export(self, stream=None):
+        """Returns (offsets int32[G+1], seg_bag int32[S+1], S, N) as host numpy arrays (synchronises)."""
+        cap = self.info()["seg_capacity"]
+        offsets = np.empty(self.G + 1, dtype=np.int32)
+        seg = np.empty(cap, dtype=np.int32)
+        S, N = ctypes.c_int32(), ctypes.c_int64()
+        _check(self._lib.dpi_plan_export(self._h, offsets.ctypes.data, seg.ctypes.data, cap, ctypes.byref(S),
+                                         ctypes.byref(N), _stream_handle(stream)))
+        return offsets, seg[: S.value + 1].copy(), int(S.value), int(N.value)
+
+    # -- dpi_lookup -----------------------------------------------------------------------------------------
+    def lookup(self, table_ptrs_dev, indices_dev, out_dev, pooling=None, offsets_dev=None, stream=None):
+        pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
+        _check(self._lib.dpi_lookup(_ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(offsets_dev), self._h,
+                                    _ptr(pool), _ptr(out_dev), _stream_handle(stream)))
+
+    # -- dpi_forward_host -----------------------------------------------------------------------------------
+    def forward_host(self, table_ptrs_dev, lengths_host, indices_host, out_host, pooling=None, stream=None):
+        pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
+        n = int(indices_host.numel() if hasattr(indices_host, "numel") else indices_host.shape[0])
+        _check(self._lib.dpi_forward_host(self._h, _ptr(table_ptrs_dev), _ptr(lengths_host), _ptr(indices_host), n,
+                                          _ptr(pool), _ptr(out_host), _stream_handle(stream)))
+
+    # -- dpi_check_indices ----------------------------------------------------------------------------------
+    def check_indices(self, indices_dev, stream=None) -> int:
+        n_bad = ctypes.c_int64()
+        st = self._lib.dpi_check_indices(self._h, _ptr(indices_dev), ctypes.byref(n_bad), _stream_handle(stream))
+        if st not in (DPI_OK, 5):
+            _check(st)
+        return int(n_bad.value)
+
+
+def dpi_plan(table_rows, dims, dtype: int, lengths_dev, B: int, max_indices: int, stream=None) -> Plan:
+    """north_star spelling: create + build."""
+    p = Plan(table_rows, dims, dtype, B, max_indices)
+    p.build(lengths_dev, stream)
+    return p
+
+
+def dpi_lookup(table_ptrs_dev, indices_dev, offsets_dev, plan: Plan, pooling, out_dev, stream=None):
+    plan.lookup(table_ptrs_dev, indices_dev, out_dev, pooling=pooling, offsets_dev=offsets_dev, stream=stream)
+
+
+# ----------------------------------------------------------------------------------------------------
+# bench/test helper library (synthetic table fill on the device) -- not part of the method
+# ----------------------------------------------------------------------------------------------------
+_synth = None
+
+
+def synth_fill_table(dst_dev, n_elems: int, dtype: int, key: int, stream=None):
+    global _synth
+    if _synth is None:
+        path = _build.lib_path("libdpi_synth.so")
+        if not os.path.exists(path):
+            raise DpiLibraryMissing(f"{path} not found: run `python -m paper_2606_21101_b200.build`")
+        _synth = ctypes.CDLL(path)
+        _synth.dpi_synth_fill_table.restype = ctypes.c_int
+        _synth.dpi_synth_fill_table.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int, ctypes.c_uint64,
+                                                ctypes.c_void_p]
+    rc = _synth.dpi_synth_fill_table(_ptr(dst_dev), int(n_elems), int(dtype), int(key), _stream_handle(stream))
+    if rc != 0:
+        raise RuntimeError(f"dpi_synth_fill_table failed with cudaError {rc}")

@@ -1,0 +1,449 @@
+// dpi_api.cu -- the C ABI of include/dpi.h. Host-side validation, plan ownership and launches only:
+// every step of the path runs in plan_kernels.cu / lookup_*.cu. No CPU fallback anywhere.
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "dpi_internal.cuh"
+
+namespace dpi {
+namespace {
+
+thread_local char g_err[512] = "";
+std::atomic<long long> g_launches{0};
+
+dpi_status_t fail(dpi_status_t st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return st;
+}
+dpi_status_t cuda_fail(cudaError_t e, const char* what) {
+    (void)cudaGetLastError();
+    return fail(e == cudaErrorMemoryAllocation ? DPI_ERR_ALLOC : DPI_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+#define DPI_CUDA(call)                                       \
+    do {                                                     \
+        cudaError_t e_ = (call);                             \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);  \
+    } while (0)
+
+int pow2ceil(int x) {
+    int p = 1;
+    while (p < x) p <<= 1;
+    return p;
+}
+
+}  // namespace
+
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+}  // namespace dpi
+
+using namespace dpi;
+
+struct dpi_plan_s {
+    // shape
+    int32_t T = 0, B = 0, D = 0;
+    dpi_dtype_t dtype = DPI_F32;
+    uint32_t G = 0;
+    int64_t max_indices = 0;
+    uint32_t nvec = 0;   // 16-byte vectors per row
+    int lanes = 0;       // lanes per row
+    std::vector<int64_t> table_rows;
+    // plan parameters
+    int32_t K = 0;           // effective quantum
+    int32_t K_user = 0;      // 0 = default
+    uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
+    uint32_t num_tiles = 0;
+    uint32_t epoch = 0;
+    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0};
+    // device
+    int device = 0, num_sms = 0;
+    int32_t* offsets = nullptr;
+    int32_t* seg_bag = nullptr;
+    int32_t* meta = nullptr;
+    unsigned long long* tile_len = nullptr;
+    unsigned long long* tile_cost = nullptr;
+    unsigned int* ticket = nullptr;
+    int64_t* table_rows_dev = nullptr;
+    unsigned long long* n_bad_dev = nullptr;
+    // staging for dpi_forward_host
+    int32_t* stage_len = nullptr;
+    int32_t* stage_idx = nullptr;
+    void* stage_out = nullptr;
+    bool built = false;
+};
+
+namespace {
+
+int32_t default_quantum(const dpi_plan_t* p) {
+    // One warp-task should keep P*U row loads in flight for a few rounds: ~32 entries per task works across
+    // row sizes (64 B rows: 8 sub-warps x 4; 256 B rows: 2 sub-warps x 16). Tuned by ncu, see DESIGN.md §6.
+    (void)p;
+    return 32;
+}
+
+uint32_t seg_capacity_for(const dpi_plan_t* p, int32_t K) {
+    // S = ceil(C[G]/K) <= ceil((max_indices + G)/K); +2 for seg_bag[S] and slack
+    const uint64_t c_max = static_cast<uint64_t>(p->max_indices) + p->G;
+    return static_cast<uint32_t>((c_max + K - 1) / K + 2);
+}
+
+dpi_status_t ensure_seg_capacity(dpi_plan_t* p, int32_t K) {
+    const uint32_t need = seg_capacity_for(p, K);
+    if (need <= p->seg_cap && p->seg_bag) return DPI_OK;
+    if (p->seg_bag) DPI_CUDA(cudaFree(p->seg_bag));
+    p->seg_bag = nullptr;
+    DPI_CUDA(cudaMalloc(&p->seg_bag, static_cast<size_t>(need) * sizeof(int32_t)));
+    p->seg_cap = need;
+    return DPI_OK;
+}
+
+void free_plan(dpi_plan_t* p) {
+    if (!p) return;
+    cudaFree(p->offsets); cudaFree(p->seg_bag); cudaFree(p->meta); cudaFree(p->tile_len);
+    cudaFree(p->tile_cost); cudaFree(p->ticket); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
+    cudaFree(p->stage_len); cudaFree(p->stage_idx); cudaFree(p->stage_out);
+    (void)cudaGetLastError();
+    delete p;
+}
+
+struct LaunchChoice {
+    LookupLaunch l;
+    int row_no_alloc;
+};
+
+int occupancy(const dpi_plan_t* p, int lanes, int unroll, int threads) {
+    switch (p->dtype) {
+        case DPI_F32: return lookup_occupancy_f32(lanes, unroll, threads);
+        case DPI_F16: return lookup_occupancy_f16(lanes, unroll, threads);
+        default: return lookup_occupancy_bf16(lanes, unroll, threads);
+    }
+}
+
+LaunchChoice choose_launch(const dpi_plan_t* p) {
+    LaunchChoice c{};
+    c.l.lanes = p->lanes;
+    c.l.unroll = p->opt[DPI_OPT_UNROLL] ? p->opt[DPI_OPT_UNROLL] : 8;
+    c.l.block_threads = p->opt[DPI_OPT_BLOCK_THREADS] ? p->opt[DPI_OPT_BLOCK_THREADS] : 256;
+    int per_sm = p->opt[DPI_OPT_BLOCKS_PER_SM];
+    if (per_sm <= 0) {
+        per_sm = occupancy(p, c.l.lanes, c.l.unroll, c.l.block_threads);
+        if (per_sm <= 0) per_sm = 1;
+    }
+    c.l.grid = p->num_sms * per_sm;  // persistent: a whole number of waves, every CTA resident
+    c.l.pdl = p->opt[DPI_OPT_PDL] != 0;
+    c.row_no_alloc = p->opt[DPI_OPT_ROW_L1_NO_ALLOC] < 0 ? 1 : p->opt[DPI_OPT_ROW_L1_NO_ALLOC];
+    return c;
+}
+
+dpi_status_t do_lookup(const dpi_plan_t* p, const void* const* tables, const int32_t* indices, const int32_t* offsets,
+                       const uint8_t* pooling, void* out, cudaStream_t stream) {
+    LookupArgs a{};
+    a.tables = tables;
+    a.indices = indices;
+    a.offsets = offsets ? offsets : p->offsets;
+    a.seg_bag = p->seg_bag;
+    a.meta = p->meta;
+    a.out = out;
+    a.G = p->G;
+    a.T = static_cast<uint32_t>(p->T);
+    a.nvec = p->nvec;
+    a.mode = p->opt[DPI_OPT_MODE];
+    std::memset(&a.pool, 0, sizeof a.pool);
+    if (pooling) {
+        for (int t = 0; t < p->T; ++t) {
+            if (pooling[t] > 1) return fail(DPI_ERR_INVALID_ARG, "pooling[%d] = %d is not a dpi_pool_t", t, pooling[t]);
+            if (pooling[t] == DPI_POOL_MEAN) a.pool.w[t >> 5] |= 1u << (t & 31);
+        }
+    }
+    const LaunchChoice c = choose_launch(p);
+    a.row_no_alloc = c.row_no_alloc;
+    cudaError_t e;
+    switch (p->dtype) {
+        case DPI_F32: e = launch_lookup_f32(a, c.l, stream); break;
+        case DPI_F16: e = launch_lookup_f16(a, c.l, stream); break;
+        default: e = launch_lookup_bf16(a, c.l, stream); break;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "lookup kernel launch");
+    return DPI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t* dims, dpi_dtype_t dtype, int32_t B,
+                             int64_t max_indices, dpi_plan_t** plan) {
+    if (!plan) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    *plan = nullptr;
+    if (!table_rows || !dims) return fail(DPI_ERR_INVALID_ARG, "table_rows/dims is NULL");
+    if (T < 1 || B < 1) return fail(DPI_ERR_INVALID_ARG, "T=%d and B=%d must be >= 1", T, B);
+    if (T > DPI_MAX_TABLES) return fail(DPI_ERR_UNSUPPORTED, "T=%d exceeds DPI_MAX_TABLES=%d", T, DPI_MAX_TABLES);
+    if (dtype != DPI_F32 && dtype != DPI_F16 && dtype != DPI_BF16) return fail(DPI_ERR_INVALID_ARG, "unknown dtype %d", (int)dtype);
+    if (max_indices < 0 || max_indices >= (1ll << 31)) return fail(DPI_ERR_INVALID_ARG, "max_indices=%lld outside [0, 2^31)", (long long)max_indices);
+    const int64_t G64 = static_cast<int64_t>(B) * T;
+    if (G64 >= (1ll << 31) || G64 + max_indices >= (1ll << 32) - 16) return fail(DPI_ERR_INVALID_ARG, "B*T=%lld too large", (long long)G64);
+    const int32_t D = dims[0];
+    for (int t = 0; t < T; ++t) {
+        if (dims[t] < 1) return fail(DPI_ERR_INVALID_ARG, "dims[%d]=%d", t, dims[t]);
+        if (dims[t] != D) return fail(DPI_ERR_UNSUPPORTED, "mixed dims (dims[%d]=%d != dims[0]=%d): v1 needs one D (DESIGN.md R10)", t, dims[t], D);
+        if (table_rows[t] < 1) return fail(DPI_ERR_INVALID_ARG, "table_rows[%d]=%lld must be >= 1", t, (long long)table_rows[t]);
+        if (table_rows[t] > 0x7fffffffll) return fail(DPI_ERR_UNSUPPORTED, "table_rows[%d] exceeds int32 index range", t);
+    }
+    const int elt = dtype == DPI_F32 ? 4 : 2;
+    const int64_t row_bytes = static_cast<int64_t>(D) * elt;
+    if (row_bytes % 16 != 0) return fail(DPI_ERR_UNSUPPORTED, "row size %lld B is not a multiple of 16 B", (long long)row_bytes);
+    if (row_bytes > 512) return fail(DPI_ERR_UNSUPPORTED, "row size %lld B exceeds 512 B (one warp-wide 128-bit load)", (long long)row_bytes);
+
+    int dev = 0, n_dev = 0;
+    cudaError_t e = cudaGetDeviceCount(&n_dev);
+    if (e != cudaSuccess || n_dev == 0) {
+        (void)cudaGetLastError();
+        return fail(DPI_ERR_CUDA, "no CUDA device (%s); libdpi has no CPU fallback", e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    }
+    DPI_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    DPI_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) return fail(DPI_ERR_UNSUPPORTED, "device sm_%d%d: libdpi is built for sm_100a only", prop.major, prop.minor);
+
+    dpi_plan_t* p = new (std::nothrow) dpi_plan_s();
+    if (!p) return fail(DPI_ERR_ALLOC, "host allocation failed");
+    p->T = T; p->B = B; p->D = D; p->dtype = dtype;
+    p->G = static_cast<uint32_t>(G64);
+    p->max_indices = max_indices;
+    p->nvec = static_cast<uint32_t>(row_bytes / 16);
+    p->lanes = pow2ceil(static_cast<int>(p->nvec));
+    p->table_rows.assign(table_rows, table_rows + T);
+    p->device = dev;
+    p->num_sms = prop.multiProcessorCount;
+    p->num_tiles = (p->G + kScanTile - 1) / kScanTile;
+    p->K = default_quantum(p);
+
+#define DPI_TRY(call)                                   \
+    do {                                                \
+        cudaError_t e2_ = (call);                       \
+        if (e2_ != cudaSuccess) {                       \
+            dpi_status_t st_ = cuda_fail(e2_, #call);   \
+            free_plan(p);                               \
+            return st_;                                 \
+        }                                               \
+    } while (0)
+    DPI_TRY(cudaMalloc(&p->offsets, (static_cast<size_t>(p->G) + 1) * sizeof(int32_t)));
+    DPI_TRY(cudaMalloc(&p->meta, kMetaWords * sizeof(int32_t)));
+    DPI_TRY(cudaMemset(p->meta, 0, kMetaWords * sizeof(int32_t)));
+    DPI_TRY(cudaMalloc(&p->tile_len, p->num_tiles * sizeof(unsigned long long)));
+    DPI_TRY(cudaMalloc(&p->tile_cost, p->num_tiles * sizeof(unsigned long long)));
+    DPI_TRY(cudaMemset(p->tile_len, 0, p->num_tiles * sizeof(unsigned long long)));
+    DPI_TRY(cudaMemset(p->tile_cost, 0, p->num_tiles * sizeof(unsigned long long)));
+    DPI_TRY(cudaMalloc(&p->ticket, sizeof(unsigned int)));
+    DPI_TRY(cudaMemset(p->ticket, 0, sizeof(unsigned int)));
+    DPI_TRY(cudaMalloc(&p->table_rows_dev, T * sizeof(int64_t)));
+    DPI_TRY(cudaMemcpy(p->table_rows_dev, table_rows, T * sizeof(int64_t), cudaMemcpyHostToDevice));
+    DPI_TRY(cudaMalloc(&p->n_bad_dev, sizeof(unsigned long long)));
+#undef DPI_TRY
+    dpi_status_t st = ensure_seg_capacity(p, p->K);
+    if (st != DPI_OK) { free_plan(p); return st; }
+    *plan = p;
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_set_quantum(dpi_plan_t* p, int32_t K) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (K < 0) return fail(DPI_ERR_INVALID_ARG, "K=%d must be >= 0", K);
+    p->K_user = K;
+    p->K = K ? K : default_quantum(p);
+    return ensure_seg_capacity(p, p->K);
+}
+
+dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    bool ok = false;
+    switch (opt) {
+        case DPI_OPT_UNROLL: ok = v == 0 || v == 2 || v == 4 || v == 8 || v == 16; break;
+        case DPI_OPT_BLOCK_THREADS: ok = v == 0 || (v >= 32 && v <= 512 && v % 32 == 0); break;
+        case DPI_OPT_BLOCKS_PER_SM: ok = v >= 0 && v <= 32; break;
+        case DPI_OPT_MODE: ok = v >= 0 && v <= 2; break;
+        case DPI_OPT_ROW_L1_NO_ALLOC: ok = v >= -1 && v <= 1; break;
+        case DPI_OPT_PDL: ok = v == 0 || v == 1; break;
+        default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);
+    }
+    if (!ok) return fail(DPI_ERR_INVALID_ARG, "value %d not supported for option %d", v, (int)opt);
+    p->opt[opt] = v;
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_get_option(const dpi_plan_t* p, dpi_option_t opt, int32_t* v) {
+    if (!p || !v || opt < 0 || opt >= DPI_OPT_COUNT_) return fail(DPI_ERR_INVALID_ARG, "bad argument");
+    *v = p->opt[opt];
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_build(dpi_plan_t* p, const int32_t* lengths_dev, void* stream) {
+    if (!p || !lengths_dev) return fail(DPI_ERR_INVALID_ARG, "plan/lengths_dev is NULL");
+    if (reinterpret_cast<uintptr_t>(lengths_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "lengths_dev is not 4-byte aligned");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    p->epoch += 1;
+    if (p->epoch >= (1u << 30)) {  // status words are tagged with a 30-bit epoch: clear once per wrap
+        DPI_CUDA(cudaMemsetAsync(p->tile_len, 0, p->num_tiles * sizeof(unsigned long long), s));
+        DPI_CUDA(cudaMemsetAsync(p->tile_cost, 0, p->num_tiles * sizeof(unsigned long long), s));
+        p->epoch = 1;
+    }
+    PlanArgs a{};
+    a.len = lengths_dev;
+    a.offsets = p->offsets;
+    a.seg_bag = p->seg_bag;
+    a.meta = p->meta;
+    a.tile_len = p->tile_len;
+    a.tile_cost = p->tile_cost;
+    a.ticket = p->ticket;
+    a.G = p->G;
+    a.K = static_cast<uint32_t>(p->K);
+    a.seg_cap = p->seg_cap;
+    a.num_tiles = p->num_tiles;
+    a.epoch = p->epoch;
+    a.max_indices = static_cast<uint32_t>(p->max_indices);
+    cudaError_t e = launch_plan(a, s);
+    if (e != cudaSuccess) return cuda_fail(e, "plan kernel launch");
+    p->built = true;
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims, dpi_dtype_t dtype,
+                      const int32_t* lengths_dev, int32_t B, int64_t max_indices, void* stream, dpi_plan_t** plan) {
+    dpi_status_t st = dpi_plan_create(T, table_rows, dims, dtype, B, max_indices, plan);
+    if (st != DPI_OK) return st;
+    st = dpi_plan_build(*plan, lengths_dev, stream);
+    if (st != DPI_OK) {
+        dpi_plan_destroy(*plan);
+        *plan = nullptr;
+    }
+    return st;
+}
+
+dpi_status_t dpi_plan_device_views(const dpi_plan_t* p, const int32_t** offsets_dev, const int32_t** seg_bag_dev,
+                                   const int32_t** meta_dev) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (offsets_dev) *offsets_dev = p->offsets;
+    if (seg_bag_dev) *seg_bag_dev = p->seg_bag;
+    if (meta_dev) *meta_dev = p->meta;
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_info(const dpi_plan_t* p, int32_t* T, int32_t* B, int32_t* D, int32_t* dtype, int64_t* G,
+                           int32_t* K, int64_t* seg_capacity) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (T) *T = p->T;
+    if (B) *B = p->B;
+    if (D) *D = p->D;
+    if (dtype) *dtype = static_cast<int32_t>(p->dtype);
+    if (G) *G = p->G;
+    if (K) *K = p->K;
+    if (seg_capacity) *seg_capacity = p->seg_cap;
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_export(const dpi_plan_t* p, int32_t* offsets_host, int32_t* seg_bag_host, int64_t seg_cap,
+                             int32_t* S, int64_t* N, void* stream) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int32_t meta[kMetaWords];
+    DPI_CUDA(cudaMemcpyAsync(meta, p->meta, sizeof meta, cudaMemcpyDeviceToHost, s));
+    DPI_CUDA(cudaStreamSynchronize(s));
+    if (meta[META_OVERFLOW]) return fail(DPI_ERR_INVALID_ARG, "batch has N=%u > max_indices=%lld (plan capacity exceeded)", static_cast<uint32_t>(meta[META_N]), (long long)p->max_indices);
+    if (S) *S = meta[META_S];
+    if (N) *N = static_cast<uint32_t>(meta[META_N]);
+    if (offsets_host) DPI_CUDA(cudaMemcpyAsync(offsets_host, p->offsets, (static_cast<size_t>(p->G) + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    if (seg_bag_host) {
+        if (seg_cap < static_cast<int64_t>(meta[META_S]) + 1) return fail(DPI_ERR_INVALID_ARG, "seg_cap=%lld < S+1=%d", (long long)seg_cap, meta[META_S] + 1);
+        DPI_CUDA(cudaMemcpyAsync(seg_bag_host, p->seg_bag, (static_cast<size_t>(meta[META_S]) + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    }
+    DPI_CUDA(cudaStreamSynchronize(s));
+    return DPI_OK;
+}
+
+dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,
+                        const dpi_plan_t* p, const uint8_t* pooling, void* out_dev, void* stream) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built (call dpi_plan_build first)");
+    if (!table_ptrs_dev || !out_dev) return fail(DPI_ERR_INVALID_ARG, "table_ptrs_dev/out_dev is NULL");
+    if (!indices_dev && p->max_indices > 0) return fail(DPI_ERR_INVALID_ARG, "indices_dev is NULL");
+    if (reinterpret_cast<uintptr_t>(out_dev) & 15u) return fail(DPI_ERR_INVALID_ARG, "out_dev is not 16-byte aligned");
+    if (reinterpret_cast<uintptr_t>(indices_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "indices_dev is not 4-byte aligned");
+    return do_lookup(p, table_ptrs_dev, indices_dev, offsets_dev, pooling, out_dev, static_cast<cudaStream_t>(stream));
+}
+
+dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, const int32_t* lengths_host,
+                              const int32_t* indices_host, int64_t n_indices, const uint8_t* pooling, void* out_host,
+                              void* stream) {
+    if (!p || !table_ptrs_dev || !lengths_host || !out_host) return fail(DPI_ERR_INVALID_ARG, "NULL argument");
+    if (n_indices < 0 || n_indices > p->max_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld outside [0, max_indices=%lld]", (long long)n_indices, (long long)p->max_indices);
+    if (n_indices > 0 && !indices_host) return fail(DPI_ERR_INVALID_ARG, "indices_host is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t out_bytes = static_cast<size_t>(p->G) * p->nvec * 16;
+    if (!p->stage_len) DPI_CUDA(cudaMalloc(&p->stage_len, static_cast<size_t>(p->G) * sizeof(int32_t)));
+    if (!p->stage_idx) DPI_CUDA(cudaMalloc(&p->stage_idx, (static_cast<size_t>(p->max_indices) + 4) * sizeof(int32_t)));
+    if (!p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, out_bytes));
+    DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+    if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+    dpi_status_t st = dpi_plan_build(p, p->stage_len, s);
+    if (st != DPI_OK) return st;
+    st = do_lookup(p, table_ptrs_dev, p->stage_idx, nullptr, pooling, p->stage_out, s);
+    if (st != DPI_OK) return st;
+    DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
+    DPI_CUDA(cudaStreamSynchronize(s));
+    return DPI_OK;
+}
+
+dpi_status_t dpi_check_indices(const dpi_plan_t* p, const int32_t* indices_dev, int64_t* n_bad, void* stream) {
+    if (!p || !n_bad) return fail(DPI_ERR_INVALID_ARG, "NULL argument");
+    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    DPI_CUDA(cudaMemsetAsync(p->n_bad_dev, 0, sizeof(unsigned long long), s));
+    CheckArgs a{};
+    a.indices = indices_dev;
+    a.offsets = p->offsets;
+    a.table_rows = p->table_rows_dev;
+    a.n_bad = p->n_bad_dev;
+    a.G = p->G;
+    a.T = static_cast<uint32_t>(p->T);
+    cudaError_t e = launch_check_indices(a, s);
+    if (e != cudaSuccess) return cuda_fail(e, "check_indices launch");
+    unsigned long long bad = 0;
+    DPI_CUDA(cudaMemcpyAsync(&bad, p->n_bad_dev, sizeof bad, cudaMemcpyDeviceToHost, s));
+    DPI_CUDA(cudaStreamSynchronize(s));
+    *n_bad = static_cast<int64_t>(bad);
+    if (bad) return fail(DPI_ERR_INDEX_RANGE, "%llu indices outside [0, table_rows[t])", bad);
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_destroy(dpi_plan_t* p) {
+    if (!p) return DPI_OK;
+    free_plan(p);
+    return DPI_OK;
+}
+
+int64_t dpi_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+int32_t dpi_version(void) { return DPI_VERSION; }
+
+const char* dpi_status_string(dpi_status_t st) {
+    switch (st) {
+        case DPI_OK: return "DPI_OK";
+        case DPI_ERR_INVALID_ARG: return "DPI_ERR_INVALID_ARG";
+        case DPI_ERR_UNSUPPORTED: return "DPI_ERR_UNSUPPORTED";
+        case DPI_ERR_ALLOC: return "DPI_ERR_ALLOC";
+        case DPI_ERR_CUDA: return "DPI_ERR_CUDA";
+        case DPI_ERR_INDEX_RANGE: return "DPI_ERR_INDEX_RANGE";
+        default: return "DPI_ERR_UNKNOWN";
+    }
+}
+
+const char* dpi_last_error(void) { return g_err; }
+
+}  // extern "C"

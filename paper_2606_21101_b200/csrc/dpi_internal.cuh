@@ -1,0 +1,93 @@
+// dpi_internal.cuh -- shared declarations of libdpi (sm_100a only). Not part of the public boundary.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+#include "../../include/dpi.h"
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "libdpi is written for sm_100a (B200) only"
+#endif
+
+namespace dpi {
+
+constexpr int kMetaWords = 8;  // meta_dev layout: {S, N, C[G] (low 32), overflow, K, G, 0, 0}
+enum MetaSlot { META_S = 0, META_N = 1, META_C = 2, META_OVERFLOW = 3, META_K = 4, META_G = 5 };
+
+constexpr int kPoolWords = DPI_MAX_TABLES / 32;
+struct PoolMask {
+    uint32_t w[kPoolWords];  // bit t set -> table t is mean-pooled
+};
+
+// ---- planner (plan_kernels.cu) ---------------------------------------------------------------------
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 8;                               // consecutive bags per thread (two int4 loads)
+constexpr int kScanTile = kScanThreads * kScanItems;        // 2048 bags per CTA
+
+struct PlanArgs {
+    const int32_t* __restrict__ len;   // [G]
+    int32_t* __restrict__ offsets;     // [G+1]
+    int32_t* __restrict__ seg_bag;     // [seg_cap]
+    int32_t* __restrict__ meta;        // [kMetaWords]
+    unsigned long long* tile_len;      // [num_tiles] look-back status words for the length scan
+    unsigned long long* tile_cost;     // [num_tiles] look-back status words for the cost scan
+    unsigned int* ticket;              // dynamic tile id (self-resetting atomicInc)
+    uint32_t G;
+    uint32_t K;
+    uint32_t seg_cap;
+    uint32_t num_tiles;
+    uint32_t epoch;                    // tags status words so the arrays never need clearing
+    uint32_t max_indices;
+};
+
+cudaError_t launch_plan(const PlanArgs& a, cudaStream_t stream);
+
+struct CheckArgs {
+    const int32_t* __restrict__ indices;
+    const int32_t* __restrict__ offsets;
+    const int64_t* __restrict__ table_rows;  // device [T]
+    unsigned long long* n_bad;
+    uint32_t G;
+    uint32_t T;
+};
+cudaError_t launch_check_indices(const CheckArgs& a, cudaStream_t stream);
+
+// ---- lookup (lookup_*.cu) --------------------------------------------------------------------------
+struct LookupArgs {
+    const void* const* __restrict__ tables;  // device [T] table base pointers
+    const int32_t* __restrict__ indices;     // [N]
+    const int32_t* __restrict__ offsets;     // [G+1]
+    const int32_t* __restrict__ seg_bag;     // [S+1]
+    const int32_t* __restrict__ meta;        // meta[META_S] = S
+    void* __restrict__ out;                  // [G * D] in table dtype  (out[b, t*D + c] == out[g*D + c])
+    uint32_t G;
+    uint32_t T;
+    uint32_t nvec;                           // 16-byte vectors per row = D*sizeof(elt)/16
+    int32_t mode;                            // 0 auto, 1 sub-warp per bag, 2 warp per bag
+    int32_t row_no_alloc;                    // 1: rows bypass L1
+    PoolMask pool;
+};
+
+struct LookupLaunch {
+    int lanes;          // lanes per row (power of two >= nvec)
+    int unroll;         // 2, 4, 8, 16
+    int block_threads;  // 128, 256, 512
+    int grid;           // persistent grid size
+    bool pdl;           // programmatic dependent launch
+};
+
+// Each returns cudaErrorInvalidValue when (lanes, unroll, block_threads) has no instantiation.
+cudaError_t launch_lookup_f32(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
+cudaError_t launch_lookup_f16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
+cudaError_t launch_lookup_bf16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
+// Max resident CTAs per SM of the instantiation (0 if none).
+int lookup_occupancy_f32(int lanes, int unroll, int block_threads);
+int lookup_occupancy_f16(int lanes, int unroll, int block_threads);
+int lookup_occupancy_bf16(int lanes, int unroll, int block_threads);
+
+void count_launch();
+
+}  // namespace dpi

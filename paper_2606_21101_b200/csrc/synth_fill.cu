@@ -1,0 +1,75 @@
+// synth_fill.cu -- libdpi_synth.so: device-side fill of synthetic embedding tables (bench/tests only).
+//
+// NOT part of the method: this is the input generator of workloads.py restated for the device, so that an
+// 82 GB table set can be created in place (the host cannot mirror it). Same counter-based recipe:
+//   h = fmix64(key + i*GAMMA),  i = r*D + c,   x = float(h >> 40) * 2^-24,   v = (x - 0.5f) * 0.1f
+// then one RNE cast to the table dtype. tests/test_gpu_synth.py checks host/device equality bit for bit.
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+namespace {
+
+__device__ __forceinline__ unsigned long long fmix64(unsigned long long z) {
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+__device__ __forceinline__ float value_at(unsigned long long key, unsigned long long i) {
+    const unsigned long long h = fmix64(key + i * 0x9E3779B97F4A7C15ull);
+    const float x = __uint2float_rn(static_cast<unsigned int>(h >> 40)) * 5.9604644775390625e-08f;  // 2^-24, exact
+    return __fmul_rn(__fsub_rn(x, 0.5f), 0.1f);
+}
+
+// one thread = 16 bytes of output
+template <int DT>
+__global__ void __launch_bounds__(256) fill_kernel(void* __restrict__ dst, unsigned long long n_elems,
+                                                   unsigned long long key) {
+    constexpr int kPer = DT == 0 ? 4 : 8;
+    const unsigned long long n_vec = n_elems / kPer;
+    for (unsigned long long v = blockIdx.x * static_cast<unsigned long long>(blockDim.x) + threadIdx.x; v < n_vec;
+         v += static_cast<unsigned long long>(gridDim.x) * blockDim.x) {
+        float f[kPer];
+#pragma unroll
+        for (int k = 0; k < kPer; ++k) f[k] = value_at(key, v * kPer + k);
+        uint4 o;
+        if (DT == 0) {
+            o = make_uint4(__float_as_uint(f[0]), __float_as_uint(f[1]), __float_as_uint(f[2]), __float_as_uint(f[3]));
+        } else {
+            uint32_t w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if (DT == 1) {
+                    const __half2 h = __floats2half2_rn(f[2 * k], f[2 * k + 1]);
+                    w[k] = *reinterpret_cast<const uint32_t*>(&h);
+                } else {
+                    const __nv_bfloat162 h = __floats2bfloat162_rn(f[2 * k], f[2 * k + 1]);
+                    w[k] = *reinterpret_cast<const uint32_t*>(&h);
+                }
+            }
+            o = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+        reinterpret_cast<uint4*>(dst)[v] = o;
+    }
+}
+
+}  // namespace
+
+// dst: device pointer, 16-byte aligned, n_elems = rows*D elements with (n_elems * sizeof(elt)) % 16 == 0.
+// dtype: 0 f32, 1 f16, 2 bf16.  Returns the cudaError_t value (0 = success). Asynchronous on `stream`.
+extern "C" int dpi_synth_fill_table(void* dst, uint64_t n_elems, int dtype, uint64_t key, void* stream) {
+    if (!dst || dtype < 0 || dtype > 2 || (reinterpret_cast<uintptr_t>(dst) & 15u)) return (int)cudaErrorInvalidValue;
+    const int per = dtype == 0 ? 4 : 8;
+    if (n_elems % per) return (int)cudaErrorInvalidValue;
+    if (n_elems == 0) return 0;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const unsigned long long n_vec = n_elems / per;
+    const unsigned int blocks = static_cast<unsigned int>(n_vec / 256 + 1 < 148ull * 16 ? n_vec / 256 + 1 : 148ull * 16);
+    switch (dtype) {
+        case 0: fill_kernel<0><<<blocks, 256, 0, s>>>(dst, n_elems, key); break;
+        case 1: fill_kernel<1><<<blocks, 256, 0, s>>>(dst, n_elems, key); break;
+        default: fill_kernel<2><<<blocks, 256, 0, s>>>(dst, n_elems, key); break;
+    }
+    return (int)cudaGetLastError();
+}

@@ -1,0 +1,46 @@
+"""Shared helpers of the GPU parity tests: the comparison rule of BASELINE.json's north_star and a driver
+that runs the CUDA path through the C ABI (binding) and the oracle on the same seeded inputs."""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle
+from paper_2606_21101_b200 import workloads as W
+
+
+def host_offsets(lengths: np.ndarray) -> np.ndarray:
+    """Layout helper for handing bags to the oracle (numpy cumsum; the oracle's own plan is checked elsewhere)."""
+    return np.concatenate(([0], np.cumsum(np.asarray(lengths, dtype=np.int64)))).astype(np.int32)
+
+
+def assert_outputs_match(gpu_f64: np.ndarray, ref: np.ndarray, lengths: np.ndarray, T: int, D: int, dtype: str):
+    """north_star: fp32 tables max|err| <= 1e-5 * bag length; fp16/bf16 <= 2e-3 relative (fp32 accumulate),
+    with the absolute floor 1e-6*L for cancellation. Against the UNROUNDED float64 reference.
+    Bit-exact when L <= 1; an empty bag is exactly +0.0."""
+    B = ref.shape[0]
+    g = gpu_f64.reshape(B * T, D)
+    r = ref.reshape(B * T, D)
+    L = np.asarray(lengths, dtype=np.int64).reshape(B * T)
+    assert not np.isnan(g).any(), "an output element was never written (NaN sentinel survived)"
+    err = np.abs(g - r)
+    Lm = np.maximum(L, 1).astype(np.float64)[:, None]
+    if dtype == "f32":
+        tol = 1e-5 * Lm * np.ones_like(r)
+    else:
+        tol = np.maximum(2e-3 * np.abs(r), 1e-6 * Lm)
+    bad = err > tol
+    assert not bad.any(), (f"{int(bad.sum())} elements out of tolerance; worst err {err.max():.3e} at bag "
+                           f"{int(np.argmax(err.max(axis=1)))} (L={int(L[np.argmax(err.max(axis=1))])})")
+    short = L <= 1
+    if dtype == "f32":
+        assert np.array_equal(g[short], r[short]), "bags of length <= 1 must be bit-exact (Alg. 1 is a copy)"
+    else:
+        # the reference is unrounded float64 of 16-bit values: a single row is exactly representable
+        assert np.array_equal(g[short], r[short]), "bags of length <= 1 must be bit-exact"
+    empty = L == 0
+    assert not g[empty].any() and not np.signbit(g[empty]).any(), "empty bag must be +0.0"
+    return float(err.max()) if err.size else 0.0
+
+
+def oracle_reference(host_tables, dtype: str, B: int, lengths: np.ndarray, indices: np.ndarray, pooling: np.ndarray):
+    return oracle.lookup(host_tables, W.DTYPE_CODE[dtype], B, indices, host_offsets(lengths), pooling)

@@ -1,0 +1,304 @@
+"""GPU parity tests proper (`-m gpu`): the CUDA path, called through the C ABI, against the CPU oracle on the
+same seeded inputs. Plan: bit-exact. Outputs: north_star tolerances (tests/parity.py)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_21101_b200 import binding, harness, workloads as W
+from tests.parity import assert_outputs_match, host_offsets, oracle_reference
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    from paper_2606_21101_b200 import build
+    build.build()
+    binding.load_library()
+    harness.require_cuda()
+
+
+# --------------------------------------------------------------------------------------------------
+# generator: host and device implementations of the same counter-based recipe agree bit for bit
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f32", "f16", "bf16"])
+def test_synth_fill_matches_host_generator(dtype):
+    cfg = W.Config("g", 2, (3001, 517), 32, dtype, 4, ("const", 1), ("uniform",), "sum", seed=5)
+    dt = harness.make_device_tables(cfg)
+    for t in range(cfg.T):
+        want = W.full_table_storage(cfg, t, int(dt.rows[t]))
+        got = dt.tables[t].cpu()
+        got = got.view(torch.int16).numpy().view(np.uint16) if dtype != "f32" else got.numpy()
+        want = want.view(np.uint16) if dtype != "f32" else want
+        assert np.array_equal(got, want)
+
+
+# --------------------------------------------------------------------------------------------------
+# plan (a1 + a2): bit-exact
+# --------------------------------------------------------------------------------------------------
+def _plan_parity(lengths: np.ndarray, T: int, B: int, K: int, max_indices=None):
+    N = int(lengths.astype(np.int64).sum())
+    plan = binding.Plan([10] * T, 16, binding.DPI_F32, B, N if max_indices is None else max_indices)
+    plan.set_quantum(K)
+    dev = torch.from_numpy(np.ascontiguousarray(lengths, dtype=np.int32)).cuda()
+    for _ in range(2):  # the second build reuses the look-back status words (epoch tagging)
+        plan.build(dev)
+        off, seg, S, n = plan.export()
+        o_off, o_seg, o_S = oracle.plan(lengths, K)
+        assert n == N and S == o_S
+        assert np.array_equal(off, o_off)
+        assert np.array_equal(seg, o_seg)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("K", [1, 3, 32, 64, 1000])
+def test_plan_small_ragged(K):
+    rng = np.random.default_rng(K)
+    for T, B in [(1, 1), (3, 7), (4, 128), (5, 1000), (7, 2049 // 7 + 1)]:
+        ln = rng.integers(0, 9, size=T * B).astype(np.int32)
+        _plan_parity(ln, T, B, K)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4", "c5"])
+@pytest.mark.parametrize("K", [32, 48])
+def test_plan_full_size_configs(name, K):
+    cfg = W.CONFIGS[name]
+    ln = W.make_lengths(cfg, cfg.seed)
+    _plan_parity(ln, cfg.T, cfg.B, K)
+
+
+def test_plan_degenerate_cases():
+    _plan_parity(np.zeros(5000, np.int32), 5, 1000, 32)               # all empty
+    _plan_parity(np.array([100000], np.int32), 1, 1, 32)              # one long bag spans many quanta
+    ln = np.zeros(4099, np.int32); ln[0] = 7; ln[-1] = 900; ln[2048] = 33
+    _plan_parity(ln, 1, 4099, 16)                                     # tile boundaries, ragged tail
+    _plan_parity(np.full(2048 * 3, 1, np.int32), 3, 2048, 32)         # exact multiple of the scan tile
+    _plan_parity(np.full(10, 64, np.int32), 2, 5, 7)                  # K does not divide anything
+
+
+def test_plan_many_tiles_lookback_window():
+    """More than 32 tiles behind: the look-back window has to slide."""
+    rng = np.random.default_rng(3)
+    B, T = 40000, 5  # 200000 bags = 98 tiles
+    ln = rng.integers(0, 5, size=B * T).astype(np.int32)
+    _plan_parity(ln, T, B, 32)
+
+
+def test_plan_overflow_is_reported_not_out_of_bounds():
+    ln = np.full(100, 10, np.int32)
+    plan = binding.Plan([10], 16, binding.DPI_F32, 100, 500)  # capacity 500 < N = 1000
+    plan.build(torch.from_numpy(ln).cuda())
+    with pytest.raises(binding.DpiError) as e:
+        plan.export()
+    assert e.value.status == 1 and "max_indices" in e.value.detail
+
+
+# --------------------------------------------------------------------------------------------------
+# lookup (a3)
+# --------------------------------------------------------------------------------------------------
+def _run_gpu(cfg, dt, batch, pooling, K=0, opts=None, via_explicit_offsets=False):
+    db = harness.upload_batch(batch)
+    plan = harness.make_plan(cfg, dt.rows, max(batch.N, 1))
+    if K:
+        plan.set_quantum(K)
+    for k, v in (opts or {}).items():
+        plan.set_option(k, v)
+    plan.build(db.lengths)
+    assert plan.check_indices(db.indices) == 0
+    out = harness.new_output(cfg, fill_nan=True)
+    off_dev = None
+    if via_explicit_offsets:
+        off_dev = torch.from_numpy(host_offsets(batch.lengths)).cuda()
+    plan.lookup(dt.ptrs, db.indices, out, pooling=pooling, offsets_dev=off_dev)
+    torch.cuda.synchronize()
+    res = harness.out_to_f64(out)
+    plan.destroy()
+    return res
+
+
+def _full_parity(cfg, K=0, opts=None, batch_seed=None, pooling=None):
+    rows = cfg.table_rows()
+    host_tables = [W.full_table_storage(cfg, t, int(rows[t])) for t in range(cfg.T)]
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, rows, batch_seed)
+    pooling = cfg.pooling_modes() if pooling is None else pooling
+    got = _run_gpu(cfg, dt, batch, pooling, K, opts)
+    ref = oracle_reference(host_tables, cfg.dtype, cfg.B, batch.lengths, batch.indices, pooling)
+    return assert_outputs_match(got, ref, batch.lengths, cfg.T, cfg.D, cfg.dtype)
+
+
+def test_c1_exact_config():
+    _full_parity(W.C1)
+
+
+@pytest.mark.parametrize("dtype,D", [("f32", 4), ("f32", 16), ("f32", 24), ("f32", 64), ("f32", 128),
+                                     ("f16", 8), ("f16", 32), ("f16", 72), ("f16", 256),
+                                     ("bf16", 8), ("bf16", 64), ("bf16", 128), ("bf16", 256)])
+@pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 1, 4), ("poisson", 20.0, 100, 0.05)])
+def test_shapes_dtypes_and_length_mixes(dtype, D, lengths):
+    """Several tiles, a ragged tail, every lanes-per-row instantiation (incl. non-power-of-two row sizes),
+    mixed sum/mean pooling, empty bags."""
+    cfg = W.Config("s", 5, (1000, 17, 4000, 1, 250), D, dtype, 333, lengths, ("zipf", 1.05), "half", seed=11)
+    _full_parity(cfg)
+
+
+@pytest.mark.parametrize("unroll", [2, 4, 8, 16])
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_every_kernel_variant_gives_the_same_answer(unroll, mode):
+    cfg = W.Config("v", 6, (500, 30, 2000, 7, 100, 1000), 64, "f32", 257, ("uniform", 0, 70), ("uniform",), "half", 3)
+    _full_parity(cfg, K=32, opts={binding.OPT_UNROLL: unroll, binding.OPT_MODE: mode})
+    cfg16 = cfg.scaled(dtype="bf16", D=32, lengths=("uniform", 0, 5))
+    _full_parity(cfg16, K=16, opts={binding.OPT_UNROLL: unroll, binding.OPT_MODE: mode, binding.OPT_BLOCK_THREADS: 128})
+
+
+@pytest.mark.parametrize("K", [1, 5, 32, 200, 100000])
+def test_any_quantum_gives_the_same_answer(K):
+    cfg = W.Config("k", 3, (100, 1000, 10), 32, "f16", 500, ("poisson", 6.0, 40, 0.2), ("zipf", 1.2), "mean", 4)
+    _full_parity(cfg, K=K)
+
+
+def test_degenerate_inputs():
+    # all bags empty -> zero matrix, N = 0
+    cfg = W.Config("e", 3, (5, 5, 5), 16, "f32", 64, ("const", 0), ("uniform",), "mean", 0)
+    _full_parity(cfg)
+    # single sample, single table, one long bag (spans many quanta)
+    cfg = W.Config("l", 1, (1000,), 64, "f32", 1, ("const", 5000), ("uniform",), "mean", 0)
+    _full_parity(cfg, K=32)
+    # B = 1, many tables
+    cfg = W.Config("b1", 100, ("loguniform", 10, 1000), 16, "bf16", 1, ("uniform", 0, 3), ("uniform",), "half", 2)
+    _full_parity(cfg)
+    # one-row tables: every index is 0
+    cfg = W.Config("r1", 4, (1, 1, 1, 1), 32, "f32", 77, ("uniform", 0, 9), ("uniform",), "sum", 2)
+    _full_parity(cfg)
+
+
+def test_first_and_last_bag_empty_and_explicit_offsets():
+    cfg = W.Config("x", 2, (50, 60), 16, "f32", 40, ("uniform", 1, 4), ("uniform",), "sum", 9)
+    rows = cfg.table_rows()
+    host_tables = [W.full_table_storage(cfg, t, int(rows[t])) for t in range(cfg.T)]
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, rows)
+    ln = batch.lengths.copy()
+    off = host_offsets(ln)
+    keep = np.ones(batch.N, bool)
+    keep[off[0]:off[1]] = False
+    keep[off[-2]:off[-1]] = False
+    ln[0] = 0
+    ln[-1] = 0
+    b2 = W.Batch(ln, batch.indices[keep])
+    pooling = np.array([1, 0], np.uint8)
+    got = _run_gpu(cfg, dt, b2, pooling, via_explicit_offsets=True)
+    ref = oracle_reference(host_tables, cfg.dtype, cfg.B, b2.lengths, b2.indices, pooling)
+    assert_outputs_match(got, ref, b2.lengths, cfg.T, cfg.D, cfg.dtype)
+
+
+def test_onehot_is_alg1_bit_exact_with_index_encoding_tables():
+    """Alg. 1: every output element decodes to its own (t, IDs[b,t], c)."""
+    T, B, D = 7, 1000, 16
+    rows = [7, 300, 1, 4095, 64, 4096, 33]
+    tables = [(t * 65536 + np.arange(rows[t])[:, None] * 16 + np.arange(D)[None, :]).astype(np.float32)
+              for t in range(T)]
+    cfg = W.Config("enc", T, tuple(rows), D, "f32", B, ("const", 1), ("uniform",), "sum", 1)
+    dt = harness.tables_from_host(cfg, tables)
+    batch = W.make_batch(cfg, np.asarray(rows, np.int64))
+    got = _run_gpu(cfg, dt, batch, np.zeros(T, np.uint8)).astype(np.int64).reshape(B, T, D)
+    ids = batch.indices.reshape(B, T)
+    assert np.array_equal(got >> 16, np.broadcast_to(np.arange(T)[None, :, None], (B, T, D)))
+    assert np.array_equal((got >> 4) & 0xFFF, np.broadcast_to(ids[:, :, None], (B, T, D)))
+    assert np.array_equal(got & 0xF, np.broadcast_to(np.arange(D)[None, None, :], (B, T, D)))
+    want = oracle.alg1_onehot(tables, oracle.F32, ids)
+    assert np.array_equal(got.reshape(B, T * D).astype(np.float64), want)
+
+
+@pytest.mark.parametrize("dtype", ["f16", "bf16"])
+def test_16bit_exactly_representable_values_are_bit_exact(dtype):
+    rng = np.random.default_rng(10)
+    T, B, D = 3, 300, 32
+    rows = [12, 100, 5]
+    ks = [rng.integers(-3, 4, size=(rows[t], D)) for t in range(T)]
+    host_tables = [W.to_storage((k / 1024.0).astype(np.float32), dtype) for k in ks]
+    cfg = W.Config("x16", T, tuple(rows), D, dtype, B, ("uniform", 0, 64), ("uniform",), "sum", 6)
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, np.asarray(rows, np.int64))
+    got = _run_gpu(cfg, dt, batch, np.zeros(T, np.uint8))
+    ref = oracle_reference(host_tables, dtype, B, batch.lengths, batch.indices, np.zeros(T, np.uint8))
+    assert np.array_equal(got, ref)
+
+
+def test_check_indices_counts_out_of_range():
+    cfg = W.Config("oob", 2, (10, 20), 16, "f32", 8, ("const", 2), ("uniform",), "sum", 0)
+    batch = W.make_batch(cfg)
+    idx = batch.indices.copy()
+    idx[0] = 10      # table 0 has rows 0..9
+    idx[3] = -1
+    idx[5] = 19      # fine for table 0? entry 5 belongs to bag 2 = (b=1,t=0) -> 19 >= 10 is bad
+    db = harness.upload_batch(W.Batch(batch.lengths, idx))
+    plan = harness.make_plan(cfg, cfg.table_rows(), batch.N)
+    plan.build(db.lengths)
+    assert plan.check_indices(db.indices) == 3
+    plan.destroy()
+
+
+def test_forward_host_equals_device_path():
+    cfg = W.Config("h", 4, (100, 2000, 50, 7), 32, "bf16", 513, ("uniform", 0, 6), ("zipf", 1.1), "half", 8)
+    rows = cfg.table_rows()
+    host_tables = [W.full_table_storage(cfg, t, int(rows[t])) for t in range(cfg.T)]
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, rows)
+    pooling = cfg.pooling_modes()
+    dev = _run_gpu(cfg, dt, batch, pooling)
+    plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg))
+    ln = torch.from_numpy(batch.lengths).pin_memory()
+    idx = torch.from_numpy(batch.indices).pin_memory()
+    out = torch.empty((cfg.B, cfg.T * cfg.D), dtype=torch.bfloat16).pin_memory()
+    plan.forward_host(dt.ptrs, ln, idx, out, pooling=pooling)
+    assert np.array_equal(out.double().numpy(), dev)
+    plan.destroy()
+
+
+# --------------------------------------------------------------------------------------------------
+# BASELINE.json configs at full size, in the launch configuration bench.py times (library defaults)
+# --------------------------------------------------------------------------------------------------
+def _sampled_full_size(cfg, n_samples, rotate=1):
+    dt = harness.make_device_tables(cfg)
+    rng = np.random.default_rng(123)
+    worst = 0.0
+    for r in range(rotate):
+        batch = W.make_batch(cfg, dt.rows, cfg.seed + r)
+        pooling = cfg.pooling_modes()
+        got = _run_gpu(cfg, dt, batch, pooling)
+        # properties that hold at any size: written everywhere, empty bags are +0.0
+        L = batch.lengths.reshape(cfg.B, cfg.T)
+        g3 = got.reshape(cfg.B, cfg.T, cfg.D)
+        assert not np.isnan(got).any()
+        assert not g3[L == 0].any()
+        samples = np.sort(rng.choice(cfg.B, size=min(n_samples, cfg.B), replace=False))
+        samples[0] = 0
+        samples[-1] = cfg.B - 1  # both ends of the batch (first and last warp-task)
+        sub = W.compact_subproblem(cfg, batch, samples)
+        ref = oracle.lookup(sub.tables, W.DTYPE_CODE[cfg.dtype], len(samples), sub.indices,
+                            host_offsets(sub.lengths), pooling)
+        worst = max(worst, assert_outputs_match(got[samples], ref, sub.lengths, cfg.T, cfg.D, cfg.dtype))
+    del dt
+    torch.cuda.empty_cache()
+    return worst
+
+
+def test_c2_full_size_every_sample():
+    _sampled_full_size(W.C2, W.C2.B, rotate=2)
+
+
+def test_c3_full_size_every_sample():
+    _sampled_full_size(W.C3, W.C3.B)
+
+
+def test_c4_full_size_sampled():
+    _sampled_full_size(W.C4, 512)
+
+
+def test_c5_full_size_sampled():
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.fail(f"config 5 needs ~82 GB of tables; only {free / 1e9:.0f} GB free on this device")
+    _sampled_full_size(W.C5, 4096)
