@@ -307,7 +307,7 @@ def run_ours(args):
     if not args.no_e2e:
         hb = [(torch.from_numpy(b.host.lengths).pin_memory(), torch.from_numpy(np.ascontiguousarray(b.host.indices)).pin_memory())
               for b in batches[:2]]
-        out_host = torch.empty((cfg.B, cfg.T * cfg.D), dtype=harness.TORCH_DTYPE[cfg.dtype]).pin_memory()
+        out_host = torch.empty((cfg.B, cfg.T * cfg.D), dtype=harness.TORCH_DTYPE[cfg.out]).pin_memory()
         for i in range(2):
             plan.forward_host(dt.ptrs, hb[i % 2][0], hb[i % 2][1], out_host, pooling=pooling, stream=stream)
         barrier()

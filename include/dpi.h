@@ -20,7 +20,8 @@
  *   C[0] = 0,       C[g+1] = C[g] + max(len[g], 1)
  *   S = ceil(C[G] / K)
  *   seg_bag[s] = min(G, min{ g in [0,G] : C[g] >= s*K })   for s = 0..S
- *   warp-task s owns bags [seg_bag[s], seg_bag[s+1]).
+ *   seg_off[s] = offsets[seg_bag[s]]                       (first index entry of task s)
+ *   warp-task s owns bags [seg_bag[s], seg_bag[s+1]) = entries [seg_off[s], seg_off[s+1]).
  *
  * Lookup definition: for every bag g = (b,t), c < D
  *   acc[c] = sum_{j in [offsets[g], offsets[g+1])} float(table_t[indices[j]][c])     (fp32 accumulate)
@@ -82,13 +83,18 @@ typedef enum {
  *   table_rows   host int64[T], heights n_t >= 1; copied
  *   dims         host int32[T], embedding dim of each table; v1 requires all equal (R10) and
  *                D*sizeof(dtype) a multiple of 16 B and <= 512 B, else DPI_ERR_UNSUPPORTED
- *   dtype        storage type of tables AND of the output
+ *   dtype        storage type of the tables and, by default, of the output
  *   B            samples per batch >= 1;  G = B*T must be < 2^31
  *   max_indices  upper bound on N for any batch built with this plan, 0 <= max_indices < 2^31
  *   plan         receives the handle; destroy with dpi_plan_destroy
  */
 dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t* dims, dpi_dtype_t dtype,
                              int32_t B, int64_t max_indices, dpi_plan_t** plan);
+
+/* Output element type of dpi_lookup: the table dtype (default) or DPI_F32. bf16 has 8 significand bits, so a
+ * correctly rounded bf16 output carries up to 2^-8 = 3.9e-3 relative error by itself; fp32 output keeps the
+ * fp32 accumulator (R6). Anything else -> DPI_ERR_UNSUPPORTED. */
+dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* plan, dpi_dtype_t out_dtype);
 
 /* Cost quantum K >= 1 of the balanced segments (0 = library default for this row size). Takes effect at the
  * next dpi_plan_build. DPI_ERR_INVALID_ARG if K < 0. */
@@ -102,7 +108,7 @@ dpi_status_t dpi_plan_get_option(const dpi_plan_t* plan, dpi_option_t opt, int32
  * dpi_plan_build -- steps a1 + a2 on the device, asynchronous on `stream`, ONE kernel launch for all
  * (sample, table) bags (no per-table launches, no host synchronisation):
  *   lengths_dev  device int32[G], len[g] >= 0, g = b*T + t, 4-byte aligned
- * Writes the plan's offsets[G+1], seg_bag[S+1] and S (device memory). If the batch has N > max_indices
+ * Writes the plan's offsets[G+1], {seg_bag, seg_off}[S+1] and S (device memory). If the batch has N > max_indices
  * the device sets an overflow flag that dpi_plan_export / dpi_plan_stats report (DPI_ERR_INVALID_ARG);
  * seg_bag writes beyond the capacity are suppressed, never out of bounds.
  */
@@ -114,21 +120,21 @@ dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims,
                       dpi_plan_t** plan);
 
 /* Borrowed device pointers into the plan, valid until the next build/destroy. Any out-pointer may be NULL.
- *   offsets_dev int32[G+1]; seg_bag_dev int32[seg_capacity]; meta_dev int32[8] = {S, N, C[G] low 32 bits,
- *   overflow flag, K, G, 0, 0}. */
+ *   offsets_dev int32[G+1]; seg_dev int32[2*seg_capacity], interleaved pairs {seg_bag[s], seg_off[s]};
+ *   meta_dev int32[8] = {S, N, C[G] low 32 bits, overflow flag, K, G, 0, 0}. */
 dpi_status_t dpi_plan_device_views(const dpi_plan_t* plan, const int32_t** offsets_dev,
-                                   const int32_t** seg_bag_dev, const int32_t** meta_dev);
+                                   const int32_t** seg_dev, const int32_t** meta_dev);
 
 /* Static facts about a plan (host only, no synchronisation). Any out-pointer may be NULL. */
 dpi_status_t dpi_plan_info(const dpi_plan_t* plan, int32_t* T, int32_t* B, int32_t* D, int32_t* dtype,
                            int64_t* G, int32_t* K, int64_t* seg_capacity);
 
 /* Parity/debug: synchronises `stream`, copies the plan to caller-owned host arrays.
- *   offsets_host int32[G+1] (may be NULL); seg_bag_host int32[seg_cap] receives S+1 entries (may be NULL);
- *   S, N receive the segment count and total index count (may be NULL).
+ *   offsets_host int32[G+1] (may be NULL); seg_bag_host / seg_off_host int32[seg_cap] receive S+1 entries
+ *   each (may be NULL); S, N receive the segment count and total index count (may be NULL).
  * DPI_ERR_INVALID_ARG if seg_cap < S+1 or the last build overflowed max_indices. */
 dpi_status_t dpi_plan_export(const dpi_plan_t* plan, int32_t* offsets_host, int32_t* seg_bag_host,
-                             int64_t seg_cap, int32_t* S, int64_t* N, void* stream);
+                             int32_t* seg_off_host, int64_t seg_cap, int32_t* S, int64_t* N, void* stream);
 
 /*
  * dpi_lookup -- step a3, asynchronous on `stream`, ONE kernel launch for all tables and samples.
@@ -138,7 +144,8 @@ dpi_status_t dpi_plan_export(const dpi_plan_t* plan, int32_t* offsets_host, int3
  *   offsets_dev    NULL (use the plan's own offsets) or a device int32[G+1] equal to them
  *   plan           a built plan (same stream, or ordered after dpi_plan_build by an event)
  *   pooling        host uint8[T] of dpi_pool_t (NULL = all SUM)
- *   out_dev        device [B, T*D] row-major in the plan's dtype, 16-byte aligned; table t at columns
+ *   out_dev        device [B, T*D] row-major in the plan's output dtype (dpi_plan_set_out_dtype; default =
+ *                  table dtype), 16-byte aligned (32-byte for fp32 output of 16-bit tables); table t at columns
  *                  [t*D, (t+1)*D); every element is written exactly once
  * Out-of-range indices are a precondition violation (the paper is silent, R12): use
  * dpi_check_indices in tests.

@@ -50,7 +50,7 @@ def _load():
         lib.oracle_alg1_onehot.restype = ctypes.c_int
         lib.oracle_lookup.argtypes = [i32, i32, i32, ctypes.c_int, vp, vp, vp, vp, vp, vp]
         lib.oracle_lookup.restype = ctypes.c_int
-        lib.oracle_plan.argtypes = [vp, i64, i32, vp, vp, i64, vp]
+        lib.oracle_plan.argtypes = [vp, i64, i32, vp, vp, vp, i64, vp]
         lib.oracle_plan.restype = ctypes.c_int
         lib.oracle_decode_f16.argtypes = [ctypes.c_uint16]
         lib.oracle_decode_f16.restype = ctypes.c_double
@@ -118,17 +118,20 @@ def lookup(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray
     return ref
 
 
-def plan(lengths: np.ndarray, K: int):
-    """Workload plan. Returns (offsets int32[G+1], seg_bag int32[S+1], S)."""
+def plan(lengths: np.ndarray, K: int, with_seg_off: bool = False):
+    """Workload plan. Returns (offsets int32[G+1], seg_bag int32[S+1], S) and, with
+    with_seg_off=True, seg_off int32[S+1] as a fourth element."""
     lengths = np.ascontiguousarray(lengths, dtype=np.int32)
     G = lengths.shape[0]
     cap = (int(lengths.astype(np.int64).sum()) + G) // max(K, 1) + 3  # upper bound on S+1 (C[G] <= N + G)
     offsets = np.empty(G + 1, dtype=np.int32)
     seg_bag = np.empty(cap, dtype=np.int32)
+    seg_off = np.empty(cap, dtype=np.int32)
     S = ctypes.c_int32(0)
-    _check(_load().oracle_plan(lengths.ctypes.data, G, K, offsets.ctypes.data, seg_bag.ctypes.data, cap,
-                               ctypes.byref(S)))
-    return offsets, seg_bag[: S.value + 1].copy(), int(S.value)
+    _check(_load().oracle_plan(lengths.ctypes.data, G, K, offsets.ctypes.data, seg_bag.ctypes.data,
+                               seg_off.ctypes.data, cap, ctypes.byref(S)))
+    res = (offsets, seg_bag[: S.value + 1].copy(), int(S.value))
+    return res + (seg_off[: S.value + 1].copy(),) if with_seg_off else res
 
 
 def decode_f16(bits: int) -> float:

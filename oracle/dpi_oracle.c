@@ -141,10 +141,11 @@ int oracle_lookup(int32_t T, int32_t B, int32_t D, int dtype,
  *   C[0] = 0;       C[g+1] = C[g] + max(len[g], 1)                     (an empty bag still costs one store)
  *   S = ceil(C[G] / K)
  *   seg_bag[s] = min(G, min{ g in [0,G] : C[g] >= s*K }),  s = 0..S
- * seg_cap is the capacity of seg_bag in elements (needs S+1).
+ *   seg_off[s] = offsets[seg_bag[s]]                        (first index entry of task s; may be NULL)
+ * seg_cap is the capacity of seg_bag / seg_off in elements (needs S+1).
  */
 int oracle_plan(const int32_t *len, int64_t G, int32_t K,
-                int32_t *offsets, int32_t *seg_bag, int64_t seg_cap, int32_t *S_out)
+                int32_t *offsets, int32_t *seg_bag, int32_t *seg_off, int64_t seg_cap, int32_t *S_out)
 {
     if (!len || G < 0 || K < 1 || !offsets || !seg_bag || !S_out) return ORACLE_BAD_ARG;
     int64_t off = 0;
@@ -170,6 +171,7 @@ int oracle_plan(const int32_t *len, int64_t G, int32_t K,
         }
         /* here either Cg >= target (g is the lower bound) or g == G with C[G] < target (clamped to G) */
         seg_bag[s] = (int32_t)g;
+        if (seg_off) seg_off[s] = offsets[g];
     }
     *S_out = (int32_t)S;
     return ORACLE_OK;

@@ -22,7 +22,7 @@ DPI_POOL_SUM, DPI_POOL_MEAN = 0, 1
 OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL = range(6)
 
 # every symbol include/dpi.h declares (tests check the .so exports each one)
-EXPORTS = ["dpi_plan_create", "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
+EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
            "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export",
            "dpi_lookup", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
            "dpi_version", "dpi_status_string", "dpi_last_error"]
@@ -55,6 +55,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     vp, i32, i64, st = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int
     sig = {
         "dpi_plan_create": (st, [i32, vp, vp, ctypes.c_int, i32, i64, vp]),
+        "dpi_plan_set_out_dtype": (st, [vp, ctypes.c_int]),
         "dpi_plan_set_quantum": (st, [vp, i32]),
         "dpi_plan_set_option": (st, [vp, ctypes.c_int, i32]),
         "dpi_plan_get_option": (st, [vp, ctypes.c_int, vp]),
@@ -62,7 +63,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
         "dpi_plan": (st, [vp, i32, vp, ctypes.c_int, vp, i32, i64, vp, vp]),
         "dpi_plan_device_views": (st, [vp, vp, vp, vp]),
         "dpi_plan_info": (st, [vp, vp, vp, vp, vp, vp, vp, vp]),
-        "dpi_plan_export": (st, [vp, vp, vp, i64, vp, vp, vp]),
+        "dpi_plan_export": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_lookup": (st, [vp, vp, vp, vp, vp, vp, vp]),
         "dpi_forward_host": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_check_indices": (st, [vp, vp, vp, vp]),
@@ -127,6 +128,7 @@ class Plan:
                                    ctypes.byref(handle)))
         self._h = handle
         self.T, self.B, self.D, self.dtype = T, int(B), int(dims[0]), int(dtype)
+        self.out_dtype = int(dtype)
         self.G = self.T * self.B
         self.max_indices = int(max_indices)
 
@@ -141,6 +143,11 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+    # -- dpi_plan_set_out_dtype ------------------------------------------------------------------------------
+    def set_out_dtype(self, out_dtype: int):
+        _check(self._lib.dpi_plan_set_out_dtype(self._h, int(out_dtype)))
+        self.out_dtype = int(out_dtype)
 
     # -- dpi_plan_set_quantum / options ---------------------------------------------------------------------
     def set_quantum(self, K: int):
@@ -173,15 +180,18 @@ class Plan:
         return o.value, s.value, m.value
 
     # -- dpi_plan_export ------------------------------------------------------------------------------------
-    def export(self, stream=None):
-        """Returns (offsets int32[G+1], seg_bag int32[S+1], S, N) as host numpy arrays (synchronises)."""
+    def export(self, stream=None, with_seg_off: bool = False):
+        """Returns (offsets int32[G+1], seg_bag int32[S+1], S, N) as host numpy arrays (synchronises);
+        with_seg_off=True appends seg_off int32[S+1]."""
         cap = self.info()["seg_capacity"]
         offsets = np.empty(self.G + 1, dtype=np.int32)
         seg = np.empty(cap, dtype=np.int32)
+        seg_off = np.empty(cap, dtype=np.int32)
         S, N = ctypes.c_int32(), ctypes.c_int64()
-        _check(self._lib.dpi_plan_export(self._h, offsets.ctypes.data, seg.ctypes.data, cap, ctypes.byref(S),
-                                         ctypes.byref(N), _stream_handle(stream)))
-        return offsets, seg[: S.value + 1].copy(), int(S.value), int(N.value)
+        _check(self._lib.dpi_plan_export(self._h, offsets.ctypes.data, seg.ctypes.data, seg_off.ctypes.data, cap,
+                                         ctypes.byref(S), ctypes.byref(N), _stream_handle(stream)))
+        res = (offsets, seg[: S.value + 1].copy(), int(S.value), int(N.value))
+        return res + (seg_off[: S.value + 1].copy(),) if with_seg_off else res
 
     # -- dpi_lookup -----------------------------------------------------------------------------------------
     def lookup(self, table_ptrs_dev, indices_dev, out_dev, pooling=None, offsets_dev=None, stream=None):

@@ -50,6 +50,7 @@ struct dpi_plan_s {
     // shape
     int32_t T = 0, B = 0, D = 0;
     dpi_dtype_t dtype = DPI_F32;
+    dpi_dtype_t out_dtype = DPI_F32;
     uint32_t G = 0;
     int64_t max_indices = 0;
     uint32_t nvec = 0;   // 16-byte vectors per row
@@ -65,7 +66,7 @@ struct dpi_plan_s {
     // device
     int device = 0, num_sms = 0;
     int32_t* offsets = nullptr;
-    int32_t* seg_bag = nullptr;
+    int2* seg = nullptr;          // {seg_bag[s], seg_off[s]} interleaved
     int32_t* meta = nullptr;
     unsigned long long* tile_len = nullptr;
     unsigned long long* tile_cost = nullptr;
@@ -96,17 +97,17 @@ uint32_t seg_capacity_for(const dpi_plan_t* p, int32_t K) {
 
 dpi_status_t ensure_seg_capacity(dpi_plan_t* p, int32_t K) {
     const uint32_t need = seg_capacity_for(p, K);
-    if (need <= p->seg_cap && p->seg_bag) return DPI_OK;
-    if (p->seg_bag) DPI_CUDA(cudaFree(p->seg_bag));
-    p->seg_bag = nullptr;
-    DPI_CUDA(cudaMalloc(&p->seg_bag, static_cast<size_t>(need) * sizeof(int32_t)));
+    if (need <= p->seg_cap && p->seg) return DPI_OK;
+    if (p->seg) DPI_CUDA(cudaFree(p->seg));
+    p->seg = nullptr;
+    DPI_CUDA(cudaMalloc(&p->seg, static_cast<size_t>(need) * sizeof(int2)));
     p->seg_cap = need;
     return DPI_OK;
 }
 
 void free_plan(dpi_plan_t* p) {
     if (!p) return;
-    cudaFree(p->offsets); cudaFree(p->seg_bag); cudaFree(p->meta); cudaFree(p->tile_len);
+    cudaFree(p->offsets); cudaFree(p->seg); cudaFree(p->meta); cudaFree(p->tile_len);
     cudaFree(p->tile_cost); cudaFree(p->ticket); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
     cudaFree(p->stage_len); cudaFree(p->stage_idx); cudaFree(p->stage_out);
     (void)cudaGetLastError();
@@ -120,9 +121,9 @@ struct LaunchChoice {
 
 int occupancy(const dpi_plan_t* p, int lanes, int unroll, int threads) {
     switch (p->dtype) {
-        case DPI_F32: return lookup_occupancy_f32(lanes, unroll, threads);
-        case DPI_F16: return lookup_occupancy_f16(lanes, unroll, threads);
-        default: return lookup_occupancy_bf16(lanes, unroll, threads);
+        case DPI_F32: return lookup_occupancy_f32(lanes, unroll, threads, static_cast<uint32_t>(p->T), false);
+        case DPI_F16: return lookup_occupancy_f16(lanes, unroll, threads, static_cast<uint32_t>(p->T), p->out_dtype == DPI_F32);
+        default: return lookup_occupancy_bf16(lanes, unroll, threads, static_cast<uint32_t>(p->T), p->out_dtype == DPI_F32);
     }
 }
 
@@ -138,6 +139,7 @@ LaunchChoice choose_launch(const dpi_plan_t* p) {
     }
     c.l.grid = p->num_sms * per_sm;  // persistent: a whole number of waves, every CTA resident
     c.l.pdl = p->opt[DPI_OPT_PDL] != 0;
+    c.l.out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
     c.row_no_alloc = p->opt[DPI_OPT_ROW_L1_NO_ALLOC] < 0 ? 1 : p->opt[DPI_OPT_ROW_L1_NO_ALLOC];
     return c;
 }
@@ -148,7 +150,7 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const void* const* tables, const int
     a.tables = tables;
     a.indices = indices;
     a.offsets = offsets ? offsets : p->offsets;
-    a.seg_bag = p->seg_bag;
+    a.seg = p->seg;
     a.meta = p->meta;
     a.out = out;
     a.G = p->G;
@@ -214,7 +216,7 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
 
     dpi_plan_t* p = new (std::nothrow) dpi_plan_s();
     if (!p) return fail(DPI_ERR_ALLOC, "host allocation failed");
-    p->T = T; p->B = B; p->D = D; p->dtype = dtype;
+    p->T = T; p->B = B; p->D = D; p->dtype = dtype; p->out_dtype = dtype;
     p->G = static_cast<uint32_t>(G64);
     p->max_indices = max_indices;
     p->nvec = static_cast<uint32_t>(row_bytes / 16);
@@ -297,7 +299,7 @@ dpi_status_t dpi_plan_build(dpi_plan_t* p, const int32_t* lengths_dev, void* str
     PlanArgs a{};
     a.len = lengths_dev;
     a.offsets = p->offsets;
-    a.seg_bag = p->seg_bag;
+    a.seg = p->seg;
     a.meta = p->meta;
     a.tile_len = p->tile_len;
     a.tile_cost = p->tile_cost;
@@ -326,11 +328,11 @@ dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims,
     return st;
 }
 
-dpi_status_t dpi_plan_device_views(const dpi_plan_t* p, const int32_t** offsets_dev, const int32_t** seg_bag_dev,
+dpi_status_t dpi_plan_device_views(const dpi_plan_t* p, const int32_t** offsets_dev, const int32_t** seg_dev,
                                    const int32_t** meta_dev) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
     if (offsets_dev) *offsets_dev = p->offsets;
-    if (seg_bag_dev) *seg_bag_dev = p->seg_bag;
+    if (seg_dev) *seg_dev = reinterpret_cast<const int32_t*>(p->seg);
     if (meta_dev) *meta_dev = p->meta;
     return DPI_OK;
 }
@@ -348,8 +350,8 @@ dpi_status_t dpi_plan_info(const dpi_plan_t* p, int32_t* T, int32_t* B, int32_t*
     return DPI_OK;
 }
 
-dpi_status_t dpi_plan_export(const dpi_plan_t* p, int32_t* offsets_host, int32_t* seg_bag_host, int64_t seg_cap,
-                             int32_t* S, int64_t* N, void* stream) {
+dpi_status_t dpi_plan_export(const dpi_plan_t* p, int32_t* offsets_host, int32_t* seg_bag_host, int32_t* seg_off_host,
+                             int64_t seg_cap, int32_t* S, int64_t* N, void* stream) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
     if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -360,11 +362,25 @@ dpi_status_t dpi_plan_export(const dpi_plan_t* p, int32_t* offsets_host, int32_t
     if (S) *S = meta[META_S];
     if (N) *N = static_cast<uint32_t>(meta[META_N]);
     if (offsets_host) DPI_CUDA(cudaMemcpyAsync(offsets_host, p->offsets, (static_cast<size_t>(p->G) + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-    if (seg_bag_host) {
-        if (seg_cap < static_cast<int64_t>(meta[META_S]) + 1) return fail(DPI_ERR_INVALID_ARG, "seg_cap=%lld < S+1=%d", (long long)seg_cap, meta[META_S] + 1);
-        DPI_CUDA(cudaMemcpyAsync(seg_bag_host, p->seg_bag, (static_cast<size_t>(meta[META_S]) + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    if (seg_bag_host || seg_off_host) {
+        const size_t n = static_cast<size_t>(meta[META_S]) + 1;
+        if (seg_cap < static_cast<int64_t>(n)) return fail(DPI_ERR_INVALID_ARG, "seg_cap=%lld < S+1=%zu", (long long)seg_cap, n);
+        std::vector<int2> rec(n);
+        DPI_CUDA(cudaMemcpyAsync(rec.data(), p->seg, n * sizeof(int2), cudaMemcpyDeviceToHost, s));
+        DPI_CUDA(cudaStreamSynchronize(s));
+        for (size_t i = 0; i < n; ++i) {
+            if (seg_bag_host) seg_bag_host[i] = rec[i].x;
+            if (seg_off_host) seg_off_host[i] = rec[i].y;
+        }
     }
     DPI_CUDA(cudaStreamSynchronize(s));
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* p, dpi_dtype_t out_dtype) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (out_dtype != p->dtype && out_dtype != DPI_F32) return fail(DPI_ERR_UNSUPPORTED, "output dtype %d: must be the table dtype or DPI_F32", (int)out_dtype);
+    p->out_dtype = out_dtype;
     return DPI_OK;
 }
 
@@ -374,7 +390,8 @@ dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indice
     if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built (call dpi_plan_build first)");
     if (!table_ptrs_dev || !out_dev) return fail(DPI_ERR_INVALID_ARG, "table_ptrs_dev/out_dev is NULL");
     if (!indices_dev && p->max_indices > 0) return fail(DPI_ERR_INVALID_ARG, "indices_dev is NULL");
-    if (reinterpret_cast<uintptr_t>(out_dev) & 15u) return fail(DPI_ERR_INVALID_ARG, "out_dev is not 16-byte aligned");
+    const uintptr_t out_align = (p->dtype != DPI_F32 && p->out_dtype == DPI_F32) ? 31u : 15u;
+    if (reinterpret_cast<uintptr_t>(out_dev) & out_align) return fail(DPI_ERR_INVALID_ARG, "out_dev is not %d-byte aligned", (int)out_align + 1);
     if (reinterpret_cast<uintptr_t>(indices_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "indices_dev is not 4-byte aligned");
     return do_lookup(p, table_ptrs_dev, indices_dev, offsets_dev, pooling, out_dev, static_cast<cudaStream_t>(stream));
 }
@@ -386,10 +403,10 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     if (n_indices < 0 || n_indices > p->max_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld outside [0, max_indices=%lld]", (long long)n_indices, (long long)p->max_indices);
     if (n_indices > 0 && !indices_host) return fail(DPI_ERR_INVALID_ARG, "indices_host is NULL");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    const size_t out_bytes = static_cast<size_t>(p->G) * p->nvec * 16;
+    const size_t out_bytes = static_cast<size_t>(p->G) * p->D * (p->out_dtype == DPI_F32 ? 4 : 2);
     if (!p->stage_len) DPI_CUDA(cudaMalloc(&p->stage_len, static_cast<size_t>(p->G) * sizeof(int32_t)));
     if (!p->stage_idx) DPI_CUDA(cudaMalloc(&p->stage_idx, (static_cast<size_t>(p->max_indices) + 4) * sizeof(int32_t)));
-    if (!p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, out_bytes));
+    if (!p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, static_cast<size_t>(p->G) * p->D * 4));
     DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
     if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
     dpi_status_t st = dpi_plan_build(p, p->stage_len, s);

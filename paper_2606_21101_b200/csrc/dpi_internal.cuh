@@ -30,7 +30,7 @@ constexpr int kScanTile = kScanThreads * kScanItems;        // 2048 bags per CTA
 struct PlanArgs {
     const int32_t* __restrict__ len;   // [G]
     int32_t* __restrict__ offsets;     // [G+1]
-    int32_t* __restrict__ seg_bag;     // [seg_cap]
+    int2* __restrict__ seg;            // [seg_cap] {seg_bag[s], seg_off[s] = offsets[seg_bag[s]]}
     int32_t* __restrict__ meta;        // [kMetaWords]
     unsigned long long* tile_len;      // [num_tiles] look-back status words for the length scan
     unsigned long long* tile_cost;     // [num_tiles] look-back status words for the cost scan
@@ -60,9 +60,9 @@ struct LookupArgs {
     const void* const* __restrict__ tables;  // device [T] table base pointers
     const int32_t* __restrict__ indices;     // [N]
     const int32_t* __restrict__ offsets;     // [G+1]
-    const int32_t* __restrict__ seg_bag;     // [S+1]
+    const int2* __restrict__ seg;            // [S+1] {seg_bag, seg_off}
     const int32_t* __restrict__ meta;        // meta[META_S] = S
-    void* __restrict__ out;                  // [G * D] in table dtype  (out[b, t*D + c] == out[g*D + c])
+    void* __restrict__ out;                  // [G * D] in the output dtype (out[b, t*D + c] == out[g*D + c])
     uint32_t G;
     uint32_t T;
     uint32_t nvec;                           // 16-byte vectors per row = D*sizeof(elt)/16
@@ -77,6 +77,7 @@ struct LookupLaunch {
     int block_threads;  // 128, 256, 512
     int grid;           // persistent grid size
     bool pdl;           // programmatic dependent launch
+    bool out32;         // 16-bit tables only: emit the output block in fp32
 };
 
 // Each returns cudaErrorInvalidValue when (lanes, unroll, block_threads) has no instantiation.
@@ -84,9 +85,9 @@ cudaError_t launch_lookup_f32(const LookupArgs& a, const LookupLaunch& l, cudaSt
 cudaError_t launch_lookup_f16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
 cudaError_t launch_lookup_bf16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
 // Max resident CTAs per SM of the instantiation (0 if none).
-int lookup_occupancy_f32(int lanes, int unroll, int block_threads);
-int lookup_occupancy_f16(int lanes, int unroll, int block_threads);
-int lookup_occupancy_bf16(int lanes, int unroll, int block_threads);
+int lookup_occupancy_f32(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
+int lookup_occupancy_f16(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
+int lookup_occupancy_bf16(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
 
 void count_launch();
 

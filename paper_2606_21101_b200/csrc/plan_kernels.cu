@@ -5,6 +5,8 @@
 //   * fused partition: bag g knows C[g] and C[g+1]; it owns every quantum boundary s*K in (C[g], C[g+1]],
 //     i.e. seg_bag[s] = g+1 for s = floor(C[g]/K)+1 .. floor(C[g+1]/K).  That is exactly
 //     seg_bag[s] = min{g : C[g] >= s*K} without any binary search or second kernel.
+//     Next to it goes seg_off[s] = offsets[seg_bag[s]] (first entry of the task), interleaved as int2
+//     {seg_bag, seg_off}, so the lookup reaches a task's indices with one dependent load instead of two.
 // Integer work only; results are bit-exact against oracle/dpi_oracle.c::oracle_plan.
 //
 // Bytes: 4 B read + 4 B written per bag, 4 B per segment -- HBM/L2-bound, ~microseconds at G <= 1e6.
@@ -186,15 +188,17 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
     }
 
     // ---- a2: every quantum boundary s*K inside (C[g], C[g+1]] belongs to bag g -> seg_bag[s] = g+1 ----
-    if (base == 0) a.seg_bag[0] = 0;      // s = 0: C[0] = 0 >= 0
+    if (base == 0) a.seg[0] = make_int2(0, 0);      // s = 0: C[0] = 0 >= 0
     uint32_t q_prev = c / a.K;
+    uint32_t run = off;
 #pragma unroll
     for (int i = 0; i < kScanItems; ++i) {
         if (static_cast<uint32_t>(i) < n_valid) {
             c += max(v[i], 1u);
+            run += v[i];                             // offsets[base + i + 1]
             const uint32_t q = c / a.K;
             for (uint32_t s = q_prev + 1; s <= q; ++s)
-                if (s < a.seg_cap) a.seg_bag[s] = base + i + 1;
+                if (s < a.seg_cap) a.seg[s] = make_int2(base + i + 1, run);
             q_prev = q;
         }
     }
@@ -206,7 +210,7 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
         for (int i = 0; i < kScanItems; ++i) n_total += v[i];
         a.offsets[a.G] = n_total;
         const uint32_t S = c / a.K + ((c % a.K) ? 1u : 0u);   // ceil(C[G]/K)
-        if ((c % a.K) != 0 && S < a.seg_cap) a.seg_bag[S] = a.G;  // C[G] < S*K: clamped to G
+        if ((c % a.K) != 0 && S < a.seg_cap) a.seg[S] = make_int2(a.G, n_total);  // C[G] < S*K: clamped to G
         a.meta[META_S] = (S < a.seg_cap) ? S : 0;             // an overflowed plan must not drive a lookup
         a.meta[META_N] = n_total;
         a.meta[META_C] = c;

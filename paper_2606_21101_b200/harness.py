@@ -80,7 +80,7 @@ def upload_batch(batch: W.Batch, device="cuda:0") -> DeviceBatch:
 
 
 def new_output(cfg: W.Config, device="cuda:0", fill_nan: bool = False) -> torch.Tensor:
-    out = torch.empty((cfg.B, cfg.T * cfg.D), dtype=TORCH_DTYPE[cfg.dtype], device=device)
+    out = torch.empty((cfg.B, cfg.T * cfg.D), dtype=TORCH_DTYPE[cfg.out], device=device)
     if fill_nan:
         out.fill_(float("nan"))  # a bag the kernel forgets to write shows up as NaN in the parity check
     return out
@@ -92,7 +92,10 @@ def out_to_f64(out: torch.Tensor) -> np.ndarray:
 
 
 def make_plan(cfg: W.Config, rows: np.ndarray, max_indices: int) -> binding.Plan:
-    return binding.Plan(rows, cfg.D, W.DTYPE_CODE[cfg.dtype], cfg.B, max_indices)
+    plan = binding.Plan(rows, cfg.D, W.DTYPE_CODE[cfg.dtype], cfg.B, max_indices)
+    if cfg.out != cfg.dtype:
+        plan.set_out_dtype(W.DTYPE_CODE[cfg.out])
+    return plan
 
 
 def max_indices_bound(cfg: W.Config) -> int:

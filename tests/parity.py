@@ -13,10 +13,14 @@ def host_offsets(lengths: np.ndarray) -> np.ndarray:
     return np.concatenate(([0], np.cumsum(np.asarray(lengths, dtype=np.int64)))).astype(np.int32)
 
 
-def assert_outputs_match(gpu_f64: np.ndarray, ref: np.ndarray, lengths: np.ndarray, T: int, D: int, dtype: str):
-    """north_star: fp32 tables max|err| <= 1e-5 * bag length; fp16/bf16 <= 2e-3 relative (fp32 accumulate),
-    with the absolute floor 1e-6*L for cancellation. Against the UNROUNDED float64 reference.
-    Bit-exact when L <= 1; an empty bag is exactly +0.0."""
+def assert_outputs_match(gpu_f64: np.ndarray, ref: np.ndarray, lengths: np.ndarray, T: int, D: int, dtype: str,
+                         out_dtype: str = None):
+    """north_star: fp32 tables max|err| <= 1e-5 * bag length; fp16/bf16 tables <= 2e-3 relative (fp32
+    accumulate), with the absolute floor 1e-6*L for cancellation. Against the UNROUNDED
+    float64 reference. Bit-exact when L <= 1; an empty bag is exactly +0.0.
+    Only a bf16 OUTPUT cannot meet 2e-3: one correct RNE to 8 significand bits already costs up to
+    2^-8 = 3.906e-3 relative, so that variant is held to 2^-8*|ref| + 1e-6*L (reading R6)."""
+    out_dtype = out_dtype or dtype
     B = ref.shape[0]
     g = gpu_f64.reshape(B * T, D)
     r = ref.reshape(B * T, D)
@@ -26,6 +30,8 @@ def assert_outputs_match(gpu_f64: np.ndarray, ref: np.ndarray, lengths: np.ndarr
     Lm = np.maximum(L, 1).astype(np.float64)[:, None]
     if dtype == "f32":
         tol = 1e-5 * Lm * np.ones_like(r)
+    elif out_dtype == "bf16":
+        tol = 2.0 ** -8 * np.abs(r) + 1e-6 * Lm
     else:
         tol = np.maximum(2e-3 * np.abs(r), 1e-6 * Lm)
     bad = err > tol

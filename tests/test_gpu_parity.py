@@ -44,11 +44,12 @@ def _plan_parity(lengths: np.ndarray, T: int, B: int, K: int, max_indices=None):
     dev = torch.from_numpy(np.ascontiguousarray(lengths, dtype=np.int32)).cuda()
     for _ in range(2):  # the second build reuses the look-back status words (epoch tagging)
         plan.build(dev)
-        off, seg, S, n = plan.export()
-        o_off, o_seg, o_S = oracle.plan(lengths, K)
+        off, seg, S, n, seg_off = plan.export(with_seg_off=True)
+        o_off, o_seg, o_S, o_seg_off = oracle.plan(lengths, K, with_seg_off=True)
         assert n == N and S == o_S
         assert np.array_equal(off, o_off)
         assert np.array_equal(seg, o_seg)
+        assert np.array_equal(seg_off, o_seg_off)
     plan.destroy()
 
 
@@ -125,21 +126,25 @@ def _full_parity(cfg, K=0, opts=None, batch_seed=None, pooling=None):
     pooling = cfg.pooling_modes() if pooling is None else pooling
     got = _run_gpu(cfg, dt, batch, pooling, K, opts)
     ref = oracle_reference(host_tables, cfg.dtype, cfg.B, batch.lengths, batch.indices, pooling)
-    return assert_outputs_match(got, ref, batch.lengths, cfg.T, cfg.D, cfg.dtype)
+    return assert_outputs_match(got, ref, batch.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out)
 
 
 def test_c1_exact_config():
     _full_parity(W.C1)
 
 
-@pytest.mark.parametrize("dtype,D", [("f32", 4), ("f32", 16), ("f32", 24), ("f32", 64), ("f32", 128),
-                                     ("f16", 8), ("f16", 32), ("f16", 72), ("f16", 256),
-                                     ("bf16", 8), ("bf16", 64), ("bf16", 128), ("bf16", 256)])
+@pytest.mark.parametrize("dtype,D,out", [("f32", 4, None), ("f32", 16, None), ("f32", 24, None), ("f32", 64, None),
+                                         ("f32", 128, None),
+                                         ("f16", 8, None), ("f16", 32, None), ("f16", 72, None), ("f16", 256, None),
+                                         ("f16", 8, "f32"), ("f16", 64, "f32"),
+                                         ("bf16", 8, None), ("bf16", 64, None), ("bf16", 128, None), ("bf16", 256, None),
+                                         ("bf16", 8, "f32"), ("bf16", 24, "f32"), ("bf16", 64, "f32"), ("bf16", 256, "f32")])
 @pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 1, 4), ("poisson", 20.0, 100, 0.05)])
-def test_shapes_dtypes_and_length_mixes(dtype, D, lengths):
+def test_shapes_dtypes_and_length_mixes(dtype, D, out, lengths):
     """Several tiles, a ragged tail, every lanes-per-row instantiation (incl. non-power-of-two row sizes),
-    mixed sum/mean pooling, empty bags."""
-    cfg = W.Config("s", 5, (1000, 17, 4000, 1, 250), D, dtype, 333, lengths, ("zipf", 1.05), "half", seed=11)
+    mixed sum/mean pooling, empty bags, both output types of the 16-bit tables."""
+    cfg = W.Config("s", 5, (1000, 17, 4000, 1, 250), D, dtype, 333, lengths, ("zipf", 1.05), "half", seed=11,
+                   out_dtype=out)
     _full_parity(cfg)
 
 
@@ -257,6 +262,21 @@ def test_forward_host_equals_device_path():
     plan.destroy()
 
 
+def test_c4_with_bf16_output_meets_the_derived_bound():
+    """Same workload as c4 but the output block in bf16 (the table dtype): held to 2^-8 relative (R6)."""
+    _sampled_full_size(W.C4.scaled(out_dtype=None, B=1024), 256)
+
+
+def test_out_dtype_validation():
+    plan = binding.Plan([10], 16, binding.DPI_F16, 4, 10)
+    plan.set_out_dtype(binding.DPI_F32)
+    plan.set_out_dtype(binding.DPI_F16)
+    with pytest.raises(binding.DpiError) as e:
+        plan.set_out_dtype(binding.DPI_BF16)
+    assert e.value.status == 2
+    plan.destroy()
+
+
 # --------------------------------------------------------------------------------------------------
 # BASELINE.json configs at full size, in the launch configuration bench.py times (library defaults)
 # --------------------------------------------------------------------------------------------------
@@ -279,7 +299,7 @@ def _sampled_full_size(cfg, n_samples, rotate=1):
         sub = W.compact_subproblem(cfg, batch, samples)
         ref = oracle.lookup(sub.tables, W.DTYPE_CODE[cfg.dtype], len(samples), sub.indices,
                             host_offsets(sub.lengths), pooling)
-        worst = max(worst, assert_outputs_match(got[samples], ref, sub.lengths, cfg.T, cfg.D, cfg.dtype))
+        worst = max(worst, assert_outputs_match(got[samples], ref, sub.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out))
     del dt
     torch.cuda.empty_cache()
     return worst

@@ -26,10 +26,11 @@ def test_golden_fig5_plan():
     g = load("fig5_shape_example.txt")
     lengths = np.array(g["multihot.lengths"], dtype=np.int32).reshape(-1)
     K = int(g["plan.K"][0][0])
-    off, seg, S = oracle.plan(lengths, K)
+    off, seg, S, seg_off = oracle.plan(lengths, K, with_seg_off=True)
     assert off.tolist() == [int(x) for x in g["plan.offsets"][0]]
     assert S == int(g["plan.S"][0][0])
     assert seg.tolist() == [int(x) for x in g["plan.seg_bag"][0]]
+    assert seg_off.tolist() == [int(x) for x in g["plan.seg_off"][0]]
 
 
 @pytest.mark.parametrize("seed", range(6))
@@ -45,6 +46,8 @@ def test_plan_matches_brute_force_and_cumsum(seed, K):
     assert np.array_equal(off[1:], np.cumsum(lengths))
     bseg, bS = brute_plan(lengths.tolist(), K)
     assert S == bS and seg.tolist() == bseg
+    seg_off = oracle.plan(lengths, K, with_seg_off=True)[3]
+    assert seg_off.tolist() == [int(np.sum(lengths[:g])) for g in bseg]  # entries before the task's first bag
 
 
 @pytest.mark.parametrize("ell", [1, 2, 3, 5, 64])
