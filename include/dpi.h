@@ -68,9 +68,10 @@ typedef enum { DPI_POOL_SUM = 0, DPI_POOL_MEAN = 1 } dpi_pool_t;
 /* Tuning knobs for dpi_plan_set_option (all kernel-internal; none changes a result). */
 typedef enum {
     DPI_OPT_UNROLL = 0,         /* independent 128-bit row loads in flight per lane: 2, 4, 8 or 16; 0 = auto */
-    DPI_OPT_BLOCK_THREADS = 1,  /* lookup CTA size: 128, 256 or 512; 0 = auto */
+    DPI_OPT_BLOCK_THREADS = 1,  /* lookup CTA size: a multiple of 32 up to 256; 0 = auto */
     DPI_OPT_BLOCKS_PER_SM = 2,  /* persistent grid = SMs * this; 0 = auto (occupancy) */
-    DPI_OPT_MODE = 3,           /* 0 auto per segment, 1 sub-warp per bag, 2 whole warp per bag */
+    DPI_OPT_MODE = 3,           /* 0 auto per task, 1 sub-warp per bag, 2 warp per bag (single-buffered),
+                                   3 warp per bag (double-buffered batches) */
     DPI_OPT_ROW_L1_NO_ALLOC = 4,/* 1: table rows bypass L1 (ld.global.nc.L1::no_allocate); 0: default; -1 auto */
     DPI_OPT_PDL = 5,            /* 1: lookup is launched with programmatic dependent launch after the planner */
     DPI_OPT_COUNT_

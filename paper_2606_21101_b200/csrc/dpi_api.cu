@@ -83,10 +83,15 @@ struct dpi_plan_s {
 namespace {
 
 int32_t default_quantum(const dpi_plan_t* p) {
-    // One warp-task should keep P*U row loads in flight for a few rounds: ~32 entries per task works across
-    // row sizes (64 B rows: 8 sub-warps x 4; 256 B rows: 2 sub-warps x 16). Tuned by ncu, see DESIGN.md §6.
-    (void)p;
-    return 32;
+    // Measured on B200 (profiles/sweeps_r01.md): K = 128 is best once there are plenty of tasks per warp (c4/c5:
+    // the per-task pipeline refill is amortised); small batches want more, smaller tasks so that every resident
+    // warp has work: aim at >= 4 tasks per warp of a full persistent grid (32 warps per SM), within [16, 128].
+    const uint64_t cost_bound = static_cast<uint64_t>(p->max_indices) + p->G;   // >= C[G]
+    const uint64_t warps = static_cast<uint64_t>(p->num_sms > 0 ? p->num_sms : 148) * 32;
+    uint64_t k = cost_bound / (4 * warps);
+    int32_t K = 16;
+    while (K < 128 && static_cast<uint64_t>(K) * 2 <= k) K *= 2;
+    return K;
 }
 
 uint32_t seg_capacity_for(const dpi_plan_t* p, int32_t K) {
@@ -130,7 +135,7 @@ int occupancy(const dpi_plan_t* p, int lanes, int unroll, int threads) {
 LaunchChoice choose_launch(const dpi_plan_t* p) {
     LaunchChoice c{};
     c.l.lanes = p->lanes;
-    c.l.unroll = p->opt[DPI_OPT_UNROLL] ? p->opt[DPI_OPT_UNROLL] : 8;
+    c.l.unroll = p->opt[DPI_OPT_UNROLL] ? p->opt[DPI_OPT_UNROLL] : 2;  // x2 by double buffering (sweeps_r01.md)
     c.l.block_threads = p->opt[DPI_OPT_BLOCK_THREADS] ? p->opt[DPI_OPT_BLOCK_THREADS] : 256;
     int per_sm = p->opt[DPI_OPT_BLOCKS_PER_SM];
     if (per_sm <= 0) {
@@ -138,9 +143,13 @@ LaunchChoice choose_launch(const dpi_plan_t* p) {
         if (per_sm <= 0) per_sm = 1;
     }
     c.l.grid = p->num_sms * per_sm;  // persistent: a whole number of waves, every CTA resident
+    const int64_t warps_per_cta = c.l.block_threads / 32;
+    const int64_t need = (static_cast<int64_t>(p->seg_cap) + warps_per_cta - 1) / warps_per_cta;  // one warp per possible task
+    if (need < c.l.grid) c.l.grid = static_cast<int>(need > 0 ? need : 1);
     c.l.pdl = p->opt[DPI_OPT_PDL] != 0;
     c.l.out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
-    c.row_no_alloc = p->opt[DPI_OPT_ROW_L1_NO_ALLOC] < 0 ? 1 : p->opt[DPI_OPT_ROW_L1_NO_ALLOC];
+    // auto: let rows allocate in L1 -- measured +17 % on c5 and +20 % on c4 over L1::no_allocate (sweeps_r01.md)
+    c.row_no_alloc = p->opt[DPI_OPT_ROW_L1_NO_ALLOC] < 0 ? 0 : p->opt[DPI_OPT_ROW_L1_NO_ALLOC];
     return c;
 }
 
@@ -268,9 +277,9 @@ dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
     bool ok = false;
     switch (opt) {
         case DPI_OPT_UNROLL: ok = v == 0 || v == 2 || v == 4 || v == 8 || v == 16; break;
-        case DPI_OPT_BLOCK_THREADS: ok = v == 0 || (v >= 32 && v <= 512 && v % 32 == 0); break;
+        case DPI_OPT_BLOCK_THREADS: ok = v == 0 || (v >= 32 && v <= 256 && v % 32 == 0); break;
         case DPI_OPT_BLOCKS_PER_SM: ok = v >= 0 && v <= 32; break;
-        case DPI_OPT_MODE: ok = v >= 0 && v <= 2; break;
+        case DPI_OPT_MODE: ok = v >= 0 && v <= 3; break;
         case DPI_OPT_ROW_L1_NO_ALLOC: ok = v >= -1 && v <= 1; break;
         case DPI_OPT_PDL: ok = v == 0 || v == 1; break;
         default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);

@@ -16,9 +16,10 @@
 // A row is NV = D*sizeof(elt)/16 128-bit vectors; W = pow2ceil(NV) lanes hold one row (lane sl < NV loads
 // vector sl), P = 32/W sub-warps per warp.  Three warp-uniform shapes per task:
 //   one-hot   (every bag in the task has length 1): pure row copy, P*U rows in flight per warp (Alg. 1)
-//   sub-warp  (short bags): sub-warp q pools bags g_lo+q, g_lo+q+P, ... with U loads in flight per lane
-//   warp      (long bags) : all P sub-warps stride the entries of one bag, U loads in flight per lane, then
-//                           log2(P) __shfl_xor steps combine the partial sums
+//   sub-warp  (mean length < 2P): sub-warp q pools bags g_lo+q, g_lo+q+P, ... with U loads in flight per lane
+//   warp      (long bags) : all P sub-warps stride the entries of one bag in batches of P*U rows; batches are
+//                           double-buffered across batch AND bag boundaries (U..2U loads in flight per lane);
+//                           log2(P) __shfl_xor steps combine the partial sums at the end of a bag
 // Row loads are branch-free (predicated ld.global.nc.v4) so the U loads of a batch issue back to back.
 // fp32 accumulation in registers; one RNE cast at the store (fp16/bf16 output) or fp32 output (OUT32).
 #pragma once
@@ -30,7 +31,7 @@ namespace dpi {
 constexpr int kStageIdx = 256;  // staged index entries per task buffer (tasks with more read global memory)
 constexpr int kStageOff = 72;   // staged offsets per task buffer (bags + 1)
 constexpr int kWarpStageInts = 2 * kStageIdx + 2 * kStageOff;
-constexpr int kLookupMaxThreads = 512;
+constexpr int kLookupMaxThreads = 256;  // natural register allocation (64-80/thread); a 512 bound made ptxas spill
 
 // ---- memory helpers ----------------------------------------------------------------------------------
 // Predicated 128-bit read-only load; lanes with pred == false get zeros and issue no memory request.
@@ -243,7 +244,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                         }
                     }
                 }
-            } else if (P == 1 || a.mode == 1 || (a.mode == 0 && nb >= P && ne < 2u * P * nb)) {
+            } else if (a.mode == 1 || (a.mode == 0 && ne < 2u * (P == 1 ? U : P) * nb)) {
                 // ---------------- sub-warp per bag (short bags) ---------------------------------------------
                 for (uint32_t g0 = g_lo; g0 < g_hi; g0 += P) {
                     const uint32_t g = g0 + sub;
@@ -272,8 +273,8 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                         store_pooled<Tr, OUT32>(out, g, a.nvec, sl, acc);
                     }
                 }
-            } else {
-                // ---------------- whole warp per bag (long bags) --------------------------------------------
+            } else if (a.mode == 2) {
+                // ---------------- whole warp per bag, one batch at a time (kept for A/B measurements) ------
                 for (uint32_t g = g_lo; g < g_hi; ++g) {
                     const int lo = op[g], hi = op[g + 1];
                     const uint32_t t = g % a.T;
@@ -301,6 +302,89 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                     if (sub == 0 && vec_ok) {
                         if (((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
                         store_pooled<Tr, OUT32>(out, g, a.nvec, sl, acc);
+                    }
+                }
+            } else {
+                // ---------------- whole warp per bag, double-buffered batches (long bags) -------------------
+                // The loads of batch k+1 (possibly the first batch of the NEXT bag: its offsets and indices
+                // are already in smem) are issued before batch k is consumed, so a warp keeps U..2U row
+                // loads per lane in flight across batch and bag boundaries instead of draining at each one.
+                auto store_zero = [&](uint32_t gz) {
+                    if (sub == 0 && vec_ok) {
+                        float z[kAcc];
+#pragma unroll
+                        for (int i = 0; i < kAcc; ++i) z[i] = 0.f;
+                        store_pooled<Tr, OUT32>(out, gz, a.nvec, sl, z);
+                    }
+                };
+                auto issue = [&](uint4 (&v)[U], int j, int hi, const char* tab) {
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        const int e = j + u * P + sub;
+                        const bool ok = e < hi;
+                        const int r = ip[ok ? e : j];
+                        v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok, no_alloc);
+                    }
+                };
+                uint32_t g = g_lo;
+                int lo = op[g], hi = op[g + 1];
+                while (hi == lo) {  // leading empty bags
+                    store_zero(g);
+                    if (++g == g_hi) break;
+                    lo = hi;
+                    hi = op[g + 1];
+                }
+                if (g < g_hi) {
+                    int j = lo;
+                    const char* tab = s_tab[g % a.T] + sl * 16;
+                    float acc[kAcc];
+#pragma unroll
+                    for (int i = 0; i < kAcc; ++i) acc[i] = 0.f;
+                    uint4 vA[U], vB[U];
+                    issue(vA, j, hi, tab);
+                    bool more = true;
+                    auto step = [&](uint4 (&cv)[U], uint4 (&nv)[U]) {
+                        uint32_t g_n = g;
+                        int j_n = j + P * U, lo_n = lo, hi_n = hi;
+                        const char* tab_n = tab;
+                        const bool last_of_bag = j_n >= hi;
+                        bool has_next = true;
+                        if (last_of_bag) {
+                            g_n = g + 1;
+                            for (;;) {
+                                if (g_n == g_hi) { has_next = false; break; }
+                                lo_n = hi_n;
+                                hi_n = op[g_n + 1];
+                                if (hi_n > lo_n) break;
+                                store_zero(g_n);
+                                ++g_n;
+                            }
+                            if (has_next) { j_n = lo_n; tab_n = s_tab[g_n % a.T] + sl * 16; }
+                        }
+                        if (has_next) issue(nv, j_n, hi_n, tab_n);
+#pragma unroll
+                        for (int u = 0; u < U; ++u) Tr::add(acc, cv[u]);
+                        if (last_of_bag) {
+#pragma unroll
+                            for (int d = W; d < 32; d <<= 1) {
+#pragma unroll
+                                for (int i = 0; i < kAcc; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], d);
+                            }
+                            if (sub == 0 && vec_ok) {
+                                const uint32_t t = g % a.T;
+                                if (((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
+                                store_pooled<Tr, OUT32>(out, g, a.nvec, sl, acc);
+                            }
+#pragma unroll
+                            for (int i = 0; i < kAcc; ++i) acc[i] = 0.f;
+                        }
+                        g = g_n; j = j_n; lo = lo_n; hi = hi_n; tab = tab_n;
+                        more = has_next;
+                    };
+                    while (more) {
+                        step(vA, vB);
+                        if (!more) break;
+                        step(vB, vA);
                     }
                 }
             }

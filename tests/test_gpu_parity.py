@@ -149,7 +149,7 @@ def test_shapes_dtypes_and_length_mixes(dtype, D, out, lengths):
 
 
 @pytest.mark.parametrize("unroll", [2, 4, 8, 16])
-@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
 def test_every_kernel_variant_gives_the_same_answer(unroll, mode):
     cfg = W.Config("v", 6, (500, 30, 2000, 7, 100, 1000), 64, "f32", 257, ("uniform", 0, 70), ("uniform",), "half", 3)
     _full_parity(cfg, K=32, opts={binding.OPT_UNROLL: unroll, binding.OPT_MODE: mode})
