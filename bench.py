@@ -30,6 +30,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "pooled embedding lookups/sec"
+DTYPE_KEY = {"f32": "f32", "f16": "f16 tables, f32 accumulate", "bf16": "bf16 tables, f32 accumulate"}
 UNIT = "lookups/s"
 R_BATCHES = 8
 
@@ -37,8 +38,8 @@ R_BATCHES = 8
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=40)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c5")
     ap.add_argument("--quantum", type=int, default=0)
@@ -48,6 +49,8 @@ def parse_args():
     ap.add_argument("--mode", type=int, default=0)
     ap.add_argument("--row-l1-no-alloc", type=int, default=-1)
     ap.add_argument("--pdl", type=int, default=0)
+    ap.add_argument("--graph", type=int, default=-1, help="1: time a CUDA-graph replay of the K steps; 0: stream launches; -1: auto (graph for c1-c3)")
+    ap.add_argument("--rotating-batches", type=int, default=R_BATCHES)
     ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -78,50 +81,96 @@ def ncu_traffic(workload: str):
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    """Samples SM clock and throttle reasons during the timed region: NVML in a thread (5 ms period), falling
+    back to an `nvidia-smi -lms` subprocess when pynvml is unavailable."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, gpu_index: int):
         self.idx = gpu_index
-        self.samples = []
+        self.samples = []     # (time, sm_mhz, set(reasons), power_w)
+        self.max_mhz = None
         self.proc = None
+        self.nvml = None
+        self._stop = threading.Event()
+        self.thread = None
+
+    def _physical_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            try:
+                return int(vis.split(",")[self.idx])
+            except Exception:
+                pass
+        return self.idx
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(self._physical_index())
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._poll_nvml, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nvml = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self._physical_index()), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread = threading.Thread(target=self._read_smi, daemon=True)
             self.thread.start()
         except Exception:
             self.proc = None
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.samples.append((time.time(), line.strip()))
+    def _poll_nvml(self):
+        n = self.nvml
+        bits = {"hw_slowdown": n.nvmlClocksEventReasonHwSlowdown if hasattr(n, "nvmlClocksEventReasonHwSlowdown") else 0x8,
+                "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+        while not self._stop.is_set():
+            try:
+                mhz = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+                try:
+                    mask = int(n.nvmlDeviceGetCurrentClocksEventReasons(self.handle))
+                except Exception:
+                    mask = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+                try:
+                    pw = n.nvmlDeviceGetPowerUsage(self.handle) / 1000.0
+                except Exception:
+                    pw = None
+                self.samples.append((time.time(), mhz, {k for k, b in bits.items() if mask & b}, pw))
+            except Exception:
+                pass
+            time.sleep(0.005)
 
-    def stop(self, t0: float, t1: float) -> dict:
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, mx, reasons = [], None, set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        rows = [s for s in self.samples if t0 - 0.05 <= s[0] <= t1 + 0.15] or self.samples
-        for _, line in rows:
+    def _read_smi(self):
+        for line in self.proc.stdout:
             p = [x.strip() for x in line.split(",")]
             try:
-                sm.append(float(p[0]))
-                mx = float(p[1])
-                for n, v in zip(names, p[3:7]):
-                    if v.lower().startswith("active"):
-                        reasons.add(n)
+                self.max_mhz = float(p[1])
+                rs = {n for n, v in zip(self.NAMES, p[3:7]) if v.lower().startswith("active")}
+                self.samples.append((time.time(), float(p[0]), rs, float(p[2])))
             except Exception:
                 continue
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(rows)}
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.thread is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["clock sampling unavailable"]}
+        time.sleep(0.06)
+        self._stop.set()
+        if self.proc is not None:
+            self.proc.terminate()
+        rows = [s for s in self.samples if t0 <= s[0] <= t1] or [s for s in self.samples if t0 - 0.1 <= s[0] <= t1 + 0.1]
+        sm = [r[1] for r in rows]
+        reasons = set().union(*[r[2] for r in rows]) if rows else set()
+        pw = [r[3] for r in rows if r[3] is not None]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_min_mhz": min(sm) if sm else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(reasons), "samples": len(rows),
+                "power_w_max": max(pw) if pw else None, "source": "nvml" if self.nvml else "nvidia-smi"}
 
 
 def apply_options(plan, args, binding):
@@ -144,11 +193,11 @@ def workload_config(args):
     return cfg, rows
 
 
-def describe(cfg, rows, extra=None):
+def describe(cfg, rows, extra=None, R=R_BATCHES):
     d = {"workload": f"{cfg.name} (BASELINE.json configs[{int(cfg.name[1]) - 1}])", "tables": cfg.T,
          "rows_total": int(rows.sum()), "D": cfg.D, "table_dtype": cfg.dtype, "batch": cfg.B,
          "bag_lengths": list(cfg.lengths), "indices": list(cfg.index_dist), "pooling": cfg.pooling,
-         "rotating_batches": R_BATCHES,
+         "rotating_batches": R,
          "l2": "inputs larger than L2 (no flush)" if cfg.name in ("c4", "c5") else "warm L2 (working set < L2)"}
     if extra:
         d.update(extra)
@@ -203,9 +252,9 @@ def run_reference(args):
     if rank != 0:
         return
     cfg, rows = workload_config(args)
-    r = time_oracle(cfg, rows, args.cpu_seconds, steps=None if args.steps == 40 else args.steps, warmup=min(args.warmup, 1))
+    r = time_oracle(cfg, rows, args.cpu_seconds, steps=args.steps, warmup=min(args.warmup or 0, 1))
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": r["steps"], "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"],
+            "steps": r["steps"], "warmup": min(args.warmup or 0, 1), "ms_per_step": r["ms_per_step"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": describe(cfg, rows), "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -218,7 +267,7 @@ def run_reference(args):
 # ----------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
-    from paper_2606_21101_b200 import binding, build, harness, workloads as W
+    from paper_2606_21101_b200 import binding, build, harness, sharding, workloads as W
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -235,62 +284,96 @@ def run_ours(args):
     if dist is not None:
         dist.barrier()
     binding.load_library()
-    warmup = max(args.warmup, 3)
-    steps = max(args.steps, 1)
 
     cfg, rows = workload_config(args)
-    # every rank: all tables + its own rotating batches (batch-sharded replicas, no collective on the data path)
-    dt = harness.make_device_tables(cfg, rows)
-    batches = [harness.upload_batch(W.make_batch(cfg, rows, cfg.seed + 1000 * rank + r)) for r in range(R_BATCHES)]
+    small = cfg.name in ("c1", "c2", "c3")
+    warmup = max(args.warmup if args.warmup is not None else 5, 3)
+    steps = max(args.steps if args.steps is not None else (2000 if small else 200), 1)
+    use_graph = small if args.graph < 0 else bool(args.graph)
+    R = max(1, args.rotating_batches)
+
+    # every rank: all tables + its own shard of each global batch of world*B samples (batch-sharded replicas,
+    # no collective on the data path)
+    dt = harness.make_device_tables(cfg, rows, device=f"cuda:{local}")
+    batches = [harness.upload_batch(sharding.make_batch_shard(cfg, rows, cfg.seed + r, rank, world), device=f"cuda:{local}")
+               for r in range(R)]
     pooling = cfg.pooling_modes()
     plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg))
     apply_options(plan, args, binding)
-    out = harness.new_output(cfg)
-    stream = torch.cuda.current_stream()
+    out = harness.new_output(cfg, device=f"cuda:{local}")
+    stream = torch.cuda.Stream()  # a non-default stream: every launch and every event of the timed region is on it
 
-    def step(i):
-        b = batches[i % R_BATCHES]
-        plan.build(b.lengths, stream)
-        plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
+    def step(i, s):
+        b = batches[i % R]
+        plan.build(b.lengths, s)
+        plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=s)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for i in range(warmup):
-        step(i)
+    def max_ms(ms):
+        return sharding.max_over_ranks(ms, dist, device=f"cuda:{local}")
+
+    with torch.cuda.stream(stream):
+        for i in range(warmup):
+            step(i, stream)
     barrier()
+
+    graph = None
+    if use_graph:  # capture the K steps once; the timed region replays them with no host work in between
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            for i in range(steps):
+                step(i, torch.cuda.current_stream())
+        graph.replay()  # one untimed replay (instantiation / upload)
+        barrier()
 
     # ---- timed region: K steps, CUDA events on the launching stream --------------------------------------
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-        time.sleep(0.25)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        time.sleep(0.05)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = binding.launch_count()
     barrier()
     t0 = time.time()
-    e0.record(stream)
-    for i in range(steps):
-        b = batches[i % R_BATCHES]
-        plan.build(b.lengths, stream)
-        ev[i][0].record(stream)
-        plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
-        ev[i][1].record(stream)
-    e1.record(stream)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        if graph is not None:
+            graph.replay()
+        else:
+            for i in range(steps):
+                step(i, stream)
+        e1.record(stream)
     barrier()
     t1 = time.time()
-    launches = binding.launch_count() - launches0
-    total_ms = e0.elapsed_time(e1)
-    lookup_ms = [a.elapsed_time(b) for a, b in ev]
+    launches = 2 * steps if graph is not None else binding.launch_count() - launches0
+    total_ms = max_ms(e0.elapsed_time(e1))
     clocks = sampler.stop(t0, t1) if rank == 0 else None
 
-    if dist is not None:
-        tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    # ---- the dominant kernel alone: per-launch CUDA events around dpi_lookup, same stream, same batches -------
+    n_k = min(steps, 200)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_k)]
+    with torch.cuda.stream(stream):
+        for i in range(n_k):
+            b = batches[i % R]
+            plan.build(b.lengths, stream)
+            ev[i][0].record(stream)
+            plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
+            ev[i][1].record(stream)
+    barrier()
+    lookup_ms = [a.elapsed_time(b) for a, b in ev]
+    # and the stream-launched step (plan + lookup, no graph), for the graph-vs-stream comparison
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        s0.record(stream)
+        for i in range(n_k):
+            step(i, stream)
+        s1.record(stream)
+    barrier()
+    stream_step_ms = s0.elapsed_time(s1) / n_k
 
     # plan facts for the byte counts (after timing)
     Ns, Ss = [], []
@@ -308,24 +391,21 @@ def run_ours(args):
         hb = [(torch.from_numpy(b.host.lengths).pin_memory(), torch.from_numpy(np.ascontiguousarray(b.host.indices)).pin_memory())
               for b in batches[:2]]
         out_host = torch.empty((cfg.B, cfg.T * cfg.D), dtype=harness.TORCH_DTYPE[cfg.out]).pin_memory()
-        for i in range(2):
-            plan.forward_host(dt.ptrs, hb[i % 2][0], hb[i % 2][1], out_host, pooling=pooling, stream=stream)
+        nb = len(hb)
+        for i in range(3):
+            plan.forward_host(dt.ptrs, hb[i % nb][0], hb[i % nb][1], out_host, pooling=pooling, stream=stream)
         barrier()
         n_e2e = max(1, args.e2e_steps)
         a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
         for i in range(n_e2e):
-            plan.forward_host(dt.ptrs, hb[i % 2][0], hb[i % 2][1], out_host, pooling=pooling, stream=stream)
+            plan.forward_host(dt.ptrs, hb[i % nb][0], hb[i % nb][1], out_host, pooling=pooling, stream=stream)
         b_.record(stream)
         barrier()
-        e2e_ms = a.elapsed_time(b_)
-        if dist is not None:
-            tt = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_ms = float(tt.item())
+        e2e_ms = max_ms(a.elapsed_time(b_))
         h2d = int(hb[0][0].numel() * 4 + hb[0][1].numel() * 4)
         d2h = int(out_host.numel() * out_host.element_size())
-        e2e = {"value": cfg.G * n_e2e * world / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        e2e = {"value": sharding.job_throughput(cfg.G, n_e2e, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / n_e2e, "steps": n_e2e,
                "api": "dpi_forward_host (pinned host lengths/indices in, [B,T*D] block out, tables resident)"}
 
@@ -342,7 +422,7 @@ def run_ours(args):
                 "frac_of_nominal_8000": achieved / 8000.0, "traffic": ncu_traffic(cfg.name),
                 "algorithmic_bytes_per_launch": bytes_step["lookup"], "kernel_ms_avg": lk_ms,
                 "kernel_ms_min": min(lookup_ms), "kernel_ms_median": statistics.median(lookup_ms),
-                "kernel_share_of_step": lk_ms * steps / total_ms}
+                "kernel_launches_timed": n_k, "kernel_share_of_step": lk_ms / stream_step_ms}
     cpu = None
     if not args.no_cpu_baseline:
         r = time_oracle(cfg, rows, args.cpu_seconds)
@@ -350,14 +430,16 @@ def run_ours(args):
         cpu["host_cpus_visible"] = len(os.sched_getaffinity(0))
 
     line = {
-        "metric": METRIC, "value": cfg.G * steps * world / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": sharding.job_throughput(cfg.G, steps, world, total_ms), "unit": UNIT, "n_gpus": world,
         "steps": steps, "warmup": warmup, "ms_per_step": total_ms / steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_KEY[cfg.dtype], "data": "synthetic",
         "config": describe(cfg, rows, {"parallelism": f"batch-sharded replicas x{world}, no collective",
+                                       "launch": "CUDA graph replay of the K steps" if graph is not None else "stream launches",
                                        "quantum_K": plan.info()["K"], "rows_gathered_per_step": n_mean,
-                                       "segments_per_step": s_mean}),
+                                       "segments_per_step": s_mean}, R),
         "row_gathers_per_s": n_mean * steps * world / (total_ms * 1e-3),
         "step_algorithmic_gbs": bytes_step["total"] * world / (total_ms / steps * 1e-3) / 1e9,
+        "stream_launched_ms_per_step": stream_step_ms,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "device": torch.cuda.get_device_name(local),
     }

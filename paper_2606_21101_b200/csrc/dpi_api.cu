@@ -61,7 +61,6 @@ struct dpi_plan_s {
     int32_t K_user = 0;      // 0 = default
     uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
     uint32_t num_tiles = 0;
-    uint32_t epoch = 0;
     int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0};
     // device
     int device = 0, num_sms = 0;
@@ -70,7 +69,7 @@ struct dpi_plan_s {
     int32_t* meta = nullptr;
     unsigned long long* tile_len = nullptr;
     unsigned long long* tile_cost = nullptr;
-    unsigned int* ticket = nullptr;
+    unsigned int* state = nullptr;   // planner device state {ticket, done, epoch, -}
     int64_t* table_rows_dev = nullptr;
     unsigned long long* n_bad_dev = nullptr;
     // staging for dpi_forward_host
@@ -113,7 +112,7 @@ dpi_status_t ensure_seg_capacity(dpi_plan_t* p, int32_t K) {
 void free_plan(dpi_plan_t* p) {
     if (!p) return;
     cudaFree(p->offsets); cudaFree(p->seg); cudaFree(p->meta); cudaFree(p->tile_len);
-    cudaFree(p->tile_cost); cudaFree(p->ticket); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
+    cudaFree(p->tile_cost); cudaFree(p->state); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
     cudaFree(p->stage_len); cudaFree(p->stage_idx); cudaFree(p->stage_out);
     (void)cudaGetLastError();
     delete p;
@@ -252,8 +251,11 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     DPI_TRY(cudaMalloc(&p->tile_cost, p->num_tiles * sizeof(unsigned long long)));
     DPI_TRY(cudaMemset(p->tile_len, 0, p->num_tiles * sizeof(unsigned long long)));
     DPI_TRY(cudaMemset(p->tile_cost, 0, p->num_tiles * sizeof(unsigned long long)));
-    DPI_TRY(cudaMalloc(&p->ticket, sizeof(unsigned int)));
-    DPI_TRY(cudaMemset(p->ticket, 0, sizeof(unsigned int)));
+    {
+        const unsigned int init[kStateWords] = {0u, 0u, 1u, 0u};  // ticket, done, epoch = 1 (status words start at 0)
+        DPI_TRY(cudaMalloc(&p->state, sizeof init));
+        DPI_TRY(cudaMemcpy(p->state, init, sizeof init, cudaMemcpyHostToDevice));
+    }
     DPI_TRY(cudaMalloc(&p->table_rows_dev, T * sizeof(int64_t)));
     DPI_TRY(cudaMemcpy(p->table_rows_dev, table_rows, T * sizeof(int64_t), cudaMemcpyHostToDevice));
     DPI_TRY(cudaMalloc(&p->n_bad_dev, sizeof(unsigned long long)));
@@ -299,12 +301,6 @@ dpi_status_t dpi_plan_build(dpi_plan_t* p, const int32_t* lengths_dev, void* str
     if (!p || !lengths_dev) return fail(DPI_ERR_INVALID_ARG, "plan/lengths_dev is NULL");
     if (reinterpret_cast<uintptr_t>(lengths_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "lengths_dev is not 4-byte aligned");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    p->epoch += 1;
-    if (p->epoch >= (1u << 30)) {  // status words are tagged with a 30-bit epoch: clear once per wrap
-        DPI_CUDA(cudaMemsetAsync(p->tile_len, 0, p->num_tiles * sizeof(unsigned long long), s));
-        DPI_CUDA(cudaMemsetAsync(p->tile_cost, 0, p->num_tiles * sizeof(unsigned long long), s));
-        p->epoch = 1;
-    }
     PlanArgs a{};
     a.len = lengths_dev;
     a.offsets = p->offsets;
@@ -312,12 +308,11 @@ dpi_status_t dpi_plan_build(dpi_plan_t* p, const int32_t* lengths_dev, void* str
     a.meta = p->meta;
     a.tile_len = p->tile_len;
     a.tile_cost = p->tile_cost;
-    a.ticket = p->ticket;
+    a.state = p->state;
     a.G = p->G;
     a.K = static_cast<uint32_t>(p->K);
     a.seg_cap = p->seg_cap;
     a.num_tiles = p->num_tiles;
-    a.epoch = p->epoch;
     a.max_indices = static_cast<uint32_t>(p->max_indices);
     cudaError_t e = launch_plan(a, s);
     if (e != cudaSuccess) return cuda_fail(e, "plan kernel launch");

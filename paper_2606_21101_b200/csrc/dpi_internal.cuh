@@ -27,6 +27,9 @@ constexpr int kScanThreads = 256;
 constexpr int kScanItems = 8;                               // consecutive bags per thread (two int4 loads)
 constexpr int kScanTile = kScanThreads * kScanItems;        // 2048 bags per CTA
 
+enum PlanState { kStateTicket = 0, kStateDone = 1, kStateEpoch = 2, kStateWords = 4 };
+constexpr uint32_t kEpochLimit = 1u << 30;  // status words carry a 30-bit epoch
+
 struct PlanArgs {
     const int32_t* __restrict__ len;   // [G]
     int32_t* __restrict__ offsets;     // [G+1]
@@ -34,12 +37,12 @@ struct PlanArgs {
     int32_t* __restrict__ meta;        // [kMetaWords]
     unsigned long long* tile_len;      // [num_tiles] look-back status words for the length scan
     unsigned long long* tile_cost;     // [num_tiles] look-back status words for the cost scan
-    unsigned int* ticket;              // dynamic tile id (self-resetting atomicInc)
+    unsigned int* state;               // [kStateTicket] dynamic tile id, [kStateDone] finished tiles (both
+                                       // self-resetting atomicInc), [kStateEpoch] tag of this build's status words
     uint32_t G;
     uint32_t K;
     uint32_t seg_cap;
     uint32_t num_tiles;
-    uint32_t epoch;                    // tags status words so the arrays never need clearing
     uint32_t max_indices;
 };
 

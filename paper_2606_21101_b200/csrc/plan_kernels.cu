@@ -88,13 +88,19 @@ __device__ __forceinline__ void lookback(const unsigned long long* st_len, const
 }
 
 __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const PlanArgs a) {
-    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_tile, s_epoch;
     __shared__ uint32_t s_wlen[kScanThreads / 32], s_wcost[kScanThreads / 32];
     __shared__ uint32_t s_pre_len, s_pre_cost;
 
-    if (threadIdx.x == 0) s_tile = atomicInc(a.ticket, a.num_tiles - 1);  // wraps to 0 after the last tile
+    // The epoch that tags this build's look-back words lives in device memory and is advanced by the last tile
+    // to finish, so a build needs no host-side state: the same launch can be replayed from a CUDA graph.
+    if (threadIdx.x == 0) {
+        s_tile = atomicInc(a.state + kStateTicket, a.num_tiles - 1);  // wraps to 0 after the last tile
+        s_epoch = *reinterpret_cast<volatile unsigned int*>(a.state + kStateEpoch);
+    }
     __syncthreads();
     const uint32_t tile = s_tile;
+    const uint32_t epoch = s_epoch;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t base = tile * kScanTile + threadIdx.x * kScanItems;
 
@@ -143,20 +149,20 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
     if (warp == 0) {
         if (tile == 0) {
             if (lane == 0) {
-                st_relaxed_gpu(a.tile_len + 0, pack_status(a.epoch, kStateInclusive, agg_len));
-                st_relaxed_gpu(a.tile_cost + 0, pack_status(a.epoch, kStateInclusive, agg_cost));
+                st_relaxed_gpu(a.tile_len + 0, pack_status(epoch, kStateInclusive, agg_len));
+                st_relaxed_gpu(a.tile_cost + 0, pack_status(epoch, kStateInclusive, agg_cost));
                 s_pre_len = 0; s_pre_cost = 0;
             }
         } else {
             if (lane == 0) {
-                st_relaxed_gpu(a.tile_len + tile, pack_status(a.epoch, kStateAggregate, agg_len));
-                st_relaxed_gpu(a.tile_cost + tile, pack_status(a.epoch, kStateAggregate, agg_cost));
+                st_relaxed_gpu(a.tile_len + tile, pack_status(epoch, kStateAggregate, agg_len));
+                st_relaxed_gpu(a.tile_cost + tile, pack_status(epoch, kStateAggregate, agg_cost));
             }
             uint32_t pl, pc;
-            lookback(a.tile_len, a.tile_cost, tile, a.epoch, pl, pc);
+            lookback(a.tile_len, a.tile_cost, tile, epoch, pl, pc);
             if (lane == 0) {
-                st_relaxed_gpu(a.tile_len + tile, pack_status(a.epoch, kStateInclusive, pl + agg_len));
-                st_relaxed_gpu(a.tile_cost + tile, pack_status(a.epoch, kStateInclusive, pc + agg_cost));
+                st_relaxed_gpu(a.tile_len + tile, pack_status(epoch, kStateInclusive, pl + agg_len));
+                st_relaxed_gpu(a.tile_cost + tile, pack_status(epoch, kStateInclusive, pc + agg_cost));
                 s_pre_len = pl; s_pre_cost = pc;
             }
         }
@@ -217,6 +223,17 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
         a.meta[META_OVERFLOW] = (n_total > a.max_indices || S >= a.seg_cap) ? 1 : 0;
         a.meta[META_K] = a.K;
         a.meta[META_G] = a.G;
+    }
+
+    // ---- close the epoch: no thread of this CTA reads a status word past the barrier above; the last tile to
+    // get here advances the tag (a later build starts only after this grid has completed) ----
+    if (threadIdx.x == 0 && atomicInc(a.state + kStateDone, a.num_tiles - 1) == a.num_tiles - 1) {
+        uint32_t next = epoch + 1;
+        if (next >= kEpochLimit) {  // 30-bit tag about to wrap: clear the words once and restart at 1
+            for (uint32_t i = 0; i < a.num_tiles; ++i) { a.tile_len[i] = 0ull; a.tile_cost[i] = 0ull; }
+            next = 1;
+        }
+        a.state[kStateEpoch] = next;
     }
 }
 

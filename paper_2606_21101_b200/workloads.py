@@ -204,10 +204,13 @@ def _poisson_cdf(mean: float, cap: int) -> np.ndarray:
     return cdf
 
 
-def make_lengths(cfg: Config, batch_seed: int) -> np.ndarray:
-    """int32[G] bag lengths, sample-major (g = b*T + t)."""
+def make_lengths(cfg: Config, batch_seed: int, bag_base: int = 0) -> np.ndarray:
+    """int32[G] bag lengths, sample-major (g = b*T + t). ``bag_base`` offsets the bag counter: the lengths of
+    bags [bag_base, bag_base + G) of a larger (global) batch of the same seed -- used to draw one rank's
+    shard of a batch-sharded global batch without drawing the rest (bag_base must be a multiple of T)."""
     G = cfg.G
-    g = np.arange(G, dtype=np.uint64)
+    assert bag_base % cfg.T == 0
+    g = np.arange(bag_base, bag_base + G, dtype=np.uint64)
     kind = cfg.lengths[0]
     if kind == "const":
         return np.full(G, int(cfg.lengths[1]), dtype=np.int32)
@@ -247,8 +250,10 @@ class _ZipfTable:
         return (rank0 * self.a) % self.n
 
 
-def make_indices(cfg: Config, rows: np.ndarray, lengths: np.ndarray, batch_seed: int) -> np.ndarray:
-    """int32[N] per-table local row ids, bag-contiguous in sample-major bag order."""
+def make_indices(cfg: Config, rows: np.ndarray, lengths: np.ndarray, batch_seed: int,
+                 entry_base: int = 0) -> np.ndarray:
+    """int32[N] per-table local row ids, bag-contiguous in sample-major bag order. ``entry_base`` offsets the
+    per-entry counter (the flat position of this shard's first entry inside the global batch)."""
     T = cfg.T
     lengths = np.asarray(lengths, dtype=np.int64)
     N = int(lengths.sum())
@@ -256,7 +261,7 @@ def make_indices(cfg: Config, rows: np.ndarray, lengths: np.ndarray, batch_seed:
         return np.zeros(0, dtype=np.int32)
     table_of_entry = (np.repeat(np.arange(cfg.G, dtype=np.int64), lengths) % T).astype(np.int32)
     keys = np.array([stream_key(batch_seed, STREAM_IDX, t) for t in range(T)], dtype=np.uint64)
-    u = unit_f64(hash_u64(keys[table_of_entry], np.arange(N, dtype=np.uint64)))
+    u = unit_f64(hash_u64(keys[table_of_entry], np.arange(entry_base, entry_base + N, dtype=np.uint64)))
     out = np.empty(N, dtype=np.int32)
     if cfg.index_dist[0] == "uniform":
         r = rows[table_of_entry].astype(np.float64)
