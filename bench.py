@@ -47,8 +47,9 @@ def parse_args():
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--mode", type=int, default=0)
-    ap.add_argument("--row-l1-no-alloc", type=int, default=-1)
     ap.add_argument("--pdl", type=int, default=0)
+    ap.add_argument("--kernel", default="output_first", choices=["output_first", "input_first"],
+                    help="input_first = the paper's strawman mapping (ablation, PAPER.md:172-176)")
     ap.add_argument("--graph", type=int, default=-1, help="1: time a CUDA-graph replay of the K steps; 0: stream launches; -1: auto (graph for c1-c3)")
     ap.add_argument("--rotating-batches", type=int, default=R_BATCHES)
     ap.add_argument("--e2e-steps", type=int, default=8)
@@ -72,12 +73,17 @@ def measured_peak():
 
 
 def ncu_traffic(workload: str):
-    """dram bytes per lookup launch from the committed ncu --set full capture, if one exists for this workload."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per lookup launch from the committed `ncu --set full` capture
+    of this workload (profiles/ncu_traffic.csv, written from the .ncu-rep), or None if there is none."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(workload, {}).get("dram_bytes_per_launch")
+        import csv
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["kernel"] == "lookup_kernel":
+                    return float(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -180,7 +186,6 @@ def apply_options(plan, args, binding):
     plan.set_option(binding.OPT_BLOCK_THREADS, args.block_threads)
     plan.set_option(binding.OPT_BLOCKS_PER_SM, args.blocks_per_sm)
     plan.set_option(binding.OPT_MODE, args.mode)
-    plan.set_option(binding.OPT_ROW_L1_NO_ALLOC, args.row_l1_no_alloc)
     plan.set_option(binding.OPT_PDL, args.pdl)
 
 
@@ -303,10 +308,12 @@ def run_ours(args):
     out = harness.new_output(cfg, device=f"cuda:{local}")
     stream = torch.cuda.Stream()  # a non-default stream: every launch and every event of the timed region is on it
 
+    lookup = plan.lookup if args.kernel == "output_first" else plan.lookup_input_first
+
     def step(i, s):
         b = batches[i % R]
         plan.build(b.lengths, s)
-        plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=s)
+        lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=s)
 
     def barrier():
         if dist is not None:
@@ -361,7 +368,7 @@ def run_ours(args):
             b = batches[i % R]
             plan.build(b.lengths, stream)
             ev[i][0].record(stream)
-            plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
+            lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
             ev[i][1].record(stream)
     barrier()
     lookup_ms = [a.elapsed_time(b) for a, b in ev]
@@ -417,7 +424,7 @@ def run_ours(args):
     peak, peak_src = measured_peak()
     lk_ms = statistics.mean(lookup_ms)
     achieved = bytes_step["lookup"] / (lk_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "lookup_kernel (a3 fused gather-and-pool)", "achieved": achieved,
+    roofline = {"bound": "hbm", "kernel": "lookup_kernel (a3 fused gather-and-pool)" if args.kernel == "output_first" else "input_first_kernel (ablation)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "frac_of_nominal_8000": achieved / 8000.0, "traffic": ncu_traffic(cfg.name),
                 "algorithmic_bytes_per_launch": bytes_step["lookup"], "kernel_ms_avg": lk_ms,

@@ -72,7 +72,8 @@ typedef enum {
     DPI_OPT_BLOCKS_PER_SM = 2,  /* persistent grid = SMs * this; 0 = auto (occupancy) */
     DPI_OPT_MODE = 3,           /* 0 auto per task, 1 sub-warp per bag, 2 warp per bag (single-buffered),
                                    3 warp per bag (double-buffered batches) */
-    DPI_OPT_ROW_L1_NO_ALLOC = 4,/* 1: table rows bypass L1 (ld.global.nc.L1::no_allocate); 0: default; -1 auto */
+    DPI_OPT_ROW_L1_NO_ALLOC = 4,/* reserved: accepts -1 / 0 only. Rows always allocate in L1; the L1::no_allocate
+                                   variant measured 17-20 % slower on B200 and was removed */
     DPI_OPT_PDL = 5,            /* 1: lookup is launched with programmatic dependent launch after the planner */
     DPI_OPT_COUNT_
 } dpi_option_t;
@@ -154,6 +155,17 @@ dpi_status_t dpi_plan_export(const dpi_plan_t* plan, int32_t* offsets_host, int3
 dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indices_dev,
                         const int32_t* offsets_dev, const dpi_plan_t* plan, const uint8_t* pooling,
                         void* out_dev, void* stream);
+
+/*
+ * dpi_lookup_input_first -- ABLATION, not the product path: the same lookup with the paper's strawman
+ * "input-first" workload allocation (different samples on different threads, so table reads
+ * and output writes of a warp are random), kept to measure the paper's Fig. 11 claim (output-first up to 10.3x
+ * faster) on B200. Same arguments, results and error behaviour as dpi_lookup; it uses only the
+ * plan's offsets (no segments), one thread per sample.
+ */
+dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int32_t* indices_dev,
+                                    const int32_t* offsets_dev, const dpi_plan_t* plan, const uint8_t* pooling,
+                                    void* out_dev, void* stream);
 
 /*
  * dpi_forward_host -- the whole path (a1+a2+a3) for callers whose sparse inputs live in HOST memory

@@ -21,11 +21,11 @@ OBJDIR = os.path.join(HERE, "build")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 LIBS = {
-    "libdpi.so": ["dpi_api.cu", "plan_kernels.cu", "lookup_f32.cu", "lookup_f16.cu", "lookup_bf16.cu"],
+    "libdpi.so": ["dpi_api.cu", "plan_kernels.cu", "lookup_f32.cu", "lookup_f16.cu", "lookup_bf16.cu",
+                  "ablation_input_first.cu"],
     "libdpi_synth.so": ["synth_fill.cu"],
 }
 HEADERS = ["dpi_internal.cuh", "lookup_kernels.cuh", "lookup_dispatch.inc", os.path.join(INCLUDE, "dpi.h")]

@@ -120,7 +120,6 @@ void free_plan(dpi_plan_t* p) {
 
 struct LaunchChoice {
     LookupLaunch l;
-    int row_no_alloc;
 };
 
 int occupancy(const dpi_plan_t* p, int lanes, int unroll, int threads) {
@@ -147,13 +146,11 @@ LaunchChoice choose_launch(const dpi_plan_t* p) {
     if (need < c.l.grid) c.l.grid = static_cast<int>(need > 0 ? need : 1);
     c.l.pdl = p->opt[DPI_OPT_PDL] != 0;
     c.l.out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
-    // auto: let rows allocate in L1 -- measured +17 % on c5 and +20 % on c4 over L1::no_allocate (sweeps_r01.md)
-    c.row_no_alloc = p->opt[DPI_OPT_ROW_L1_NO_ALLOC] < 0 ? 0 : p->opt[DPI_OPT_ROW_L1_NO_ALLOC];
     return c;
 }
 
 dpi_status_t do_lookup(const dpi_plan_t* p, const void* const* tables, const int32_t* indices, const int32_t* offsets,
-                       const uint8_t* pooling, void* out, cudaStream_t stream) {
+                       const uint8_t* pooling, void* out, cudaStream_t stream, bool input_first = false) {
     LookupArgs a{};
     a.tables = tables;
     a.indices = indices;
@@ -172,8 +169,12 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const void* const* tables, const int
             if (pooling[t] == DPI_POOL_MEAN) a.pool.w[t >> 5] |= 1u << (t & 31);
         }
     }
+    if (input_first) {
+        cudaError_t e = launch_input_first(a, static_cast<uint32_t>(p->B), p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "input-first kernel launch");
+        return DPI_OK;
+    }
     const LaunchChoice c = choose_launch(p);
-    a.row_no_alloc = c.row_no_alloc;
     cudaError_t e;
     switch (p->dtype) {
         case DPI_F32: e = launch_lookup_f32(a, c.l, stream); break;
@@ -282,7 +283,7 @@ dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
         case DPI_OPT_BLOCK_THREADS: ok = v == 0 || (v >= 32 && v <= 256 && v % 32 == 0); break;
         case DPI_OPT_BLOCKS_PER_SM: ok = v >= 0 && v <= 32; break;
         case DPI_OPT_MODE: ok = v >= 0 && v <= 3; break;
-        case DPI_OPT_ROW_L1_NO_ALLOC: ok = v >= -1 && v <= 1; break;
+        case DPI_OPT_ROW_L1_NO_ALLOC: ok = v == -1 || v == 0; break;  // the bypass variant was removed (see dpi.h)
         case DPI_OPT_PDL: ok = v == 0 || v == 1; break;
         default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);
     }
@@ -398,6 +399,17 @@ dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indice
     if (reinterpret_cast<uintptr_t>(out_dev) & out_align) return fail(DPI_ERR_INVALID_ARG, "out_dev is not %d-byte aligned", (int)out_align + 1);
     if (reinterpret_cast<uintptr_t>(indices_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "indices_dev is not 4-byte aligned");
     return do_lookup(p, table_ptrs_dev, indices_dev, offsets_dev, pooling, out_dev, static_cast<cudaStream_t>(stream));
+}
+
+dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,
+                                    const dpi_plan_t* p, const uint8_t* pooling, void* out_dev, void* stream) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built (call dpi_plan_build first)");
+    if (!table_ptrs_dev || !out_dev) return fail(DPI_ERR_INVALID_ARG, "table_ptrs_dev/out_dev is NULL");
+    if (!indices_dev && p->max_indices > 0) return fail(DPI_ERR_INVALID_ARG, "indices_dev is NULL");
+    const uintptr_t out_align = (p->dtype != DPI_F32 && p->out_dtype == DPI_F32) ? 31u : 15u;
+    if (reinterpret_cast<uintptr_t>(out_dev) & out_align) return fail(DPI_ERR_INVALID_ARG, "out_dev is not %d-byte aligned", (int)out_align + 1);
+    return do_lookup(p, table_ptrs_dev, indices_dev, offsets_dev, pooling, out_dev, static_cast<cudaStream_t>(stream), true);
 }
 
 dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, const int32_t* lengths_host,

@@ -70,7 +70,6 @@ struct LookupArgs {
     uint32_t T;
     uint32_t nvec;                           // 16-byte vectors per row = D*sizeof(elt)/16
     int32_t mode;                            // 0 auto, 1 sub-warp per bag, 2 warp per bag
-    int32_t row_no_alloc;                    // 1: rows bypass L1
     PoolMask pool;
 };
 
@@ -91,6 +90,9 @@ cudaError_t launch_lookup_bf16(const LookupArgs& a, const LookupLaunch& l, cudaS
 int lookup_occupancy_f32(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
 int lookup_occupancy_f16(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
 int lookup_occupancy_bf16(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
+
+// Ablation (ablation_input_first.cu): one thread per sample.
+cudaError_t launch_input_first(const LookupArgs& a, uint32_t B, int dtype, bool out32, cudaStream_t stream);
 
 void count_launch();
 

@@ -34,15 +34,15 @@ constexpr int kWarpStageInts = 2 * kStageIdx + 2 * kStageOff;
 constexpr int kLookupMaxThreads = 256;  // natural register allocation (64-80/thread); a 512 bound made ptxas spill
 
 // ---- memory helpers ----------------------------------------------------------------------------------
-// Predicated 128-bit read-only load; lanes with pred == false get zeros and issue no memory request.
-__device__ __forceinline__ uint4 ld_row16(const void* p, bool pred, int no_alloc) {
+// Predicated 128-bit read-only load; lanes with pred == false get zeros and issue no memory request. Rows are
+// allowed to allocate in L1 (the unified 256 KB L1/smem): on B200 that measured +17 % (c5) and +20 % (c4) over
+// ld.global.nc.L1::no_allocate -- the Zipf head of a table is re-read by neighbouring warps of the same SM,
+// and with 256 B rows both 128 B lines of a row are requested by one warp-wide load anyway.
+__device__ __forceinline__ uint4 ld_row16(const void* p, bool pred) {
     uint4 r = make_uint4(0u, 0u, 0u, 0u);
     asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t"
-        "@p ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];\n\t}"
-        : "+r"(r.x), "+r"(r.y), "+r"(r.z), "+r"(r.w) : "l"(p), "r"(static_cast<int>(pred && no_alloc)));
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t"
         "@p ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];\n\t}"
-        : "+r"(r.x), "+r"(r.y), "+r"(r.z), "+r"(r.w) : "l"(p), "r"(static_cast<int>(pred && !no_alloc)));
+        : "+r"(r.x), "+r"(r.y), "+r"(r.z), "+r"(r.w) : "l"(p), "r"(static_cast<int>(pred)));
     return r;
 }
 // streaming stores: the output block is consumed by the next layer, not re-read here
@@ -63,34 +63,38 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ---- per-dtype arithmetic ----------------------------------------------------------------------------
+// Accumulators are fp32 pairs so that every add is one sm_100 packed add.rn.f32x2 (FADD2): the kernel is
+// issue-bound on L2-resident workloads (c3/c4), and FADD2 halves the adds per 16-byte vector.
+__device__ __forceinline__ void add2(float2& a, float x, float y) { a = __fadd2_rn(a, make_float2(x, y)); }
+
 struct F32Traits {
-    static constexpr int kAcc = 4;
+    static constexpr int kAcc = 4;   // fp32 accumulators per lane (one 16-byte vector of the row)
     static constexpr int kEltBytes = 4;
-    __device__ static __forceinline__ void add(float (&acc)[4], const uint4& v) {
-        acc[0] += __uint_as_float(v.x); acc[1] += __uint_as_float(v.y);
-        acc[2] += __uint_as_float(v.z); acc[3] += __uint_as_float(v.w);
+    __device__ static __forceinline__ void add(float2 (&acc)[2], const uint4& v) {
+        add2(acc[0], __uint_as_float(v.x), __uint_as_float(v.y));
+        add2(acc[1], __uint_as_float(v.z), __uint_as_float(v.w));
     }
-    __device__ static __forceinline__ uint4 pack(const float (&acc)[4]) {
-        return make_uint4(__float_as_uint(acc[0]), __float_as_uint(acc[1]), __float_as_uint(acc[2]),
-                          __float_as_uint(acc[3]));
+    __device__ static __forceinline__ uint4 pack(const float2 (&acc)[2]) {
+        return make_uint4(__float_as_uint(acc[0].x), __float_as_uint(acc[0].y), __float_as_uint(acc[1].x),
+                          __float_as_uint(acc[1].y));
     }
 };
 struct F16Traits {
     static constexpr int kAcc = 8;
     static constexpr int kEltBytes = 2;
-    __device__ static __forceinline__ void add(float (&acc)[8], const uint4& v) {
+    __device__ static __forceinline__ void add(float2 (&acc)[4], const uint4& v) {
         const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w[i]));
-            acc[2 * i] += f.x; acc[2 * i + 1] += f.y;
+            acc[i] = __fadd2_rn(acc[i], f);
         }
     }
-    __device__ static __forceinline__ uint4 pack(const float (&acc)[8]) {
+    __device__ static __forceinline__ uint4 pack(const float2 (&acc)[4]) {
         uint32_t w[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            const __half2 h = __floats2half2_rn(acc[2 * i], acc[2 * i + 1]);
+            const __half2 h = __floats2half2_rn(acc[i].x, acc[i].y);
             w[i] = *reinterpret_cast<const uint32_t*>(&h);
         }
         return make_uint4(w[0], w[1], w[2], w[3]);
@@ -99,46 +103,59 @@ struct F16Traits {
 struct BF16Traits {
     static constexpr int kAcc = 8;
     static constexpr int kEltBytes = 2;
-    __device__ static __forceinline__ void add(float (&acc)[8], const uint4& v) {
+    __device__ static __forceinline__ void add(float2 (&acc)[4], const uint4& v) {
         const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {  // bf16 -> fp32 is a 16-bit shift
-            acc[2 * i] += __uint_as_float(w[i] << 16);
-            acc[2 * i + 1] += __uint_as_float(w[i] & 0xffff0000u);
-        }
+        for (int i = 0; i < 4; ++i)  // bf16 -> fp32 is a 16-bit shift (low element) or a mask (high element)
+            add2(acc[i], __uint_as_float(w[i] << 16), __uint_as_float(w[i] & 0xffff0000u));
     }
-    __device__ static __forceinline__ uint4 pack(const float (&acc)[8]) {
+    __device__ static __forceinline__ uint4 pack(const float2 (&acc)[4]) {
         uint32_t w[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            const __nv_bfloat162 h = __floats2bfloat162_rn(acc[2 * i], acc[2 * i + 1]);
+            const __nv_bfloat162 h = __floats2bfloat162_rn(acc[i].x, acc[i].y);
             w[i] = *reinterpret_cast<const uint32_t*>(&h);
         }
         return make_uint4(w[0], w[1], w[2], w[3]);
     }
 };
 
-template <int N>
-__device__ __forceinline__ void scale_mean(float (&acc)[N], int len) {
-    const float L = static_cast<float>(len);
+template <int N2>
+__device__ __forceinline__ void zero_acc(float2 (&acc)[N2]) {
 #pragma unroll
-    for (int i = 0; i < N; ++i) acc[i] = __fdiv_rn(acc[i], L);
+    for (int i = 0; i < N2; ++i) acc[i] = make_float2(0.f, 0.f);
+}
+
+// Mean pooling: one IEEE reciprocal of the bag length, then packed multiplies (R8: divide vs
+// multiply-by-reciprocal differ by <= 1 ulp of fp32, far inside the tolerance; bags with L <= 1 skip this and
+// stay bit-exact). The eight IEEE divisions this replaces cost ~15 instructions each.
+template <int N2>
+__device__ __forceinline__ void scale_mean(float2 (&acc)[N2], int len) {
+    const float inv = __frcp_rn(static_cast<float>(len));
+    const float2 inv2 = make_float2(inv, inv);
+#pragma unroll
+    for (int i = 0; i < N2; ++i) acc[i] = __fmul2_rn(acc[i], inv2);
 }
 
 // Store one pooled vector of bag g: table dtype (16 B per lane) or fp32 (OUT32: 32 B per lane for 16-bit tables).
 template <class Tr, bool OUT32>
-__device__ __forceinline__ void store_pooled(char* out, size_t g, uint32_t nvec, int sl, const float (&acc)[Tr::kAcc]) {
+__device__ __forceinline__ void store_pooled(char* out, size_t g, uint32_t nvec, int sl, const float2 (&acc)[Tr::kAcc / 2]) {
     if constexpr (OUT32 && Tr::kAcc == 8) {
-        st_out32(out + g * (static_cast<size_t>(nvec) * 32) + sl * 32, acc);
+        const float f[8] = {acc[0].x, acc[0].y, acc[1].x, acc[1].y, acc[2].x, acc[2].y, acc[3].x, acc[3].y};
+        st_out32(out + g * (static_cast<size_t>(nvec) * 32) + sl * 32, f);
     } else {
         st_out16(out + g * (static_cast<size_t>(nvec) * 16) + sl * 16, Tr::pack(acc));
     }
 }
 
+// U = 2 (the default: double buffering makes it 2..4 row loads in flight per lane) is held to 64 registers so
+// that 4 CTAs = 32 warps stay resident per SM for every dtype (ptxas: 0-24 bytes of spill, all on cold paths);
+// the deeper unrolls keep their natural allocation (<= 80 registers, 3 CTAs).
 template <class Tr, int W, int U, bool OUT32>
-__global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupArgs a) {
+__global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kernel(const LookupArgs a) {
     constexpr int P = 32 / W;
     constexpr int kAcc = Tr::kAcc;
+    constexpr int kAcc2 = kAcc / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int lane = threadIdx.x & 31;
@@ -151,7 +168,6 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
     const uint32_t warp_id = blockIdx.x * warps_per_cta + warp_in_cta;
     const size_t row_bytes = static_cast<size_t>(a.nvec) * 16;
     char* const out = static_cast<char*>(a.out);
-    const int no_alloc = a.row_no_alloc;
 
     // smem: [T table base pointers][per warp: idx stage x2, offsets stage x2]
     const char** s_tab = reinterpret_cast<const char**>(smem_raw);
@@ -226,16 +242,15 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                         const bool ok = i < nb;
                         const uint32_t g = g_lo + (ok ? i : 0u);
                         const int r = ip[e_lo + (ok ? i : 0u)];
-                        v[u] = ld_row16(s_tab[g % a.T] + sl * 16 + static_cast<size_t>(r) * row_bytes, ok && vec_ok, no_alloc);
+                        v[u] = ld_row16(s_tab[g % a.T] + sl * 16 + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
                     }
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         const uint32_t i = i0 + u * P + sub;
                         if (i < nb && vec_ok) {
                             if constexpr (OUT32 && kAcc == 8) {
-                                float f[kAcc];
-#pragma unroll
-                                for (int k = 0; k < kAcc; ++k) f[k] = 0.f;
+                                float2 f[kAcc2];
+                                zero_acc(f);
                                 Tr::add(f, v[u]);
                                 store_pooled<Tr, OUT32>(out, g_lo + i, a.nvec, sl, f);
                             } else {
@@ -254,16 +269,15 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                     const int hi = active ? op[gc + 1] : lo;
                     const uint32_t t = gc % a.T;
                     const char* tab = s_tab[t] + sl * 16;
-                    float acc[kAcc];
-#pragma unroll
-                    for (int i = 0; i < kAcc; ++i) acc[i] = 0.f;
+                    float2 acc[kAcc2];
+                    zero_acc(acc);
                     for (int j = lo; j < hi; j += U) {
                         uint4 v[U];
 #pragma unroll
                         for (int u = 0; u < U; ++u) {
                             const bool ok = j + u < hi;
                             const int r = ip[ok ? j + u : lo];
-                            v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok, no_alloc);
+                            v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
                         }
 #pragma unroll
                         for (int u = 0; u < U; ++u) Tr::add(acc, v[u]);
@@ -279,9 +293,8 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                     const int lo = op[g], hi = op[g + 1];
                     const uint32_t t = g % a.T;
                     const char* tab = s_tab[t] + sl * 16;
-                    float acc[kAcc];
-#pragma unroll
-                    for (int i = 0; i < kAcc; ++i) acc[i] = 0.f;
+                    float2 acc[kAcc2];
+                    zero_acc(acc);
                     for (int j = lo; j < hi; j += P * U) {
                         uint4 v[U];
 #pragma unroll
@@ -289,7 +302,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                             const int e = j + u * P + sub;
                             const bool ok = e < hi;
                             const int r = ip[ok ? e : lo];
-                            v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok, no_alloc);
+                            v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
                         }
 #pragma unroll
                         for (int u = 0; u < U; ++u) Tr::add(acc, v[u]);
@@ -297,7 +310,9 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
 #pragma unroll
                     for (int d = W; d < 32; d <<= 1) {
 #pragma unroll
-                        for (int i = 0; i < kAcc; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], d);
+                        for (int i = 0; i < kAcc2; ++i)
+                            acc[i] = __fadd2_rn(acc[i], make_float2(__shfl_xor_sync(0xffffffffu, acc[i].x, d),
+                                                                    __shfl_xor_sync(0xffffffffu, acc[i].y, d)));
                     }
                     if (sub == 0 && vec_ok) {
                         if (((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
@@ -311,9 +326,8 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                 // loads per lane in flight across batch and bag boundaries instead of draining at each one.
                 auto store_zero = [&](uint32_t gz) {
                     if (sub == 0 && vec_ok) {
-                        float z[kAcc];
-#pragma unroll
-                        for (int i = 0; i < kAcc; ++i) z[i] = 0.f;
+                        float2 z[kAcc2];
+                        zero_acc(z);
                         store_pooled<Tr, OUT32>(out, gz, a.nvec, sl, z);
                     }
                 };
@@ -323,7 +337,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                         const int e = j + u * P + sub;
                         const bool ok = e < hi;
                         const int r = ip[ok ? e : j];
-                        v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok, no_alloc);
+                        v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
                     }
                 };
                 uint32_t g = g_lo;
@@ -337,9 +351,8 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
                 if (g < g_hi) {
                     int j = lo;
                     const char* tab = s_tab[g % a.T] + sl * 16;
-                    float acc[kAcc];
-#pragma unroll
-                    for (int i = 0; i < kAcc; ++i) acc[i] = 0.f;
+                    float2 acc[kAcc2];
+                    zero_acc(acc);
                     uint4 vA[U], vB[U];
                     issue(vA, j, hi, tab);
                     bool more = true;
@@ -368,15 +381,16 @@ __global__ void __launch_bounds__(kLookupMaxThreads) lookup_kernel(const LookupA
 #pragma unroll
                             for (int d = W; d < 32; d <<= 1) {
 #pragma unroll
-                                for (int i = 0; i < kAcc; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], d);
+                                for (int i = 0; i < kAcc2; ++i)
+                                    acc[i] = __fadd2_rn(acc[i], make_float2(__shfl_xor_sync(0xffffffffu, acc[i].x, d),
+                                                                            __shfl_xor_sync(0xffffffffu, acc[i].y, d)));
                             }
                             if (sub == 0 && vec_ok) {
                                 const uint32_t t = g % a.T;
                                 if (((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
                                 store_pooled<Tr, OUT32>(out, g, a.nvec, sl, acc);
                             }
-#pragma unroll
-                            for (int i = 0; i < kAcc; ++i) acc[i] = 0.f;
+                            zero_acc(acc);
                         }
                         g = g_n; j = j_n; lo = lo_n; hi = hi_n; tab = tab_n;
                         more = has_next;

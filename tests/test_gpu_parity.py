@@ -98,7 +98,7 @@ def test_plan_overflow_is_reported_not_out_of_bounds():
 # --------------------------------------------------------------------------------------------------
 # lookup (a3)
 # --------------------------------------------------------------------------------------------------
-def _run_gpu(cfg, dt, batch, pooling, K=0, opts=None, via_explicit_offsets=False):
+def _run_gpu(cfg, dt, batch, pooling, K=0, opts=None, via_explicit_offsets=False, input_first=False):
     db = harness.upload_batch(batch)
     plan = harness.make_plan(cfg, dt.rows, max(batch.N, 1))
     if K:
@@ -111,20 +111,23 @@ def _run_gpu(cfg, dt, batch, pooling, K=0, opts=None, via_explicit_offsets=False
     off_dev = None
     if via_explicit_offsets:
         off_dev = torch.from_numpy(host_offsets(batch.lengths)).cuda()
-    plan.lookup(dt.ptrs, db.indices, out, pooling=pooling, offsets_dev=off_dev)
+    if input_first:
+        plan.lookup_input_first(dt.ptrs, db.indices, out, pooling=pooling, offsets_dev=off_dev)
+    else:
+        plan.lookup(dt.ptrs, db.indices, out, pooling=pooling, offsets_dev=off_dev)
     torch.cuda.synchronize()
     res = harness.out_to_f64(out)
     plan.destroy()
     return res
 
 
-def _full_parity(cfg, K=0, opts=None, batch_seed=None, pooling=None):
+def _full_parity(cfg, K=0, opts=None, batch_seed=None, pooling=None, input_first=False):
     rows = cfg.table_rows()
     host_tables = [W.full_table_storage(cfg, t, int(rows[t])) for t in range(cfg.T)]
     dt = harness.tables_from_host(cfg, host_tables)
     batch = W.make_batch(cfg, rows, batch_seed)
     pooling = cfg.pooling_modes() if pooling is None else pooling
-    got = _run_gpu(cfg, dt, batch, pooling, K, opts)
+    got = _run_gpu(cfg, dt, batch, pooling, K, opts, input_first=input_first)
     ref = oracle_reference(host_tables, cfg.dtype, cfg.B, batch.lengths, batch.indices, pooling)
     return assert_outputs_match(got, ref, batch.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out)
 
@@ -161,6 +164,26 @@ def test_every_kernel_variant_gives_the_same_answer(unroll, mode):
 def test_any_quantum_gives_the_same_answer(K):
     cfg = W.Config("k", 3, (100, 1000, 10), 32, "f16", 500, ("poisson", 6.0, 40, 0.2), ("zipf", 1.2), "mean", 4)
     _full_parity(cfg, K=K)
+
+
+@pytest.mark.parametrize("dtype,D,out", [("f32", 16, None), ("f32", 24, None), ("f16", 32, None), ("bf16", 64, "f32"),
+                                         ("bf16", 8, None)])
+@pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 0, 5), ("poisson", 20.0, 100, 0.05)])
+def test_input_first_ablation_kernel_matches_the_oracle(dtype, D, out, lengths):
+    """The strawman mapping of PAPER.md:172-176 (one thread per sample) computes the same block."""
+    cfg = W.Config("if", 5, (1000, 17, 4000, 1, 250), D, dtype, 333, lengths, ("zipf", 1.05), "half", seed=12,
+                   out_dtype=out)
+    _full_parity(cfg, input_first=True)
+
+
+def test_input_first_c2_full_size_equals_output_first_bit_for_bit():
+    """One-hot (the paper's case): both mappings are pure row copies, so the blocks are identical."""
+    cfg = W.C2
+    dt = harness.make_device_tables(cfg)
+    batch = W.make_batch(cfg, dt.rows)
+    a = _run_gpu(cfg, dt, batch, cfg.pooling_modes())
+    b = _run_gpu(cfg, dt, batch, cfg.pooling_modes(), input_first=True)
+    assert np.array_equal(a, b)
 
 
 def test_degenerate_inputs():
