@@ -50,6 +50,8 @@ def _load():
         lib.oracle_alg1_onehot.restype = ctypes.c_int
         lib.oracle_lookup.argtypes = [i32, i32, i32, ctypes.c_int, vp, vp, vp, vp, vp, vp]
         lib.oracle_lookup.restype = ctypes.c_int
+        lib.oracle_lookup_general.argtypes = [i32, i32, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]
+        lib.oracle_lookup_general.restype = ctypes.c_int
         lib.oracle_plan.argtypes = [vp, i64, i32, vp, vp, vp, i64, vp]
         lib.oracle_plan.restype = ctypes.c_int
         lib.oracle_decode_f16.argtypes = [ctypes.c_uint16]
@@ -68,9 +70,11 @@ def _check(rc: int):
 _STORAGE = {F32: np.float32, F16: np.float16, BF16: np.uint16}
 
 
-def _table_ptrs(tables: Sequence[np.ndarray], dtype: int, D: int):
+def _table_ptrs(tables: Sequence[np.ndarray], dtype: int, D):
+    """D: the common embedding dim, or a per-table sequence of dims."""
     keep = []
-    for t in tables:
+    dims = [int(D)] * len(tables) if np.isscalar(D) else [int(d) for d in D]
+    for t, D in zip(tables, dims):
         a = np.ascontiguousarray(t)
         if dtype == F16 and a.dtype == np.uint16:
             pass  # raw binary16 bits are accepted as well
@@ -114,6 +118,37 @@ def lookup(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray
     _check(_load().oracle_lookup(T, B, D, dtype, ctypes.cast(ptrs, ctypes.c_void_p), rows.ctypes.data,
                                  indices.ctypes.data, offsets.ctypes.data, pooling.ctypes.data,
                                  ref.ctypes.data))
+    del keep
+    return ref
+
+
+SAMPLE_MAJOR, TABLE_MAJOR = 0, 1
+
+
+def lookup_general(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray, offsets: np.ndarray,
+                   pooling: np.ndarray, weights: np.ndarray = None, bag_order: int = SAMPLE_MAJOR) -> np.ndarray:
+    """Interface variants (mixed per-table dims, int64 indices/offsets, per-entry fp32 weights, table-major bags).
+    Returns the unrounded float64 reference [B, sum(dims)]."""
+    T = len(tables)
+    dims = np.asarray([np.asarray(t).shape[1] for t in tables], dtype=np.int32)
+    indices = np.ascontiguousarray(indices, dtype=np.int64)
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    pooling = np.ascontiguousarray(pooling, dtype=np.uint8)
+    if offsets.shape[0] != B * T + 1 or pooling.shape[0] != T:
+        raise ValueError("offsets must be [B*T+1], pooling [T]")
+    if int(offsets[-1]) > indices.shape[0]:
+        raise ValueError("offsets[-1] exceeds len(indices)")
+    w = None
+    if weights is not None:
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        if w.shape[0] != indices.shape[0]:
+            raise ValueError("weights must have one entry per index")
+    ptrs, rows, keep = _table_ptrs(tables, dtype, dims)
+    ref = np.empty((B, int(dims.sum())), dtype=np.float64)
+    _check(_load().oracle_lookup_general(T, B, dims.ctypes.data, dtype, ctypes.cast(ptrs, ctypes.c_void_p),
+                                         rows.ctypes.data, indices.ctypes.data, offsets.ctypes.data,
+                                         None if w is None else w.ctypes.data, pooling.ctypes.data, int(bag_order),
+                                         ref.ctypes.data))
     del keep
     return ref
 

@@ -25,6 +25,9 @@
  * formulation ("encoded with one-hot encoding") via numpy matmul, torch-CPU embedding_bag,
  * table independence, sample permutation, numpy cumsum, closed form for equal lengths,
  * cover/monotone/bounded-cost invariants, O(G*S) brute force, and exhaustive 16-bit decode checks.
+ * oracle_lookup_general (interface variants) is pinned in tests/test_oracle_variants.py: torch-CPU embedding_bag
+ * with per_sample_weights (float64), linearity / power-of-two / zero weights, index-encoding tables with mixed
+ * dims, hstack of single-table calls, and the bag-grid transpose for table-major input.
  */
 #include <stdint.h>
 #include <stddef.h>
@@ -131,6 +134,59 @@ int oracle_lookup(int32_t T, int32_t B, int32_t D, int dtype,
                 for (int32_t c = 0; c < D; ++c) acc[c] /= L;
             }
         }
+    }
+    return ORACLE_OK;
+}
+
+/*
+ * Interface variants of the same lookup (DESIGN.md §11 gives the readings).  The paper
+ * only hints at them: multi-hot "by marking offset information" and ids arriving as 64-bit
+ * integers from the framework.  Same definition as oracle_lookup with four generalisations:
+ *   dims[t]      per-table embedding dim; table t occupies columns [col[t], col[t] + dims[t]) of a row of width
+ *                W = sum dims, col[t] = sum_{u<t} dims[u]            ("concatenated", one d at :137)
+ *   bag_order    0: sample-major, bag (b,t) is g = b*T + t  (Alg. 1 line 7)
+ *                1: table-major,  bag (b,t) is g = t*B + b  (all bags of field 0, then field 1, ...)
+ *   indices / offsets are int64
+ *   weights      NULL, or one fp32 weight per index entry: acc += w[j] * E_t[indices[j]]  (sum pooling only;
+ *                a mean-pooled table together with weights is rejected)
+ * ref is [B, W] row-major float64, unrounded.  Loop order t -> b -> j -> c as in oracle_lookup.
+ */
+int oracle_lookup_general(int32_t T, int32_t B, const int32_t *dims, int dtype,
+                          const void *const *tables, const int64_t *table_rows,
+                          const int64_t *indices, const int64_t *offsets, const float *weights,
+                          const uint8_t *pooling, int bag_order, double *ref)
+{
+    if (T <= 0 || B < 0 || !dims || !tables || !table_rows || !offsets || !pooling || !ref) return ORACLE_BAD_ARG;
+    if (dtype != ORACLE_F32 && dtype != ORACLE_F16 && dtype != ORACLE_BF16) return ORACLE_BAD_ARG;
+    if (bag_order != 0 && bag_order != 1) return ORACLE_BAD_ARG;
+    int64_t W = 0;
+    for (int32_t t = 0; t < T; ++t) {
+        if (dims[t] <= 0) return ORACLE_BAD_ARG;
+        if (weights && pooling[t] == ORACLE_MEAN) return ORACLE_BAD_ARG;
+        W += dims[t];
+    }
+    int64_t col = 0;                                             /* col[t] */
+    for (int32_t t = 0; t < T; ++t) {
+        int32_t D = dims[t];
+        for (int32_t b = 0; b < B; ++b) {
+            int64_t g = bag_order == 0 ? (int64_t)b * T + t : (int64_t)t * B + b;
+            int64_t lo = offsets[g], hi = offsets[g + 1];
+            double *acc = ref + (int64_t)b * W + col;
+            if (hi < lo) return ORACLE_BAD_ARG;
+            for (int32_t c = 0; c < D; ++c) acc[c] = 0.0;
+            for (int64_t j = lo; j < hi; ++j) {
+                int64_t r = indices[j];
+                double w = weights ? (double)weights[j] : 1.0;
+                if (r < 0 || r >= table_rows[t]) return ORACLE_INDEX_RANGE;
+                for (int32_t c = 0; c < D; ++c)
+                    acc[c] += w * element_as_double(tables[t], dtype, r * D + c);
+            }
+            if (pooling[t] == ORACLE_MEAN && hi > lo) {
+                double L = (double)(hi - lo);
+                for (int32_t c = 0; c < D; ++c) acc[c] /= L;
+            }
+        }
+        col += D;
     }
     return ORACLE_OK;
 }
