@@ -56,7 +56,7 @@ typedef struct dpi_plan_s dpi_plan_t; /* opaque, library-owned */
 typedef enum {
     DPI_OK = 0,
     DPI_ERR_INVALID_ARG = 1,  /* NULL, non-positive sizes, misaligned pointers, capacity exceeded */
-    DPI_ERR_UNSUPPORTED = 2,  /* mixed dims, row size not a multiple of 16 B or > 512 B, T > DPI_MAX_TABLES */
+    DPI_ERR_UNSUPPORTED = 2,  /* row size not a multiple of 16 B or > 512 B, T > DPI_MAX_TABLES, weights + mean */
     DPI_ERR_ALLOC = 3,        /* host or device allocation failed */
     DPI_ERR_CUDA = 4,         /* CUDA runtime error (text in dpi_last_error) */
     DPI_ERR_INDEX_RANGE = 5   /* dpi_check_indices found indices outside [0, table_rows[t]) */
@@ -64,6 +64,13 @@ typedef enum {
 
 typedef enum { DPI_F32 = 0, DPI_F16 = 1, DPI_BF16 = 2 } dpi_dtype_t;
 typedef enum { DPI_POOL_SUM = 0, DPI_POOL_MEAN = 1 } dpi_pool_t;
+/* Order of the bags in lengths / offsets / indices (interface variant, see dpi_plan_set_layout). */
+typedef enum {
+    DPI_BAGS_SAMPLE_MAJOR = 0, /* g = b*T + t: Alg. 1 line 7 "IDs[row*k + table_id]" -- the default */
+    DPI_BAGS_TABLE_MAJOR = 1   /* g = t*B + b: all bags of field 0, then field 1, ... (how jagged feature tensors
+                                  usually arrive from a serving stack) */
+} dpi_bag_order_t;
+typedef enum { DPI_IDX_I32 = 0, DPI_IDX_I64 = 1 } dpi_index_type_t;
 
 /* Tuning knobs for dpi_plan_set_option (all kernel-internal; none changes a result). */
 typedef enum {
@@ -83,8 +90,10 @@ typedef enum {
  * is reusable for any batch of the same (T, B, dims, dtype) whose N <= max_indices.
  *   T            number of tables, 1..DPI_MAX_TABLES
  *   table_rows   host int64[T], heights n_t >= 1; copied
- *   dims         host int32[T], embedding dim of each table; v1 requires all equal (R10) and
- *                D*sizeof(dtype) a multiple of 16 B and <= 512 B, else DPI_ERR_UNSUPPORTED
+ *   dims         host int32[T], embedding dim of each table; every dims[t]*sizeof(dtype) must be a multiple of
+ *                16 B and <= 512 B, else DPI_ERR_UNSUPPORTED. The paper has one d; tables of
+ *                different widths are an interface variant (R10, §11): table t then occupies columns
+ *                [col[t], col[t] + dims[t]) with col[t] = sum of dims[u], u < t ("concatenated")
  *   dtype        storage type of the tables and, by default, of the output
  *   B            samples per batch >= 1;  G = B*T must be < 2^31
  *   max_indices  upper bound on N for any batch built with this plan, 0 <= max_indices < 2^31
@@ -97,6 +106,22 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
  * correctly rounded bf16 output carries up to 2^-8 = 3.9e-3 relative error by itself; fp32 output keeps the
  * fp32 accumulator (R6). Anything else -> DPI_ERR_UNSUPPORTED. */
 dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* plan, dpi_dtype_t out_dtype);
+
+/*
+ * dpi_plan_set_layout -- interface variants of the sparse input (the paper only says multi-hot
+ * is supported "by marking offset information", and that ids reach the model as 64-bit integers,
+ * PAPER.md:336). Takes effect for the next dpi_plan_build / dpi_lookup*.
+ *   order       DPI_BAGS_SAMPLE_MAJOR (default) or DPI_BAGS_TABLE_MAJOR: the position g of bag (b, t) in `lengths`,
+ *               `offsets` and the bag-contiguous `indices`. The plan itself (offsets, segments) is a function of the
+ *               length sequence only, so its definition does not change; the output stays [B, sum dims] with table
+ *               t in its own column block.
+ *   index_type  DPI_IDX_I32 (default) or DPI_IDX_I64: element type of `indices` (values must still lie in
+ *               [0, table_rows[t]), table_rows[t] < 2^31). Offsets stay int32 inside the plan (N < 2^31).
+ */
+dpi_status_t dpi_plan_set_layout(dpi_plan_t* plan, dpi_bag_order_t order, dpi_index_type_t index_type);
+
+/* Elements per output row = sum of dims (T*D when every table has the same D). */
+dpi_status_t dpi_plan_out_width(const dpi_plan_t* plan, int64_t* width);
 
 /* Cost quantum K >= 1 of the balanced segments (0 = library default for this row size). Takes effect at the
  * next dpi_plan_build. DPI_ERR_INVALID_ARG if K < 0. */
@@ -127,7 +152,8 @@ dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims,
 dpi_status_t dpi_plan_device_views(const dpi_plan_t* plan, const int32_t** offsets_dev,
                                    const int32_t** seg_dev, const int32_t** meta_dev);
 
-/* Static facts about a plan (host only, no synchronisation). Any out-pointer may be NULL. */
+/* Static facts about a plan (host only, no synchronisation). Any out-pointer may be NULL. D is the widest table's
+ * dim (the common D when all are equal). */
 dpi_status_t dpi_plan_info(const dpi_plan_t* plan, int32_t* T, int32_t* B, int32_t* D, int32_t* dtype,
                            int64_t* G, int32_t* K, int64_t* seg_capacity);
 
@@ -157,6 +183,36 @@ dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indice
                         void* out_dev, void* stream);
 
 /*
+ * dpi_lookup_ex -- step a3 with the interface variants: the same fused gather-and-pool,
+ * asynchronous on `stream`, ONE launch. Anything the plan's layout says (mixed dims, table-major bags, int64 ids)
+ * plus, per call:
+ *   weights_dev  NULL, or device fp32[N]: one weight per index entry, acc += w[j] * row (fp32 fused multiply-add;
+ *                with every w = 1 the result is bit-identical to the unweighted sum). Sum pooling only: a
+ *                mean-pooled table together with weights -> DPI_ERR_UNSUPPORTED.
+ *   out_ld       elements between consecutive output rows; 0 = dense (= dpi_plan_out_width). A larger value writes
+ *                this call's [B, width] block into a wider row-major matrix (e.g. next to dense features, or as
+ *                one rank's column block of a table-sharded model). The pitch in bytes must keep rows 16-byte
+ *                aligned (32-byte for fp32 output of 16-bit tables), else DPI_ERR_INVALID_ARG.
+ *   indices_dev  int32 or int64 per the plan's index type; the other fields as in dpi_lookup.
+ *   flags        DPI_LOOKUP_FORCE_GENERAL runs the general kernel even when the call needs none of the variants
+ *                (used by the parity tests to compare the two instantiations).
+ * Set struct_size = sizeof(dpi_lookup_args_t); a mismatch -> DPI_ERR_INVALID_ARG. Unused fields must be zero.
+ */
+#define DPI_LOOKUP_FORCE_GENERAL 1u
+typedef struct dpi_lookup_args_s {
+    uint32_t struct_size;
+    uint32_t flags;
+    const void* const* table_ptrs_dev;
+    const void* indices_dev;
+    const int32_t* offsets_dev;
+    const float* weights_dev;
+    const uint8_t* pooling; /* host[T] or NULL */
+    void* out_dev;
+    int64_t out_ld;
+} dpi_lookup_args_t;
+dpi_status_t dpi_lookup_ex(const dpi_lookup_args_t* args, const dpi_plan_t* plan, void* stream);
+
+/*
  * dpi_lookup_input_first -- ABLATION, not the product path: the same lookup with the paper's strawman
  * "input-first" workload allocation (different samples on different threads, so table reads
  * and output writes of a warp are random), kept to measure the paper's Fig. 11 claim (output-first up to 10.3x
@@ -172,16 +228,17 @@ dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int
  * (the end-to-end number of bench.py): copies lengths and indices host->device into plan-owned staging,
  * builds the plan, runs the lookup and copies the [B, T*D] block back, then synchronises `stream`.
  * Tables stay resident on the device (they are the model, not a per-batch input).
- *   lengths_host int32[G]; indices_host int32[n_indices] (n_indices <= max_indices); out_host [B,T*D].
+ *   lengths_host int32[G]; indices_host int32 / int64 [n_indices] per the plan's index type
+ *   (n_indices <= max_indices); out_host [B, sum dims].
  *   Pinned (page-locked) host buffers make the copies asynchronous and faster but are not required.
  */
 dpi_status_t dpi_forward_host(dpi_plan_t* plan, const void* const* table_ptrs_dev,
-                              const int32_t* lengths_host, const int32_t* indices_host, int64_t n_indices,
+                              const int32_t* lengths_host, const void* indices_host, int64_t n_indices,
                               const uint8_t* pooling, void* out_host, void* stream);
 
 /* Off the hot path: counts indices outside [0, table_rows[t]) for the last built batch; synchronises.
  * Returns DPI_ERR_INDEX_RANGE (and *n_bad > 0) if any. */
-dpi_status_t dpi_check_indices(const dpi_plan_t* plan, const int32_t* indices_dev, int64_t* n_bad,
+dpi_status_t dpi_check_indices(const dpi_plan_t* plan, const void* indices_dev, int64_t* n_bad,
                                void* stream);
 
 dpi_status_t dpi_plan_destroy(dpi_plan_t* plan);

@@ -20,12 +20,23 @@ STATUS_NAMES = {0: "DPI_OK", 1: "DPI_ERR_INVALID_ARG", 2: "DPI_ERR_UNSUPPORTED",
 DPI_F32, DPI_F16, DPI_BF16 = 0, 1, 2
 DPI_POOL_SUM, DPI_POOL_MEAN = 0, 1
 OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL = range(6)
+BAGS_SAMPLE_MAJOR, BAGS_TABLE_MAJOR = 0, 1
+IDX_I32, IDX_I64 = 0, 1
+LOOKUP_FORCE_GENERAL = 1
 
 # every symbol include/dpi.h declares (tests check the .so exports each one)
-EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
+EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "dpi_plan_out_width", "dpi_lookup_ex",
+           "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
            "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export",
            "dpi_lookup", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
            "dpi_version", "dpi_status_string", "dpi_last_error"]
+
+
+class LookupArgs(ctypes.Structure):
+    """dpi_lookup_args_t of include/dpi.h."""
+    _fields_ = [("struct_size", ctypes.c_uint32), ("flags", ctypes.c_uint32), ("table_ptrs_dev", ctypes.c_void_p),
+                ("indices_dev", ctypes.c_void_p), ("offsets_dev", ctypes.c_void_p), ("weights_dev", ctypes.c_void_p),
+                ("pooling", ctypes.c_void_p), ("out_dev", ctypes.c_void_p), ("out_ld", ctypes.c_int64)]
 
 
 class DpiLibraryMissing(RuntimeError):
@@ -56,6 +67,9 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     sig = {
         "dpi_plan_create": (st, [i32, vp, vp, ctypes.c_int, i32, i64, vp]),
         "dpi_plan_set_out_dtype": (st, [vp, ctypes.c_int]),
+        "dpi_plan_set_layout": (st, [vp, ctypes.c_int, ctypes.c_int]),
+        "dpi_plan_out_width": (st, [vp, vp]),
+        "dpi_lookup_ex": (st, [vp, vp, vp]),
         "dpi_plan_set_quantum": (st, [vp, i32]),
         "dpi_plan_set_option": (st, [vp, ctypes.c_int, i32]),
         "dpi_plan_get_option": (st, [vp, ctypes.c_int, vp]),
@@ -128,7 +142,9 @@ class Plan:
         _check(lib.dpi_plan_create(T, rows.ctypes.data, dims.ctypes.data, int(dtype), int(B), int(max_indices),
                                    ctypes.byref(handle)))
         self._h = handle
-        self.T, self.B, self.D, self.dtype = T, int(B), int(dims[0]), int(dtype)
+        self.T, self.B, self.D, self.dtype = T, int(B), int(dims.max()), int(dtype)
+        self.dims = dims.copy()
+        self.out_width = int(dims.sum())
         self.out_dtype = int(dtype)
         self.G = self.T * self.B
         self.max_indices = int(max_indices)
@@ -149,6 +165,15 @@ class Plan:
     def set_out_dtype(self, out_dtype: int):
         _check(self._lib.dpi_plan_set_out_dtype(self._h, int(out_dtype)))
         self.out_dtype = int(out_dtype)
+
+    # -- dpi_plan_set_layout / dpi_plan_out_width -----------------------------------------------------------
+    def set_layout(self, bag_order: int = BAGS_SAMPLE_MAJOR, index_type: int = IDX_I32):
+        _check(self._lib.dpi_plan_set_layout(self._h, int(bag_order), int(index_type)))
+
+    def plan_out_width(self) -> int:
+        w = ctypes.c_int64()
+        _check(self._lib.dpi_plan_out_width(self._h, ctypes.byref(w)))
+        return int(w.value)
 
     # -- dpi_plan_set_quantum / options ---------------------------------------------------------------------
     def set_quantum(self, K: int):
@@ -199,6 +224,14 @@ class Plan:
         pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
         _check(self._lib.dpi_lookup(_ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(offsets_dev), self._h,
                                     _ptr(pool), _ptr(out_dev), _stream_handle(stream)))
+
+    # -- dpi_lookup_ex ----------------------------------------------------------------------------------------
+    def lookup_ex(self, table_ptrs_dev, indices_dev, out_dev, pooling=None, offsets_dev=None, weights_dev=None,
+                  out_ld: int = 0, flags: int = 0, stream=None):
+        pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
+        a = LookupArgs(ctypes.sizeof(LookupArgs), int(flags), _ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(offsets_dev),
+                       _ptr(weights_dev), _ptr(pool), _ptr(out_dev), int(out_ld))
+        _check(self._lib.dpi_lookup_ex(ctypes.byref(a), self._h, _stream_handle(stream)))
 
     # -- dpi_lookup_input_first (ablation) ---------------------------------------------------
     def lookup_input_first(self, table_ptrs_dev, indices_dev, out_dev, pooling=None, offsets_dev=None, stream=None):

@@ -31,7 +31,8 @@ __global__ void __launch_bounds__(128) input_first_kernel(const LookupArgs a, co
                 Tr::add(acc, ld_row16(tab + static_cast<size_t>(r) * row_bytes + v * 16, true));
             }
             if (mean) scale_mean(acc, hi - lo);
-            store_pooled<Tr, OUT32>(out, g, a.nvec, static_cast<int>(v), acc);
+            constexpr size_t kOutVec = (OUT32 && kAcc == 8) ? 32 : 16;
+            store_pooled<Tr, OUT32>(out + (g * a.nvec + v) * kOutVec, acc);
         }
     }
 }

@@ -48,7 +48,12 @@ using namespace dpi;
 
 struct dpi_plan_s {
     // shape
-    int32_t T = 0, B = 0, D = 0;
+    int32_t T = 0, B = 0, D = 0;   // D = the widest table's dim
+    int64_t out_width = 0;         // sum of dims = elements per output row
+    bool mixed_dims = false;
+    std::vector<int32_t> dims;
+    dpi_bag_order_t bag_order = DPI_BAGS_SAMPLE_MAJOR;
+    dpi_index_type_t index_type = DPI_IDX_I32;
     dpi_dtype_t dtype = DPI_F32;
     dpi_dtype_t out_dtype = DPI_F32;
     uint32_t G = 0;
@@ -71,10 +76,13 @@ struct dpi_plan_s {
     unsigned long long* tile_cost = nullptr;
     unsigned int* state = nullptr;   // planner device state {ticket, done, epoch, -}
     int64_t* table_rows_dev = nullptr;
+    uint32_t* tab_nvec_dev = nullptr;   // [T] 16-byte vectors per row of each table
+    uint32_t* tab_col_dev = nullptr;    // [T] first output vector of each table's column block
     unsigned long long* n_bad_dev = nullptr;
     // staging for dpi_forward_host
     int32_t* stage_len = nullptr;
-    int32_t* stage_idx = nullptr;
+    void* stage_idx = nullptr;
+    size_t stage_idx_bytes = 0;
     void* stage_out = nullptr;
     bool built = false;
 };
@@ -113,75 +121,113 @@ void free_plan(dpi_plan_t* p) {
     if (!p) return;
     cudaFree(p->offsets); cudaFree(p->seg); cudaFree(p->meta); cudaFree(p->tile_len);
     cudaFree(p->tile_cost); cudaFree(p->state); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
+    cudaFree(p->tab_nvec_dev); cudaFree(p->tab_col_dev);
     cudaFree(p->stage_len); cudaFree(p->stage_idx); cudaFree(p->stage_out);
     (void)cudaGetLastError();
     delete p;
 }
 
-struct LaunchChoice {
-    LookupLaunch l;
-};
-
-int occupancy(const dpi_plan_t* p, int lanes, int unroll, int threads) {
+int occupancy(const dpi_plan_t* p, const LookupArgs& a, const LookupLaunch& l) {
     switch (p->dtype) {
-        case DPI_F32: return lookup_occupancy_f32(lanes, unroll, threads, static_cast<uint32_t>(p->T), false);
-        case DPI_F16: return lookup_occupancy_f16(lanes, unroll, threads, static_cast<uint32_t>(p->T), p->out_dtype == DPI_F32);
-        default: return lookup_occupancy_bf16(lanes, unroll, threads, static_cast<uint32_t>(p->T), p->out_dtype == DPI_F32);
+        case DPI_F32: return lookup_occupancy_f32(a, l);
+        case DPI_F16: return lookup_occupancy_f16(a, l);
+        default: return lookup_occupancy_bf16(a, l);
     }
 }
 
-LaunchChoice choose_launch(const dpi_plan_t* p) {
-    LaunchChoice c{};
-    c.l.lanes = p->lanes;
-    c.l.unroll = p->opt[DPI_OPT_UNROLL] ? p->opt[DPI_OPT_UNROLL] : 2;  // x2 by double buffering (sweeps_r01.md)
-    c.l.block_threads = p->opt[DPI_OPT_BLOCK_THREADS] ? p->opt[DPI_OPT_BLOCK_THREADS] : 256;
+LookupLaunch choose_launch(const dpi_plan_t* p, const LookupArgs& a, bool general) {
+    LookupLaunch l{};
+    l.lanes = p->lanes;
+    l.general = general;
+    l.unroll = (p->opt[DPI_OPT_UNROLL] && !general) ? p->opt[DPI_OPT_UNROLL] : 2;  // x2 by double buffering (sweeps_r01.md)
+    l.block_threads = p->opt[DPI_OPT_BLOCK_THREADS] ? p->opt[DPI_OPT_BLOCK_THREADS] : 256;
+    l.out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
     int per_sm = p->opt[DPI_OPT_BLOCKS_PER_SM];
     if (per_sm <= 0) {
-        per_sm = occupancy(p, c.l.lanes, c.l.unroll, c.l.block_threads);
+        per_sm = occupancy(p, a, l);
         if (per_sm <= 0) per_sm = 1;
     }
-    c.l.grid = p->num_sms * per_sm;  // persistent: a whole number of waves, every CTA resident
-    const int64_t warps_per_cta = c.l.block_threads / 32;
+    l.grid = p->num_sms * per_sm;  // persistent: a whole number of waves, every CTA resident
+    const int64_t warps_per_cta = l.block_threads / 32;
     const int64_t need = (static_cast<int64_t>(p->seg_cap) + warps_per_cta - 1) / warps_per_cta;  // one warp per possible task
-    if (need < c.l.grid) c.l.grid = static_cast<int>(need > 0 ? need : 1);
-    c.l.pdl = p->opt[DPI_OPT_PDL] != 0;
-    c.l.out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
-    return c;
+    if (need < l.grid) l.grid = static_cast<int>(need > 0 ? need : 1);
+    l.pdl = p->opt[DPI_OPT_PDL] != 0;
+    return l;
 }
 
-dpi_status_t do_lookup(const dpi_plan_t* p, const void* const* tables, const int32_t* indices, const int32_t* offsets,
-                       const uint8_t* pooling, void* out, cudaStream_t stream, bool input_first = false) {
+struct LookupCall {
+    const void* const* tables = nullptr;
+    const void* indices = nullptr;
+    const int32_t* offsets = nullptr;
+    const float* weights = nullptr;
+    const uint8_t* pooling = nullptr;
+    void* out = nullptr;
+    int64_t out_ld = 0;     // elements; 0 = dense
+    bool force_general = false;
+};
+
+size_t out_elt_bytes(const dpi_plan_t* p) { return p->out_dtype == DPI_F32 ? 4 : 2; }
+
+dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t stream, bool input_first = false) {
     LookupArgs a{};
-    a.tables = tables;
-    a.indices = indices;
-    a.offsets = offsets ? offsets : p->offsets;
+    a.tables = c.tables;
+    a.indices = static_cast<const int32_t*>(c.indices);
+    a.offsets = c.offsets ? c.offsets : p->offsets;
     a.seg = p->seg;
     a.meta = p->meta;
-    a.out = out;
+    a.out = c.out;
     a.G = p->G;
     a.T = static_cast<uint32_t>(p->T);
+    a.B = static_cast<uint32_t>(p->B);
     a.nvec = p->nvec;
     a.mode = p->opt[DPI_OPT_MODE];
+    a.weights = c.weights;
+    a.tab_nvec = p->tab_nvec_dev;
+    a.tab_col = p->tab_col_dev;
+    a.idx_shift = p->index_type == DPI_IDX_I64 ? 1u : 0u;
+    a.table_major = p->bag_order == DPI_BAGS_TABLE_MAJOR ? 1u : 0u;
+    const int64_t ld = c.out_ld ? c.out_ld : p->out_width;
+    if (ld < p->out_width) return fail(DPI_ERR_INVALID_ARG, "out_ld=%lld is smaller than the row width %lld", (long long)ld, (long long)p->out_width);
+    a.out_pitch = static_cast<uint64_t>(ld) * out_elt_bytes(p);
+    const uintptr_t out_align = (p->dtype != DPI_F32 && p->out_dtype == DPI_F32) ? 31u : 15u;
+    if (a.out_pitch & out_align) return fail(DPI_ERR_INVALID_ARG, "output row pitch %llu B is not a multiple of %d B", (unsigned long long)a.out_pitch, (int)out_align + 1);
     std::memset(&a.pool, 0, sizeof a.pool);
-    if (pooling) {
+    if (c.pooling) {
         for (int t = 0; t < p->T; ++t) {
-            if (pooling[t] > 1) return fail(DPI_ERR_INVALID_ARG, "pooling[%d] = %d is not a dpi_pool_t", t, pooling[t]);
-            if (pooling[t] == DPI_POOL_MEAN) a.pool.w[t >> 5] |= 1u << (t & 31);
+            if (c.pooling[t] > 1) return fail(DPI_ERR_INVALID_ARG, "pooling[%d] = %d is not a dpi_pool_t", t, c.pooling[t]);
+            if (c.pooling[t] == DPI_POOL_MEAN) {
+                if (c.weights) return fail(DPI_ERR_UNSUPPORTED, "per-entry weights need sum pooling (table %d is mean-pooled)", t);
+                a.pool.w[t >> 5] |= 1u << (t & 31);
+            }
         }
     }
+    const bool general = c.force_general || p->mixed_dims || a.idx_shift || a.table_major || c.weights || ld != p->out_width;
     if (input_first) {
+        if (general) return fail(DPI_ERR_UNSUPPORTED, "the input-first ablation kernel only takes the dense int32 sample-major layout");
         cudaError_t e = launch_input_first(a, static_cast<uint32_t>(p->B), p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, stream);
         if (e != cudaSuccess) return cuda_fail(e, "input-first kernel launch");
         return DPI_OK;
     }
-    const LaunchChoice c = choose_launch(p);
+    const LookupLaunch l = choose_launch(p, a, general);
     cudaError_t e;
     switch (p->dtype) {
-        case DPI_F32: e = launch_lookup_f32(a, c.l, stream); break;
-        case DPI_F16: e = launch_lookup_f16(a, c.l, stream); break;
-        default: e = launch_lookup_bf16(a, c.l, stream); break;
+        case DPI_F32: e = launch_lookup_f32(a, l, stream); break;
+        case DPI_F16: e = launch_lookup_f16(a, l, stream); break;
+        default: e = launch_lookup_bf16(a, l, stream); break;
     }
     if (e != cudaSuccess) return cuda_fail(e, "lookup kernel launch");
+    return DPI_OK;
+}
+
+dpi_status_t check_lookup_pointers(const dpi_plan_t* p, const void* tables, const void* indices, const void* out) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built (call dpi_plan_build first)");
+    if (!tables || !out) return fail(DPI_ERR_INVALID_ARG, "table_ptrs_dev/out_dev is NULL");
+    if (!indices && p->max_indices > 0) return fail(DPI_ERR_INVALID_ARG, "indices_dev is NULL");
+    const uintptr_t out_align = (p->dtype != DPI_F32 && p->out_dtype == DPI_F32) ? 31u : 15u;
+    if (reinterpret_cast<uintptr_t>(out) & out_align) return fail(DPI_ERR_INVALID_ARG, "out_dev is not %d-byte aligned", (int)out_align + 1);
+    const uintptr_t idx_align = p->index_type == DPI_IDX_I64 ? 7u : 3u;
+    if (reinterpret_cast<uintptr_t>(indices) & idx_align) return fail(DPI_ERR_INVALID_ARG, "indices_dev is not %d-byte aligned", (int)idx_align + 1);
     return DPI_OK;
 }
 
@@ -200,17 +246,22 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     if (max_indices < 0 || max_indices >= (1ll << 31)) return fail(DPI_ERR_INVALID_ARG, "max_indices=%lld outside [0, 2^31)", (long long)max_indices);
     const int64_t G64 = static_cast<int64_t>(B) * T;
     if (G64 >= (1ll << 31) || G64 + max_indices >= (1ll << 32) - 16) return fail(DPI_ERR_INVALID_ARG, "B*T=%lld too large", (long long)G64);
-    const int32_t D = dims[0];
+    const int elt = dtype == DPI_F32 ? 4 : 2;
+    int32_t D = dims[0];
+    bool mixed = false;
+    int64_t out_width = 0;
     for (int t = 0; t < T; ++t) {
         if (dims[t] < 1) return fail(DPI_ERR_INVALID_ARG, "dims[%d]=%d", t, dims[t]);
-        if (dims[t] != D) return fail(DPI_ERR_UNSUPPORTED, "mixed dims (dims[%d]=%d != dims[0]=%d): v1 needs one D (DESIGN.md R10)", t, dims[t], D);
+        const int64_t rb = static_cast<int64_t>(dims[t]) * elt;
+        if (rb % 16 != 0) return fail(DPI_ERR_UNSUPPORTED, "row size %lld B of table %d is not a multiple of 16 B", (long long)rb, t);
+        if (rb > 512) return fail(DPI_ERR_UNSUPPORTED, "row size %lld B of table %d exceeds 512 B (one warp-wide 128-bit load)", (long long)rb, t);
+        if (dims[t] != dims[0]) mixed = true;
+        if (dims[t] > D) D = dims[t];
+        out_width += dims[t];
         if (table_rows[t] < 1) return fail(DPI_ERR_INVALID_ARG, "table_rows[%d]=%lld must be >= 1", t, (long long)table_rows[t]);
         if (table_rows[t] > 0x7fffffffll) return fail(DPI_ERR_UNSUPPORTED, "table_rows[%d] exceeds int32 index range", t);
     }
-    const int elt = dtype == DPI_F32 ? 4 : 2;
-    const int64_t row_bytes = static_cast<int64_t>(D) * elt;
-    if (row_bytes % 16 != 0) return fail(DPI_ERR_UNSUPPORTED, "row size %lld B is not a multiple of 16 B", (long long)row_bytes);
-    if (row_bytes > 512) return fail(DPI_ERR_UNSUPPORTED, "row size %lld B exceeds 512 B (one warp-wide 128-bit load)", (long long)row_bytes);
+    const int64_t row_bytes = static_cast<int64_t>(D) * elt;   // the widest table
 
     int dev = 0, n_dev = 0;
     cudaError_t e = cudaGetDeviceCount(&n_dev);
@@ -231,6 +282,9 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     p->nvec = static_cast<uint32_t>(row_bytes / 16);
     p->lanes = pow2ceil(static_cast<int>(p->nvec));
     p->table_rows.assign(table_rows, table_rows + T);
+    p->dims.assign(dims, dims + T);
+    p->mixed_dims = mixed;
+    p->out_width = out_width;
     p->device = dev;
     p->num_sms = prop.multiProcessorCount;
     p->num_tiles = (p->G + kScanTile - 1) / kScanTile;
@@ -260,6 +314,19 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     DPI_TRY(cudaMalloc(&p->table_rows_dev, T * sizeof(int64_t)));
     DPI_TRY(cudaMemcpy(p->table_rows_dev, table_rows, T * sizeof(int64_t), cudaMemcpyHostToDevice));
     DPI_TRY(cudaMalloc(&p->n_bad_dev, sizeof(unsigned long long)));
+    {
+        std::vector<uint32_t> nv(T), col(T);
+        uint32_t c = 0;
+        for (int t = 0; t < T; ++t) {
+            nv[t] = static_cast<uint32_t>(static_cast<int64_t>(dims[t]) * elt / 16);
+            col[t] = c;
+            c += nv[t];
+        }
+        DPI_TRY(cudaMalloc(&p->tab_nvec_dev, T * sizeof(uint32_t)));
+        DPI_TRY(cudaMalloc(&p->tab_col_dev, T * sizeof(uint32_t)));
+        DPI_TRY(cudaMemcpy(p->tab_nvec_dev, nv.data(), T * sizeof(uint32_t), cudaMemcpyHostToDevice));
+        DPI_TRY(cudaMemcpy(p->tab_col_dev, col.data(), T * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    }
 #undef DPI_TRY
     dpi_status_t st = ensure_seg_capacity(p, p->K);
     if (st != DPI_OK) { free_plan(p); return st; }
@@ -391,50 +458,83 @@ dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* p, dpi_dtype_t out_dtype) {
 
 dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,
                         const dpi_plan_t* p, const uint8_t* pooling, void* out_dev, void* stream) {
-    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
-    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built (call dpi_plan_build first)");
-    if (!table_ptrs_dev || !out_dev) return fail(DPI_ERR_INVALID_ARG, "table_ptrs_dev/out_dev is NULL");
-    if (!indices_dev && p->max_indices > 0) return fail(DPI_ERR_INVALID_ARG, "indices_dev is NULL");
-    const uintptr_t out_align = (p->dtype != DPI_F32 && p->out_dtype == DPI_F32) ? 31u : 15u;
-    if (reinterpret_cast<uintptr_t>(out_dev) & out_align) return fail(DPI_ERR_INVALID_ARG, "out_dev is not %d-byte aligned", (int)out_align + 1);
-    if (reinterpret_cast<uintptr_t>(indices_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "indices_dev is not 4-byte aligned");
-    return do_lookup(p, table_ptrs_dev, indices_dev, offsets_dev, pooling, out_dev, static_cast<cudaStream_t>(stream));
+    dpi_status_t st = check_lookup_pointers(p, table_ptrs_dev, indices_dev, out_dev);
+    if (st != DPI_OK) return st;
+    LookupCall c;
+    c.tables = table_ptrs_dev; c.indices = indices_dev; c.offsets = offsets_dev; c.pooling = pooling; c.out = out_dev;
+    return do_lookup(p, c, static_cast<cudaStream_t>(stream));
+}
+
+dpi_status_t dpi_lookup_ex(const dpi_lookup_args_t* args, const dpi_plan_t* p, void* stream) {
+    if (!args) return fail(DPI_ERR_INVALID_ARG, "args is NULL");
+    if (args->struct_size != sizeof(dpi_lookup_args_t)) return fail(DPI_ERR_INVALID_ARG, "args->struct_size=%u, expected %zu", args->struct_size, sizeof(dpi_lookup_args_t));
+    dpi_status_t st = check_lookup_pointers(p, args->table_ptrs_dev, args->indices_dev, args->out_dev);
+    if (st != DPI_OK) return st;
+    if (reinterpret_cast<uintptr_t>(args->weights_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "weights_dev is not 4-byte aligned");
+    if (args->out_ld < 0) return fail(DPI_ERR_INVALID_ARG, "out_ld=%lld", (long long)args->out_ld);
+    LookupCall c;
+    c.tables = args->table_ptrs_dev; c.indices = args->indices_dev; c.offsets = args->offsets_dev;
+    c.weights = args->weights_dev; c.pooling = args->pooling; c.out = args->out_dev; c.out_ld = args->out_ld;
+    c.force_general = (args->flags & DPI_LOOKUP_FORCE_GENERAL) != 0;
+    return do_lookup(p, c, static_cast<cudaStream_t>(stream));
 }
 
 dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,
                                     const dpi_plan_t* p, const uint8_t* pooling, void* out_dev, void* stream) {
+    dpi_status_t st = check_lookup_pointers(p, table_ptrs_dev, indices_dev, out_dev);
+    if (st != DPI_OK) return st;
+    LookupCall c;
+    c.tables = table_ptrs_dev; c.indices = indices_dev; c.offsets = offsets_dev; c.pooling = pooling; c.out = out_dev;
+    return do_lookup(p, c, static_cast<cudaStream_t>(stream), true);
+}
+
+dpi_status_t dpi_plan_set_layout(dpi_plan_t* p, dpi_bag_order_t order, dpi_index_type_t index_type) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
-    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built (call dpi_plan_build first)");
-    if (!table_ptrs_dev || !out_dev) return fail(DPI_ERR_INVALID_ARG, "table_ptrs_dev/out_dev is NULL");
-    if (!indices_dev && p->max_indices > 0) return fail(DPI_ERR_INVALID_ARG, "indices_dev is NULL");
-    const uintptr_t out_align = (p->dtype != DPI_F32 && p->out_dtype == DPI_F32) ? 31u : 15u;
-    if (reinterpret_cast<uintptr_t>(out_dev) & out_align) return fail(DPI_ERR_INVALID_ARG, "out_dev is not %d-byte aligned", (int)out_align + 1);
-    return do_lookup(p, table_ptrs_dev, indices_dev, offsets_dev, pooling, out_dev, static_cast<cudaStream_t>(stream), true);
+    if (order != DPI_BAGS_SAMPLE_MAJOR && order != DPI_BAGS_TABLE_MAJOR) return fail(DPI_ERR_INVALID_ARG, "unknown bag order %d", (int)order);
+    if (index_type != DPI_IDX_I32 && index_type != DPI_IDX_I64) return fail(DPI_ERR_INVALID_ARG, "unknown index type %d", (int)index_type);
+    p->bag_order = order;
+    p->index_type = index_type;
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_out_width(const dpi_plan_t* p, int64_t* width) {
+    if (!p || !width) return fail(DPI_ERR_INVALID_ARG, "NULL argument");
+    *width = p->out_width;
+    return DPI_OK;
 }
 
 dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, const int32_t* lengths_host,
-                              const int32_t* indices_host, int64_t n_indices, const uint8_t* pooling, void* out_host,
+                              const void* indices_host, int64_t n_indices, const uint8_t* pooling, void* out_host,
                               void* stream) {
     if (!p || !table_ptrs_dev || !lengths_host || !out_host) return fail(DPI_ERR_INVALID_ARG, "NULL argument");
     if (n_indices < 0 || n_indices > p->max_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld outside [0, max_indices=%lld]", (long long)n_indices, (long long)p->max_indices);
     if (n_indices > 0 && !indices_host) return fail(DPI_ERR_INVALID_ARG, "indices_host is NULL");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    const size_t out_bytes = static_cast<size_t>(p->G) * p->D * (p->out_dtype == DPI_F32 ? 4 : 2);
+    const size_t out_bytes = static_cast<size_t>(p->B) * p->out_width * out_elt_bytes(p);
+    const size_t idx_elt = p->index_type == DPI_IDX_I64 ? 8 : 4;
+    const size_t idx_bytes = (static_cast<size_t>(p->max_indices) + 4) * idx_elt;
     if (!p->stage_len) DPI_CUDA(cudaMalloc(&p->stage_len, static_cast<size_t>(p->G) * sizeof(int32_t)));
-    if (!p->stage_idx) DPI_CUDA(cudaMalloc(&p->stage_idx, (static_cast<size_t>(p->max_indices) + 4) * sizeof(int32_t)));
-    if (!p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, static_cast<size_t>(p->G) * p->D * 4));
+    if (p->stage_idx_bytes < idx_bytes) {
+        if (p->stage_idx) DPI_CUDA(cudaFree(p->stage_idx));
+        p->stage_idx = nullptr; p->stage_idx_bytes = 0;
+        DPI_CUDA(cudaMalloc(&p->stage_idx, idx_bytes));
+        p->stage_idx_bytes = idx_bytes;
+    }
+    if (!p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, static_cast<size_t>(p->B) * p->out_width * 4));
     DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
-    if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+    if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * idx_elt, cudaMemcpyHostToDevice, s));
     dpi_status_t st = dpi_plan_build(p, p->stage_len, s);
     if (st != DPI_OK) return st;
-    st = do_lookup(p, table_ptrs_dev, p->stage_idx, nullptr, pooling, p->stage_out, s);
+    LookupCall c;
+    c.tables = table_ptrs_dev; c.indices = p->stage_idx; c.pooling = pooling; c.out = p->stage_out;
+    st = do_lookup(p, c, s);
     if (st != DPI_OK) return st;
     DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
     DPI_CUDA(cudaStreamSynchronize(s));
     return DPI_OK;
 }
 
-dpi_status_t dpi_check_indices(const dpi_plan_t* p, const int32_t* indices_dev, int64_t* n_bad, void* stream) {
+dpi_status_t dpi_check_indices(const dpi_plan_t* p, const void* indices_dev, int64_t* n_bad, void* stream) {
     if (!p || !n_bad) return fail(DPI_ERR_INVALID_ARG, "NULL argument");
     if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -446,6 +546,9 @@ dpi_status_t dpi_check_indices(const dpi_plan_t* p, const int32_t* indices_dev, 
     a.n_bad = p->n_bad_dev;
     a.G = p->G;
     a.T = static_cast<uint32_t>(p->T);
+    a.B = static_cast<uint32_t>(p->B);
+    a.idx64 = p->index_type == DPI_IDX_I64;
+    a.table_major = p->bag_order == DPI_BAGS_TABLE_MAJOR;
     cudaError_t e = launch_check_indices(a, s);
     if (e != cudaSuccess) return cuda_fail(e, "check_indices launch");
     unsigned long long bad = 0;

@@ -49,12 +49,15 @@ struct PlanArgs {
 cudaError_t launch_plan(const PlanArgs& a, cudaStream_t stream);
 
 struct CheckArgs {
-    const int32_t* __restrict__ indices;
+    const void* __restrict__ indices;        // int32 or int64 (idx64)
     const int32_t* __restrict__ offsets;
     const int64_t* __restrict__ table_rows;  // device [T]
     unsigned long long* n_bad;
     uint32_t G;
     uint32_t T;
+    uint32_t B;
+    bool idx64;
+    bool table_major;
 };
 cudaError_t launch_check_indices(const CheckArgs& a, cudaStream_t stream);
 
@@ -68,8 +71,16 @@ struct LookupArgs {
     void* __restrict__ out;                  // [G * D] in the output dtype (out[b, t*D + c] == out[g*D + c])
     uint32_t G;
     uint32_t T;
-    uint32_t nvec;                           // 16-byte vectors per row = D*sizeof(elt)/16
+    uint32_t nvec;                           // 16-byte vectors per row = D*sizeof(elt)/16 (the widest table when dims differ)
     int32_t mode;                            // 0 auto, 1 sub-warp per bag, 2 warp per bag
+    // ---- general variant only (dpi_lookup_ex; lookup_kernel<..., GEN = true>) ----
+    const float* __restrict__ weights;       // NULL or fp32[N]: one weight per index entry
+    const uint32_t* __restrict__ tab_nvec;   // device [T] vectors per row of each table
+    const uint32_t* __restrict__ tab_col;    // device [T] first output vector of each table's column block
+    uint64_t out_pitch;                      // bytes between consecutive output rows
+    uint32_t B;
+    uint32_t idx_shift;                      // 0: int32 ids, 1: int64 ids (indices then points at the low words)
+    uint32_t table_major;                    // 0: g = b*T + t, 1: g = t*B + b
     PoolMask pool;
 };
 
@@ -80,6 +91,7 @@ struct LookupLaunch {
     int grid;           // persistent grid size
     bool pdl;           // programmatic dependent launch
     bool out32;         // 16-bit tables only: emit the output block in fp32
+    bool general;       // the GEN instantiation (interface variants)
 };
 
 // Each returns cudaErrorInvalidValue when (lanes, unroll, block_threads) has no instantiation.
@@ -87,9 +99,9 @@ cudaError_t launch_lookup_f32(const LookupArgs& a, const LookupLaunch& l, cudaSt
 cudaError_t launch_lookup_f16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
 cudaError_t launch_lookup_bf16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
 // Max resident CTAs per SM of the instantiation (0 if none).
-int lookup_occupancy_f32(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
-int lookup_occupancy_f16(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
-int lookup_occupancy_bf16(int lanes, int unroll, int block_threads, uint32_t T, bool out32);
+int lookup_occupancy_f32(const LookupArgs& a, const LookupLaunch& l);
+int lookup_occupancy_f16(const LookupArgs& a, const LookupLaunch& l);
+int lookup_occupancy_bf16(const LookupArgs& a, const LookupLaunch& l);
 
 // Ablation (ablation_input_first.cu): one thread per sample.
 cudaError_t launch_input_first(const LookupArgs& a, uint32_t B, int dtype, bool out32, cudaStream_t stream);

@@ -30,7 +30,6 @@ namespace dpi {
 
 constexpr int kStageIdx = 256;  // staged index entries per task buffer (tasks with more read global memory)
 constexpr int kStageOff = 72;   // staged offsets per task buffer (bags + 1)
-constexpr int kWarpStageInts = 2 * kStageIdx + 2 * kStageOff;
 constexpr int kLookupMaxThreads = 256;  // natural register allocation (64-80/thread); a 512 bound made ptxas spill
 
 // ---- memory helpers ----------------------------------------------------------------------------------
@@ -74,6 +73,10 @@ struct F32Traits {
         add2(acc[0], __uint_as_float(v.x), __uint_as_float(v.y));
         add2(acc[1], __uint_as_float(v.z), __uint_as_float(v.w));
     }
+    __device__ static __forceinline__ void fma(float2 (&acc)[2], const uint4& v, const float2 w) {
+        acc[0] = __ffma2_rn(make_float2(__uint_as_float(v.x), __uint_as_float(v.y)), w, acc[0]);
+        acc[1] = __ffma2_rn(make_float2(__uint_as_float(v.z), __uint_as_float(v.w)), w, acc[1]);
+    }
     __device__ static __forceinline__ uint4 pack(const float2 (&acc)[2]) {
         return make_uint4(__float_as_uint(acc[0].x), __float_as_uint(acc[0].y), __float_as_uint(acc[1].x),
                           __float_as_uint(acc[1].y));
@@ -89,6 +92,12 @@ struct F16Traits {
             const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w[i]));
             acc[i] = __fadd2_rn(acc[i], f);
         }
+    }
+    __device__ static __forceinline__ void fma(float2 (&acc)[4], const uint4& v, const float2 wt) {
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            acc[i] = __ffma2_rn(__half22float2(*reinterpret_cast<const __half2*>(&w[i])), wt, acc[i]);
     }
     __device__ static __forceinline__ uint4 pack(const float2 (&acc)[4]) {
         uint32_t w[4];
@@ -108,6 +117,12 @@ struct BF16Traits {
 #pragma unroll
         for (int i = 0; i < 4; ++i)  // bf16 -> fp32 is a 16-bit shift (low element) or a mask (high element)
             add2(acc[i], __uint_as_float(w[i] << 16), __uint_as_float(w[i] & 0xffff0000u));
+    }
+    __device__ static __forceinline__ void fma(float2 (&acc)[4], const uint4& v, const float2 wt) {
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            acc[i] = __ffma2_rn(make_float2(__uint_as_float(w[i] << 16), __uint_as_float(w[i] & 0xffff0000u)), wt, acc[i]);
     }
     __device__ static __forceinline__ uint4 pack(const float2 (&acc)[4]) {
         uint32_t w[4];
@@ -137,25 +152,47 @@ __device__ __forceinline__ void scale_mean(float2 (&acc)[N2], int len) {
     for (int i = 0; i < N2; ++i) acc[i] = __fmul2_rn(acc[i], inv2);
 }
 
-// Store one pooled vector of bag g: table dtype (16 B per lane) or fp32 (OUT32: 32 B per lane for 16-bit tables).
+// Store one pooled vector (16 B of table-dtype elements, or 32 B of fp32 for OUT32 with 16-bit tables) at p.
 template <class Tr, bool OUT32>
-__device__ __forceinline__ void store_pooled(char* out, size_t g, uint32_t nvec, int sl, const float2 (&acc)[Tr::kAcc / 2]) {
+__device__ __forceinline__ void store_pooled(char* p, const float2 (&acc)[Tr::kAcc / 2]) {
     if constexpr (OUT32 && Tr::kAcc == 8) {
         const float f[8] = {acc[0].x, acc[0].y, acc[1].x, acc[1].y, acc[2].x, acc[2].y, acc[3].x, acc[3].y};
-        st_out32(out + g * (static_cast<size_t>(nvec) * 32) + sl * 32, f);
+        st_out32(p, f);
     } else {
-        st_out16(out + g * (static_cast<size_t>(nvec) * 16) + sl * 16, Tr::pack(acc));
+        st_out16(p, Tr::pack(acc));
     }
 }
+
+// Per-table record of the general (GEN) variant, staged in shared memory.
+struct TableInfo {
+    const char* base;
+    uint32_t nvec;     // 16-byte vectors per row of this table
+    uint32_t col_vec;  // first output vector of this table's column block = sum of nvec over earlier tables
+};
+
+// One bag as the kernel sees it: where its rows come from and where its pooled vector goes.
+struct BagRef {
+    const char* tab;   // table base + this lane's 16-byte slot
+    char* outp;        // GEN only: this lane's output slot (the dense layout recomputes it from g at the store)
+    uint32_t t;
+    uint32_t row_bytes;
+    bool ok;           // this lane holds a vector of the row
+};
 
 // U = 2 (the default: double buffering makes it 2..4 row loads in flight per lane) is held to 64 registers so
 // that 4 CTAs = 32 warps stay resident per SM for every dtype (ptxas: 0-24 bytes of spill, all on cold paths);
 // the deeper unrolls keep their natural allocation (<= 80 registers, 3 CTAs).
-template <class Tr, int W, int U, bool OUT32>
-__global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kernel(const LookupArgs a) {
+//
+// GEN = false is the path of BASELINE.json's configs: one D, int32 ids, sample-major bags, dense [B, T*D] block.
+// GEN = true adds the interface variants of SURVEY.md §8(f) NEXT-2 / NEXT-3 (dpi_lookup_ex): per-table dims,
+// int64 ids (the low word is read: rows < 2^31), per-entry fp32 weights (acc = fma(w, row, acc)), table-major
+// bags (g = t*B + b) and an output row pitch, so a column block can be written into a wider row.
+template <class Tr, int W, int U, bool OUT32, bool GEN>
+__global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <= 2 ? 3 : 1)) lookup_kernel(const LookupArgs a) {
     constexpr int P = 32 / W;
     constexpr int kAcc = Tr::kAcc;
     constexpr int kAcc2 = kAcc / 2;
+    constexpr int kOutVec = (OUT32 && kAcc == 8) ? 32 : 16;  // output bytes per lane
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int lane = threadIdx.x & 31;
@@ -166,28 +203,88 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
     const uint32_t n_warps = gridDim.x * warps_per_cta;
     const uint32_t warp_in_cta = threadIdx.x >> 5;
     const uint32_t warp_id = blockIdx.x * warps_per_cta + warp_in_cta;
-    const size_t row_bytes = static_cast<size_t>(a.nvec) * 16;
+    const uint32_t row_bytes_u = a.nvec * 16;  // non-GEN: every table
     char* const out = static_cast<char*>(a.out);
 
-    // smem: [T table base pointers][per warp: idx stage x2, offsets stage x2]
+    // smem: [per-table records][per warp: idx stage x2, offsets stage x2, (GEN) weight stage x2]
+    const int ish = GEN ? static_cast<int>(a.idx_shift) : 0;
+    const int stage_idx = kStageIdx << ish;  // 32-bit words per index buffer
     const char** s_tab = reinterpret_cast<const char**>(smem_raw);
-    int* const s_warp = reinterpret_cast<int*>(smem_raw + ((static_cast<size_t>(a.T) * 8 + 15) & ~static_cast<size_t>(15))) +
-                        warp_in_cta * kWarpStageInts;
-    for (uint32_t t = threadIdx.x; t < a.T; t += blockDim.x) s_tab[t] = static_cast<const char*>(a.tables[t]);
+    const TableInfo* s_info = reinterpret_cast<const TableInfo*>(smem_raw);
+    const size_t tab_bytes = GEN ? static_cast<size_t>(a.T) * sizeof(TableInfo)
+                                 : ((static_cast<size_t>(a.T) * 8 + 15) & ~static_cast<size_t>(15));
+    const int warp_words = 2 * stage_idx + 2 * kStageOff + ((GEN && a.weights) ? 2 * kStageIdx : 0);
+    int* const s_warp = reinterpret_cast<int*>(smem_raw + tab_bytes) + warp_in_cta * warp_words;
+    int* const s_off = s_warp + 2 * stage_idx;
+    float* const s_wgt = reinterpret_cast<float*>(s_off + 2 * kStageOff);
+    if constexpr (GEN) {
+        TableInfo* w_info = reinterpret_cast<TableInfo*>(smem_raw);
+        for (uint32_t t = threadIdx.x; t < a.T; t += blockDim.x) {
+            TableInfo ti;
+            ti.base = static_cast<const char*>(a.tables[t]);
+            ti.nvec = a.tab_nvec[t];
+            ti.col_vec = a.tab_col[t];
+            w_info[t] = ti;
+        }
+    } else {
+        const char** w_tab = reinterpret_cast<const char**>(smem_raw);
+        for (uint32_t t = threadIdx.x; t < a.T; t += blockDim.x) w_tab[t] = static_cast<const char*>(a.tables[t]);
+    }
     __syncthreads();
 
     griddep_wait();  // PDL: the planner's writes are visible past this point (no-op otherwise)
     const uint32_t S = static_cast<uint32_t>(a.meta[META_S]);
     if (warp_id >= S) return;
 
-    // Stage offsets[g_lo..g_hi] and indices[e_lo..e_hi) of one task into buffer `b` (if they fit).
+    // bag id -> table, rows, output slot
+    auto bag_ref = [&](uint32_t g) -> BagRef {
+        BagRef r;
+        if constexpr (GEN) {
+            uint32_t b;
+            if (a.table_major) { r.t = g / a.B; b = g - r.t * a.B; }
+            else { b = g / a.T; r.t = g - b * a.T; }
+            const TableInfo ti = s_info[r.t];
+            r.tab = ti.base + sl * 16;
+            r.row_bytes = ti.nvec * 16;
+            r.ok = static_cast<uint32_t>(sl) < ti.nvec;
+            r.outp = out + static_cast<size_t>(b) * a.out_pitch + static_cast<size_t>(ti.col_vec) * kOutVec + sl * kOutVec;
+        } else {
+            r.t = g % a.T;
+            r.tab = s_tab[r.t] + sl * 16;
+            r.row_bytes = row_bytes_u;
+            r.ok = vec_ok;
+            r.outp = nullptr;
+        }
+        return r;
+    };
+    auto out_of = [&](uint32_t g, const BagRef& r) -> char* {
+        if constexpr (GEN) return r.outp;
+        else return out + static_cast<size_t>(g) * (static_cast<size_t>(a.nvec) * kOutVec) + sl * kOutVec;
+    };
+    auto idx_at = [&](const int* ip, int e) -> int { return GEN ? ip[e << ish] : ip[e]; };
+    auto wgt_at = [&](const float* wp, int e) -> float { return (GEN && wp) ? wp[e] : 1.f; };
+    auto accum = [&](float2 (&acc)[kAcc2], const uint4& v, float w) {
+        if constexpr (GEN) Tr::fma(acc, v, make_float2(w, w));  // fma(x, 1, acc) == x + acc exactly
+        else Tr::add(acc, v);
+    };
+    auto is_mean = [&](uint32_t t) -> bool { return (a.pool.w[t >> 5] >> (t & 31)) & 1u; };
+
+    // Stage offsets[g_lo..g_hi] and indices[e_lo..e_hi) (and weights) of one task into buffer `b` (if they fit).
     auto stage = [&](const int2 r_lo, const int2 r_hi, int b) {
         const int nb1 = r_hi.x - r_lo.x + 1, ne = r_hi.y - r_lo.y;
         if (r_hi.x > r_lo.x && nb1 <= kStageOff && ne <= kStageIdx) {
-            int* ib = s_warp + b * kStageIdx;
-            int* ob = s_warp + 2 * kStageIdx + b * kStageOff;
-            for (int i = lane; i < ne; i += 32) cp_async4(ib + i, a.indices + r_lo.y + i);
+            int* ib = s_warp + b * stage_idx;
+            int* ob = s_off + b * kStageOff;
+            const int nw = ne << ish;
+            const int* src = a.indices + (static_cast<size_t>(r_lo.y) << ish);
+            for (int i = lane; i < nw; i += 32) cp_async4(ib + i, src + i);
             for (int i = lane; i < nb1; i += 32) cp_async4(ob + i, a.offsets + r_lo.x + i);
+            if constexpr (GEN) {
+                if (a.weights) {
+                    float* wb = s_wgt + b * kStageIdx;
+                    for (int i = lane; i < ne; i += 32) cp_async4(wb + i, a.weights + r_lo.y + i);
+                }
+            }
         }
         cp_async_commit();
     };
@@ -222,11 +319,15 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
             const uint32_t ne = static_cast<uint32_t>(e_hi - e_lo);
             const bool staged = (nb + 1 <= static_cast<uint32_t>(kStageOff)) && (ne <= static_cast<uint32_t>(kStageIdx));
             // generic pointers indexed by ABSOLUTE entry / bag id: staged smem or the global arrays
-            const int* ip = staged ? (s_warp + buf * kStageIdx - e_lo) : a.indices;
-            const int* op = staged ? (s_warp + 2 * kStageIdx + buf * kStageOff - static_cast<int>(g_lo)) : a.offsets;
+            const int* ip = staged ? (s_warp + buf * stage_idx - (e_lo << ish)) : a.indices;
+            const int* op = staged ? (s_off + buf * kStageOff - static_cast<int>(g_lo)) : a.offsets;
+            const float* wp = nullptr;
+            if constexpr (GEN) {
+                if (a.weights) wp = staged ? (s_wgt + buf * kStageIdx - e_lo) : a.weights;
+            }
 
             bool onehot = false;
-            if (ne == nb && a.mode != 2) {
+            if (ne == nb && a.mode != 2 && !(GEN && wp)) {
                 // a task with ne == nb could still mix empty and longer bags: verify
                 bool all_one = true;
                 for (uint32_t i = lane; i < nb; i += 32) all_one &= (op[g_lo + i + 1] - op[g_lo + i]) == 1;
@@ -236,25 +337,29 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
                 // ---------------- one-hot task: Alg. 1, a pure row copy (bit-exact) ------------------------
                 for (uint32_t i0 = 0; i0 < nb; i0 += P * U) {
                     uint4 v[U];
+                    BagRef br[GEN ? U : 1];
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         const uint32_t i = i0 + u * P + sub;
                         const bool ok = i < nb;
-                        const uint32_t g = g_lo + (ok ? i : 0u);
-                        const int r = ip[e_lo + (ok ? i : 0u)];
-                        v[u] = ld_row16(s_tab[g % a.T] + sl * 16 + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
+                        BagRef& b = br[GEN ? u : 0];
+                        b = bag_ref(g_lo + (ok ? i : 0u));
+                        const int r = idx_at(ip, e_lo + (ok ? i : 0u));
+                        v[u] = ld_row16(b.tab + static_cast<size_t>(r) * b.row_bytes, ok && b.ok);
                     }
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         const uint32_t i = i0 + u * P + sub;
-                        if (i < nb && vec_ok) {
+                        const BagRef& b = br[GEN ? u : 0];
+                        if (i < nb && b.ok) {  // dense layout: b.ok == vec_ok for every bag
+                            char* po = out_of(g_lo + i, b);
                             if constexpr (OUT32 && kAcc == 8) {
                                 float2 f[kAcc2];
                                 zero_acc(f);
                                 Tr::add(f, v[u]);
-                                store_pooled<Tr, OUT32>(out, g_lo + i, a.nvec, sl, f);
+                                store_pooled<Tr, OUT32>(po, f);
                             } else {
-                                st_out16(out + static_cast<size_t>(g_lo + i) * row_bytes + sl * 16, v[u]);
+                                st_out16(po, v[u]);
                             }
                         }
                     }
@@ -267,45 +372,49 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
                     const uint32_t gc = active ? g : g_lo;
                     const int lo = op[gc];
                     const int hi = active ? op[gc + 1] : lo;
-                    const uint32_t t = gc % a.T;
-                    const char* tab = s_tab[t] + sl * 16;
+                    const BagRef br = bag_ref(gc);
                     float2 acc[kAcc2];
                     zero_acc(acc);
                     for (int j = lo; j < hi; j += U) {
                         uint4 v[U];
+                        float w[U];
 #pragma unroll
                         for (int u = 0; u < U; ++u) {
                             const bool ok = j + u < hi;
-                            const int r = ip[ok ? j + u : lo];
-                            v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
+                            const int e = ok ? j + u : lo;
+                            const int r = idx_at(ip, e);
+                            w[u] = wgt_at(wp, e);
+                            v[u] = ld_row16(br.tab + static_cast<size_t>(r) * br.row_bytes, ok && br.ok);
                         }
 #pragma unroll
-                        for (int u = 0; u < U; ++u) Tr::add(acc, v[u]);
+                        for (int u = 0; u < U; ++u) accum(acc, v[u], w[u]);
                     }
-                    if (active && vec_ok) {
-                        if (((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
-                        store_pooled<Tr, OUT32>(out, g, a.nvec, sl, acc);
+                    if (active && br.ok) {
+                        if (is_mean(br.t) && hi - lo > 1) scale_mean(acc, hi - lo);
+                        store_pooled<Tr, OUT32>(out_of(g, br), acc);
                     }
                 }
             } else if (a.mode == 2) {
                 // ---------------- whole warp per bag, one batch at a time (kept for A/B measurements) ------
                 for (uint32_t g = g_lo; g < g_hi; ++g) {
                     const int lo = op[g], hi = op[g + 1];
-                    const uint32_t t = g % a.T;
-                    const char* tab = s_tab[t] + sl * 16;
+                    const BagRef br = bag_ref(g);
                     float2 acc[kAcc2];
                     zero_acc(acc);
                     for (int j = lo; j < hi; j += P * U) {
                         uint4 v[U];
+                        float w[U];
 #pragma unroll
                         for (int u = 0; u < U; ++u) {
                             const int e = j + u * P + sub;
                             const bool ok = e < hi;
-                            const int r = ip[ok ? e : lo];
-                            v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
+                            const int ec = ok ? e : lo;
+                            const int r = idx_at(ip, ec);
+                            w[u] = wgt_at(wp, ec);
+                            v[u] = ld_row16(br.tab + static_cast<size_t>(r) * br.row_bytes, ok && br.ok);
                         }
 #pragma unroll
-                        for (int u = 0; u < U; ++u) Tr::add(acc, v[u]);
+                        for (int u = 0; u < U; ++u) accum(acc, v[u], w[u]);
                     }
 #pragma unroll
                     for (int d = W; d < 32; d <<= 1) {
@@ -314,9 +423,9 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
                             acc[i] = __fadd2_rn(acc[i], make_float2(__shfl_xor_sync(0xffffffffu, acc[i].x, d),
                                                                     __shfl_xor_sync(0xffffffffu, acc[i].y, d)));
                     }
-                    if (sub == 0 && vec_ok) {
-                        if (((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
-                        store_pooled<Tr, OUT32>(out, g, a.nvec, sl, acc);
+                    if (sub == 0 && br.ok) {
+                        if (is_mean(br.t) && hi - lo > 1) scale_mean(acc, hi - lo);
+                        store_pooled<Tr, OUT32>(out_of(g, br), acc);
                     }
                 }
             } else {
@@ -324,20 +433,27 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
                 // The loads of batch k+1 (possibly the first batch of the NEXT bag: its offsets and indices
                 // are already in smem) are issued before batch k is consumed, so a warp keeps U..2U row
                 // loads per lane in flight across batch and bag boundaries instead of draining at each one.
+                struct Buf {
+                    uint4 v[U];
+                    float w[GEN ? U : 1];
+                };
                 auto store_zero = [&](uint32_t gz) {
-                    if (sub == 0 && vec_ok) {
+                    const BagRef bz = bag_ref(gz);
+                    if (sub == 0 && bz.ok) {
                         float2 z[kAcc2];
                         zero_acc(z);
-                        store_pooled<Tr, OUT32>(out, gz, a.nvec, sl, z);
+                        store_pooled<Tr, OUT32>(out_of(gz, bz), z);
                     }
                 };
-                auto issue = [&](uint4 (&v)[U], int j, int hi, const char* tab) {
+                auto issue = [&](Buf& bf, int j, int hi, const BagRef& br) {
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         const int e = j + u * P + sub;
                         const bool ok = e < hi;
-                        const int r = ip[ok ? e : j];
-                        v[u] = ld_row16(tab + static_cast<size_t>(r) * row_bytes, ok && vec_ok);
+                        const int ec = ok ? e : j;
+                        const int r = idx_at(ip, ec);
+                        if constexpr (GEN) bf.w[u] = wgt_at(wp, ec);
+                        bf.v[u] = ld_row16(br.tab + static_cast<size_t>(r) * br.row_bytes, ok && br.ok);
                     }
                 };
                 uint32_t g = g_lo;
@@ -350,16 +466,16 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
                 }
                 if (g < g_hi) {
                     int j = lo;
-                    const char* tab = s_tab[g % a.T] + sl * 16;
+                    BagRef br = bag_ref(g);
                     float2 acc[kAcc2];
                     zero_acc(acc);
-                    uint4 vA[U], vB[U];
-                    issue(vA, j, hi, tab);
+                    Buf bA, bB;
+                    issue(bA, j, hi, br);
                     bool more = true;
-                    auto step = [&](uint4 (&cv)[U], uint4 (&nv)[U]) {
+                    auto step = [&](Buf& cv, Buf& nv) {
                         uint32_t g_n = g;
                         int j_n = j + P * U, lo_n = lo, hi_n = hi;
-                        const char* tab_n = tab;
+                        BagRef br_n = br;
                         const bool last_of_bag = j_n >= hi;
                         bool has_next = true;
                         if (last_of_bag) {
@@ -372,11 +488,11 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
                                 store_zero(g_n);
                                 ++g_n;
                             }
-                            if (has_next) { j_n = lo_n; tab_n = s_tab[g_n % a.T] + sl * 16; }
+                            if (has_next) { j_n = lo_n; br_n = bag_ref(g_n); }
                         }
-                        if (has_next) issue(nv, j_n, hi_n, tab_n);
+                        if (has_next) issue(nv, j_n, hi_n, br_n);
 #pragma unroll
-                        for (int u = 0; u < U; ++u) Tr::add(acc, cv[u]);
+                        for (int u = 0; u < U; ++u) accum(acc, cv.v[u], GEN ? cv.w[u] : 1.f);
                         if (last_of_bag) {
 #pragma unroll
                             for (int d = W; d < 32; d <<= 1) {
@@ -385,20 +501,19 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
                                     acc[i] = __fadd2_rn(acc[i], make_float2(__shfl_xor_sync(0xffffffffu, acc[i].x, d),
                                                                             __shfl_xor_sync(0xffffffffu, acc[i].y, d)));
                             }
-                            if (sub == 0 && vec_ok) {
-                                const uint32_t t = g % a.T;
-                                if (((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
-                                store_pooled<Tr, OUT32>(out, g, a.nvec, sl, acc);
+                            if (sub == 0 && br.ok) {
+                                if (is_mean(br.t) && hi - lo > 1) scale_mean(acc, hi - lo);
+                                store_pooled<Tr, OUT32>(out_of(g, br), acc);
                             }
                             zero_acc(acc);
                         }
-                        g = g_n; j = j_n; lo = lo_n; hi = hi_n; tab = tab_n;
+                        g = g_n; j = j_n; lo = lo_n; hi = hi_n; br = br_n;
                         more = has_next;
                     };
                     while (more) {
-                        step(vA, vB);
+                        step(bA, bB);
                         if (!more) break;
-                        step(vB, vA);
+                        step(bB, bA);
                     }
                 }
             }
@@ -415,17 +530,20 @@ __global__ void __launch_bounds__(kLookupMaxThreads, U <= 2 ? 4 : 1) lookup_kern
 }
 
 // ---- host-side dispatch (one translation unit per dtype keeps nvcc parallel) ------------------------------
-inline size_t lookup_smem_bytes(uint32_t T, int block_threads) {
-    return ((static_cast<size_t>(T) * 8 + 15) & ~static_cast<size_t>(15)) +
-           static_cast<size_t>(block_threads / 32) * kWarpStageInts * sizeof(int);
+inline size_t lookup_smem_bytes(const LookupArgs& a, bool gen, int block_threads) {
+    const size_t tab = gen ? static_cast<size_t>(a.T) * sizeof(TableInfo)
+                           : ((static_cast<size_t>(a.T) * 8 + 15) & ~static_cast<size_t>(15));
+    const int ish = gen ? static_cast<int>(a.idx_shift) : 0;
+    const size_t warp_words = 2 * (static_cast<size_t>(kStageIdx) << ish) + 2 * kStageOff + ((gen && a.weights) ? 2 * kStageIdx : 0);
+    return tab + static_cast<size_t>(block_threads / 32) * warp_words * sizeof(int);
 }
 
-template <class Tr, int W, int U, bool OUT32>
+template <class Tr, int W, int U, bool OUT32, bool GEN>
 cudaError_t launch_one(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream) {
-    const size_t smem = lookup_smem_bytes(a.T, l.block_threads);
+    const size_t smem = lookup_smem_bytes(a, GEN, l.block_threads);
     static size_t smem_set = 0;  // per instantiation: raise the dynamic smem limit once (or when it grows)
     if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(lookup_kernel<Tr, W, U, OUT32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(lookup_kernel<Tr, W, U, OUT32, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              static_cast<int>(smem));
         if (e != cudaSuccess) return e;
         smem_set = smem;
@@ -441,16 +559,16 @@ cudaError_t launch_one(const LookupArgs& a, const LookupLaunch& l, cudaStream_t 
     cfg.attrs = attr;
     cfg.numAttrs = l.pdl ? 1 : 0;
     count_launch();
-    return cudaLaunchKernelEx(&cfg, lookup_kernel<Tr, W, U, OUT32>, a);
+    return cudaLaunchKernelEx(&cfg, lookup_kernel<Tr, W, U, OUT32, GEN>, a);
 }
 
-template <class Tr, int W, int U, bool OUT32>
-int occupancy_one(uint32_t T, int block_threads) {
+template <class Tr, int W, int U, bool OUT32, bool GEN>
+int occupancy_one(const LookupArgs& a, int block_threads) {
     int n = 0;
-    const size_t smem = lookup_smem_bytes(T, block_threads);
+    const size_t smem = lookup_smem_bytes(a, GEN, block_threads);
     if (smem > 48 * 1024)
-        (void)cudaFuncSetAttribute(lookup_kernel<Tr, W, U, OUT32>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, lookup_kernel<Tr, W, U, OUT32>, block_threads, smem) != cudaSuccess) {
+        (void)cudaFuncSetAttribute(lookup_kernel<Tr, W, U, OUT32, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, lookup_kernel<Tr, W, U, OUT32, GEN>, block_threads, smem) != cudaSuccess) {
         (void)cudaGetLastError();
         return 0;
     }
@@ -461,6 +579,8 @@ int occupancy_one(uint32_t T, int block_threads) {
 #define DPI_FOR_EACH_WU(M) \
     DPI_FOR_EACH_U(M, 1) DPI_FOR_EACH_U(M, 2) DPI_FOR_EACH_U(M, 4) DPI_FOR_EACH_U(M, 8) DPI_FOR_EACH_U(M, 16) \
     DPI_FOR_EACH_U(M, 32)
+// The general variant (GEN) exists for the default unroll only.
+#define DPI_FOR_EACH_W_GEN(M) M(1, 2) M(2, 2) M(4, 2) M(8, 2) M(16, 2) M(32, 2)
 // Each lookup_<dtype>.cu defines DPI_TRAITS / DPI_SUFFIX (/ DPI_HAS_OUT32) and includes lookup_dispatch.inc.
 
 }  // namespace dpi

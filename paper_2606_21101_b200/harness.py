@@ -63,6 +63,18 @@ def tables_from_host(cfg: W.Config, host_tables: List[np.ndarray], device="cuda:
     return DeviceTables(cfg, rows, tables, ptrs)
 
 
+def tables_from_host_mixed(host_tables: List[np.ndarray], dtype: str, device="cuda:0"):
+    """Upload host tables of possibly different widths; returns (device tensors, device pointer array)."""
+    require_cuda()
+    tables = []
+    for a in host_tables:
+        a = np.ascontiguousarray(a)
+        t = torch.from_numpy(a.view(np.int16)).to(device).view(torch.bfloat16) if dtype == "bf16" else torch.from_numpy(a).to(device)
+        assert t.dtype == TORCH_DTYPE[dtype]
+        tables.append(t.contiguous())
+    return tables, torch.tensor([t.data_ptr() for t in tables], dtype=torch.int64, device=device)
+
+
 @dataclass
 class DeviceBatch:
     lengths: torch.Tensor  # int32[G] device

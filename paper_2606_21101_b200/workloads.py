@@ -41,7 +41,7 @@ GAMMA = 0x9E3779B97F4A7C15
 SUBMUL = 0xD1B54A32D192ED03
 _M64 = (1 << 64) - 1
 
-STREAM_ROWS, STREAM_LEN, STREAM_EMPTY, STREAM_IDX, STREAM_VAL = 1, 2, 3, 4, 5
+STREAM_ROWS, STREAM_LEN, STREAM_EMPTY, STREAM_IDX, STREAM_VAL, STREAM_WGT = 1, 2, 3, 4, 5, 6
 
 DTYPES = ("f32", "f16", "bf16")
 DTYPE_BYTES = {"f32": 4, "f16": 2, "bf16": 2}
@@ -374,6 +374,32 @@ def compact_subproblem(cfg: Config, batch: Batch, sample_ids: Sequence[int]) -> 
         heights.append(uniq.size)
     return CompactProblem(cfg, sample_ids, ln.astype(np.int32), new_idx, tables,
                           np.asarray(heights, dtype=np.int64))
+
+
+# ----------------------------------------------------------------------------------------------------
+# interface variants: data movement and draws only
+# ----------------------------------------------------------------------------------------------------
+def make_weights(batch_seed: int, n: int, lo: float = 0.0, hi: float = 2.0) -> np.ndarray:
+    """float32[n] per-entry weights, uniform in [lo, hi) (one per flat index entry, sample-major entry order)."""
+    u = unit_f64(hash_u64(stream_key(batch_seed, STREAM_WGT), np.arange(n, dtype=np.uint64)))
+    return (lo + u * (hi - lo)).astype(np.float32)
+
+
+def to_table_major(T: int, B: int, lengths: np.ndarray, *per_entry: np.ndarray):
+    """Re-order a sample-major batch (bag g = b*T + t) into table-major order (bag g' = t*B + b): returns the
+    permuted lengths and every per-entry array (indices, weights, ...) with its bags moved along. Pure permutation."""
+    lengths = np.asarray(lengths, dtype=np.int64)
+    perm = np.arange(B * T).reshape(B, T).T.reshape(-1)  # table-major position -> sample-major bag id
+    starts = np.concatenate(([0], np.cumsum(lengths)))[:-1]
+    ln_tm = lengths[perm]
+    n = int(lengths.sum())
+    src = np.repeat(starts[perm], ln_tm) + (np.arange(n) - np.repeat(np.cumsum(ln_tm) - ln_tm, ln_tm))
+    return (ln_tm.astype(np.int32),) + tuple(np.ascontiguousarray(np.asarray(a)[src]) for a in per_entry)
+
+
+def mixed_dim_tables(seed: int, dims: Sequence[int], rows: Sequence[int], dtype: str) -> List[np.ndarray]:
+    """Host tables of different widths with the seeded value recipe (storage format), small tables only."""
+    return [to_storage(table_values_f32(seed, t, int(dims[t]), np.arange(int(rows[t]))), dtype) for t in range(len(dims))]
 
 
 def algorithmic_bytes(cfg: Config, G: int, N: int, S: int = 0) -> dict:

@@ -123,3 +123,22 @@ def test_compact_subproblem_matches_full_tables():
             assert np.array_equal(got_rows, full[t][orig])
             pos += L
     assert pos == sub.indices.shape[0]
+
+
+def test_to_table_major_is_the_bag_grid_transpose():
+    rng = np.random.default_rng(0)
+    T, B = 3, 5
+    ln = rng.integers(0, 4, size=B * T).astype(np.int32)
+    idx = np.arange(int(ln.sum()), dtype=np.int32) + 100
+    w = W.make_weights(1, idx.shape[0])
+    assert w.dtype == np.float32 and (w >= 0).all() and (w < 2).all()
+    ln_tm, idx_tm, w_tm = W.to_table_major(T, B, ln, idx, w)
+    starts = np.concatenate(([0], np.cumsum(ln)))
+    pos = 0
+    for t in range(T):
+        for b in range(B):
+            g = b * T + t
+            assert ln_tm[t * B + b] == ln[g]
+            seg = slice(starts[g], starts[g + 1])
+            assert np.array_equal(idx_tm[pos:pos + ln[g]], idx[seg]) and np.array_equal(w_tm[pos:pos + ln[g]], w[seg])
+            pos += ln[g]
