@@ -65,15 +65,14 @@ struct dpi_plan_s {
     int32_t K = 0;           // effective quantum
     int32_t K_user = 0;      // 0 = default
     uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
-    uint32_t num_tiles = 0;
+    uint32_t num_tiles = 0, num_chunks = 0, tiles_per_chunk = 0;
     int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0};
     // device
     int device = 0, num_sms = 0;
     int32_t* offsets = nullptr;
     int2* seg = nullptr;          // {seg_bag[s], seg_off[s]} interleaved
     int32_t* meta = nullptr;
-    unsigned long long* tile_len = nullptr;
-    unsigned long long* tile_cost = nullptr;
+    ulonglong2* status = nullptr;    // planner look-back records, one per chunk
     unsigned int* state = nullptr;   // planner device state {ticket, done, epoch, -}
     int64_t* table_rows_dev = nullptr;
     uint32_t* tab_nvec_dev = nullptr;   // [T] 16-byte vectors per row of each table
@@ -119,8 +118,8 @@ dpi_status_t ensure_seg_capacity(dpi_plan_t* p, int32_t K) {
 
 void free_plan(dpi_plan_t* p) {
     if (!p) return;
-    cudaFree(p->offsets); cudaFree(p->seg); cudaFree(p->meta); cudaFree(p->tile_len);
-    cudaFree(p->tile_cost); cudaFree(p->state); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
+    cudaFree(p->offsets); cudaFree(p->seg); cudaFree(p->meta); cudaFree(p->status);
+    cudaFree(p->state); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
     cudaFree(p->tab_nvec_dev); cudaFree(p->tab_col_dev);
     cudaFree(p->stage_len); cudaFree(p->stage_idx); cudaFree(p->stage_out);
     (void)cudaGetLastError();
@@ -288,6 +287,16 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     p->device = dev;
     p->num_sms = prop.multiProcessorCount;
     p->num_tiles = (p->G + kScanTile - 1) / kScanTile;
+    {
+        // planner grid: whole tiles per CTA, at most 2 CTAs per SM (all co-resident: 64 registers x 256 threads)
+        uint32_t max_chunks = static_cast<uint32_t>(2 * p->num_sms);
+        if (max_chunks > static_cast<uint32_t>(kMaxChunks)) max_chunks = kMaxChunks;
+        if (max_chunks < 1) max_chunks = 1;
+        p->tiles_per_chunk = (p->num_tiles + max_chunks - 1) / max_chunks;
+        if (p->tiles_per_chunk < 1) p->tiles_per_chunk = 1;
+        p->num_chunks = (p->num_tiles + p->tiles_per_chunk - 1) / p->tiles_per_chunk;
+        if (p->num_chunks < 1) p->num_chunks = 1;
+    }
     p->K = default_quantum(p);
 
 #define DPI_TRY(call)                                   \
@@ -302,10 +311,8 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     DPI_TRY(cudaMalloc(&p->offsets, (static_cast<size_t>(p->G) + 1) * sizeof(int32_t)));
     DPI_TRY(cudaMalloc(&p->meta, kMetaWords * sizeof(int32_t)));
     DPI_TRY(cudaMemset(p->meta, 0, kMetaWords * sizeof(int32_t)));
-    DPI_TRY(cudaMalloc(&p->tile_len, p->num_tiles * sizeof(unsigned long long)));
-    DPI_TRY(cudaMalloc(&p->tile_cost, p->num_tiles * sizeof(unsigned long long)));
-    DPI_TRY(cudaMemset(p->tile_len, 0, p->num_tiles * sizeof(unsigned long long)));
-    DPI_TRY(cudaMemset(p->tile_cost, 0, p->num_tiles * sizeof(unsigned long long)));
+    DPI_TRY(cudaMalloc(&p->status, kMaxChunks * sizeof(ulonglong2)));
+    DPI_TRY(cudaMemset(p->status, 0, kMaxChunks * sizeof(ulonglong2)));
     {
         const unsigned int init[kStateWords] = {0u, 0u, 1u, 0u};  // ticket, done, epoch = 1 (status words start at 0)
         DPI_TRY(cudaMalloc(&p->state, sizeof init));
@@ -374,13 +381,14 @@ dpi_status_t dpi_plan_build(dpi_plan_t* p, const int32_t* lengths_dev, void* str
     a.offsets = p->offsets;
     a.seg = p->seg;
     a.meta = p->meta;
-    a.tile_len = p->tile_len;
-    a.tile_cost = p->tile_cost;
+    a.status = p->status;
     a.state = p->state;
     a.G = p->G;
     a.K = static_cast<uint32_t>(p->K);
     a.seg_cap = p->seg_cap;
     a.num_tiles = p->num_tiles;
+    a.num_chunks = p->num_chunks;
+    a.tiles_per_chunk = p->tiles_per_chunk;
     a.max_indices = static_cast<uint32_t>(p->max_indices);
     cudaError_t e = launch_plan(a, s);
     if (e != cudaSuccess) return cuda_fail(e, "plan kernel launch");

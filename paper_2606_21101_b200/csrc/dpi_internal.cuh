@@ -25,7 +25,8 @@ struct PoolMask {
 // ---- planner (plan_kernels.cu) ---------------------------------------------------------------------
 constexpr int kScanThreads = 256;
 constexpr int kScanItems = 8;                               // consecutive bags per thread (two int4 loads)
-constexpr int kScanTile = kScanThreads * kScanItems;        // 2048 bags per CTA
+constexpr int kScanTile = kScanThreads * kScanItems;        // 2048 bags per tile
+constexpr int kMaxChunks = 320;                             // CTAs of the planner (all co-resident); multiple of 32
 
 enum PlanState { kStateTicket = 0, kStateDone = 1, kStateEpoch = 2, kStateWords = 4 };
 constexpr uint32_t kEpochLimit = 1u << 30;  // status words carry a 30-bit epoch
@@ -35,14 +36,16 @@ struct PlanArgs {
     int32_t* __restrict__ offsets;     // [G+1]
     int2* __restrict__ seg;            // [seg_cap] {seg_bag[s], seg_off[s] = offsets[seg_bag[s]]}
     int32_t* __restrict__ meta;        // [kMetaWords]
-    unsigned long long* tile_len;      // [num_tiles] look-back status words for the length scan
-    unsigned long long* tile_cost;     // [num_tiles] look-back status words for the cost scan
+    ulonglong2* status;                // [num_chunks] look-back records {len aggregate, cost aggregate}, each half
+                                       // tagged {epoch:30 | state:2 | value:32}
     unsigned int* state;               // [kStateTicket] dynamic tile id, [kStateDone] finished tiles (both
                                        // self-resetting atomicInc), [kStateEpoch] tag of this build's status words
     uint32_t G;
     uint32_t K;
     uint32_t seg_cap;
-    uint32_t num_tiles;
+    uint32_t num_tiles;                // ceil(G / kScanTile)
+    uint32_t num_chunks;               // CTAs: min(num_tiles, 2 * SMs, kMaxChunks)
+    uint32_t tiles_per_chunk;          // ceil(num_tiles / num_chunks) (num_chunks is then re-derived so no chunk is empty)
     uint32_t max_indices;
 };
 

@@ -1,7 +1,17 @@
 // plan_kernels.cu -- steps a1 + a2 of the path: "anticipate the whole workload".
 //
 // ONE launch over all G = B*T (sample, table) bags -- no per-table launches:
-//   * single-pass decoupled look-back exclusive scan of (len, cost = max(len,1)) pairs  -> offsets[G+1]
+//   * chunked single-pass exclusive scan of (len, cost = max(len,1)) pairs -> offsets[G+1]. The bags are cut into
+//     C <= kMaxChunks contiguous chunks (whole 2048-bag tiles), one CTA per chunk, all CTAs co-resident:
+//       pass 1  the CTA sums its chunk and publishes ONE status record {len aggregate, cost aggregate};
+//       look-back  warp 0 reads the records of ALL earlier chunks at once (<= 320 records, 16 B each, every load
+//                  in flight together) and adds them up -- one L2 round trip after the last predecessor publishes,
+//                  no inclusive state, no chain;
+//       pass 2  the CTA scans its chunk tile by tile from that prefix (a one-tile chunk keeps its lengths in
+//               registers, larger chunks re-read them from L1/L2) and writes offsets and segments.
+//     (The first version was a textbook decoupled look-back over one status word per 2048-bag tile: with hundreds
+//     of CTAs polling the same few cache lines it cost ~25 ns per TILE -- 13.5 us at G = 524 K, 75 us at
+//     G = 6.5 M -- against ~3 us of launch latency.)
 //   * fused partition: bag g knows C[g] and C[g+1]; it owns every quantum boundary s*K in (C[g], C[g+1]],
 //     i.e. seg_bag[s] = g+1 for s = floor(C[g]/K)+1 .. floor(C[g+1]/K).  That is exactly
 //     seg_bag[s] = min{g : C[g] >= s*K} without any binary search or second kernel.
@@ -16,18 +26,23 @@ namespace dpi {
 namespace {
 
 constexpr uint32_t kStateAggregate = 1u;
-constexpr uint32_t kStateInclusive = 2u;
 
-__device__ __forceinline__ unsigned long long ld_relaxed_gpu(const unsigned long long* p) {
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+__device__ __forceinline__ ulonglong2 ld_status(const ulonglong2* p) {
+    // The two 64-bit halves are validated independently (each carries epoch + state), so a torn 128-bit read is
+    // harmless: a half that is not ready yet is simply read again.
+    ulonglong2 v;
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_relaxed_gpu(unsigned long long* p, unsigned long long v) {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+__device__ __forceinline__ void st_status(ulonglong2* p, unsigned long long x, unsigned long long y) {
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(x), "l"(y) : "memory");
 }
 __device__ __forceinline__ unsigned long long pack_status(uint32_t epoch, uint32_t state, uint32_t value) {
     return (static_cast<unsigned long long>((epoch << 2) | state) << 32) | value;
+}
+__device__ __forceinline__ bool status_ready(unsigned long long w, uint32_t epoch) {
+    const uint32_t hi = static_cast<uint32_t>(w >> 32);
+    return (hi >> 2) == epoch && (hi & 3u) != 0u;
 }
 
 __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
@@ -36,205 +51,233 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
     return v;
 }
 
-// Warp-parallel decoupled look-back over two status arrays at once. Lane l inspects tile pos-l; the window
-// slides back 32 tiles until some lane sees an INCLUSIVE word. Tiles before 0 count as inclusive-zero.
-__device__ __forceinline__ void lookback(const unsigned long long* st_len, const unsigned long long* st_cost,
-                                         uint32_t tile, uint32_t epoch, uint32_t& pre_len, uint32_t& pre_cost) {
-    const int lane = threadIdx.x & 31;
-    uint32_t run_len = 0, run_cost = 0;
-    bool done_len = false, done_cost = false;  // warp-uniform
-    int pos = static_cast<int>(tile) - 1;
-    while (!(done_len && done_cost)) {
-        const int my = pos - lane;
-        uint32_t f_len = kStateInclusive, v_len = 0, f_cost = kStateInclusive, v_cost = 0;
-        if (my >= 0) {
-            if (!done_len) {
-                unsigned long long w;
-                uint32_t hi;
-                do {
-                    w = ld_relaxed_gpu(st_len + my);
-                    hi = static_cast<uint32_t>(w >> 32);
-                } while ((hi >> 2) != epoch || (hi & 3u) == 0u);
-                f_len = hi & 3u;
-                v_len = static_cast<uint32_t>(w);
-            }
-            if (!done_cost) {
-                unsigned long long w;
-                uint32_t hi;
-                do {
-                    w = ld_relaxed_gpu(st_cost + my);
-                    hi = static_cast<uint32_t>(w >> 32);
-                } while ((hi >> 2) != epoch || (hi & 3u) == 0u);
-                f_cost = hi & 3u;
-                v_cost = static_cast<uint32_t>(w);
-            }
-        }
-        if (!done_len) {
-            const uint32_t incl = __ballot_sync(0xffffffffu, f_len == kStateInclusive);
-            const int first = __ffs(incl) - 1;  // nearest predecessor that already has its inclusive prefix
-            run_len += warp_sum((first < 0 || lane <= first) ? v_len : 0u);
-            done_len = first >= 0;
-        }
-        if (!done_cost) {
-            const uint32_t incl = __ballot_sync(0xffffffffu, f_cost == kStateInclusive);
-            const int first = __ffs(incl) - 1;
-            run_cost += warp_sum((first < 0 || lane <= first) ? v_cost : 0u);
-            done_cost = first >= 0;
-        }
-        pos -= 32;
+// Sum of the aggregates of chunks 0..chunk-1 (warp-wide; every lane returns the totals). Lane l owns chunks
+// l, l+32, ...; all its loads are issued before the first is examined; only records that are not ready are re-read.
+__device__ __forceinline__ void lookback_all(const ulonglong2* status, uint32_t chunk, uint32_t epoch,
+                                             uint32_t& pre_len, uint32_t& pre_cost) {
+    constexpr int kDepth = kMaxChunks / 32;
+    const uint32_t lane = threadIdx.x & 31;
+    ulonglong2 w[kDepth];
+#pragma unroll
+    for (int k = 0; k < kDepth; ++k) {
+        const uint32_t c = lane + 32u * k;
+        w[k] = c < chunk ? ld_status(status + c) : make_ulonglong2(pack_status(epoch, kStateAggregate, 0u), pack_status(epoch, kStateAggregate, 0u));
     }
-    pre_len = run_len;
-    pre_cost = run_cost;
+    // Re-read every record that is not ready yet, all of them in flight together, until none is left (a serial
+    // re-poll costs one L2 round trip per record: 8 us for the last chunks when traced with %globaltimer).
+    for (;;) {
+        bool all_ready = true;
+#pragma unroll
+        for (int k = 0; k < kDepth; ++k) all_ready &= status_ready(w[k].x, epoch) && status_ready(w[k].y, epoch);
+        if (all_ready) break;
+#pragma unroll
+        for (int k = 0; k < kDepth; ++k) {
+            if (!(status_ready(w[k].x, epoch) && status_ready(w[k].y, epoch))) w[k] = ld_status(status + lane + 32u * k);
+        }
+    }
+    uint32_t sl = 0, sc = 0;
+#pragma unroll
+    for (int k = 0; k < kDepth; ++k) {
+        sl += static_cast<uint32_t>(w[k].x);
+        sc += static_cast<uint32_t>(w[k].y);
+    }
+    pre_len = warp_sum(sl);
+    pre_cost = warp_sum(sc);
 }
 
-__global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const PlanArgs a) {
-    __shared__ uint32_t s_tile, s_epoch;
-    __shared__ uint32_t s_wlen[kScanThreads / 32], s_wcost[kScanThreads / 32];
-    __shared__ uint32_t s_pre_len, s_pre_cost;
-
-    // The epoch that tags this build's look-back words lives in device memory and is advanced by the last tile
-    // to finish, so a build needs no host-side state: the same launch can be replayed from a CUDA graph.
-    if (threadIdx.x == 0) {
-        s_tile = atomicInc(a.state + kStateTicket, a.num_tiles - 1);  // wraps to 0 after the last tile
-        s_epoch = *reinterpret_cast<volatile unsigned int*>(a.state + kStateEpoch);
-    }
-    __syncthreads();
-    const uint32_t tile = s_tile;
-    const uint32_t epoch = s_epoch;
-    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+// Loads the kScanItems consecutive lengths of this thread in tile `tile` (zeros past G); returns how many are valid.
+__device__ __forceinline__ uint32_t load_items(const PlanArgs& a, uint32_t tile, uint32_t (&v)[kScanItems]) {
     const uint32_t base = tile * kScanTile + threadIdx.x * kScanItems;
-
-    // ---- load kScanItems consecutive lengths (two 128-bit loads when the whole run is in range) ----
-    uint32_t v[kScanItems];
-    uint32_t n_valid;
     if (base + kScanItems <= a.G && (reinterpret_cast<uintptr_t>(a.len) & 15u) == 0) {
         const int4 p0 = __ldg(reinterpret_cast<const int4*>(a.len + base));
         const int4 p1 = __ldg(reinterpret_cast<const int4*>(a.len + base) + 1);
         v[0] = p0.x; v[1] = p0.y; v[2] = p0.z; v[3] = p0.w;
         v[4] = p1.x; v[5] = p1.y; v[6] = p1.z; v[7] = p1.w;
-        n_valid = kScanItems;
-    } else {
-        n_valid = base < a.G ? min(a.G - base, static_cast<uint32_t>(kScanItems)) : 0u;
-#pragma unroll
-        for (int i = 0; i < kScanItems; ++i) v[i] = (static_cast<uint32_t>(i) < n_valid) ? __ldg(a.len + base + i) : 0u;
+        return kScanItems;
     }
-    uint32_t t_len = 0, t_cost = 0;
+    const uint32_t n_valid = base < a.G ? min(a.G - base, static_cast<uint32_t>(kScanItems)) : 0u;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) v[i] = (static_cast<uint32_t>(i) < n_valid) ? __ldg(a.len + base + i) : 0u;
+    return n_valid;
+}
+
+__device__ __forceinline__ void thread_sums(const uint32_t (&v)[kScanItems], uint32_t n_valid, uint32_t& t_len, uint32_t& t_cost) {
+    t_len = 0; t_cost = 0;
 #pragma unroll
     for (int i = 0; i < kScanItems; ++i) {
         t_len += v[i];
         t_cost += (static_cast<uint32_t>(i) < n_valid) ? max(v[i], 1u) : 0u;
     }
+}
 
-    // ---- CTA-wide exclusive scan of the per-thread sums ----
-    uint32_t i_len = t_len, i_cost = t_cost;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t ul = __shfl_up_sync(0xffffffffu, i_len, d);
-        const uint32_t uc = __shfl_up_sync(0xffffffffu, i_cost, d);
-        if (lane >= static_cast<uint32_t>(d)) { i_len += ul; i_cost += uc; }
+#ifdef DPI_PLAN_TRACE
+__device__ unsigned long long g_trace[kMaxChunks * 8];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define DPI_TRACE(slot, c) do { if (threadIdx.x == 0) g_trace[(c) * 8 + (slot)] = gtime(); } while (0)
+#else
+#define DPI_TRACE(slot, c) do { } while (0)
+#endif
+
+__global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const PlanArgs a) {
+#ifdef DPI_PLAN_TRACE
+    const unsigned long long t_start = gtime();
+#endif
+    __shared__ uint32_t s_chunk, s_epoch;
+    __shared__ uint32_t s_wlen[2][kScanThreads / 32], s_wcost[2][kScanThreads / 32];
+    __shared__ uint32_t s_pre_len, s_pre_cost;
+
+    // Chunk ids are handed out by a ticket, so a chunk only ever waits on chunks that already run. The epoch that
+    // tags this build's status records lives in device memory and is advanced by the last CTA to finish, so a
+    // build needs no host-side state: the same launch can be replayed from a CUDA graph.
+    if (threadIdx.x == 0) {
+        s_chunk = atomicInc(a.state + kStateTicket, a.num_chunks - 1);  // wraps to 0 after the last chunk
+        s_epoch = *reinterpret_cast<volatile unsigned int*>(a.state + kStateEpoch);
     }
-    if (lane == 31) { s_wlen[warp] = i_len; s_wcost[warp] = i_cost; }
     __syncthreads();
-    uint32_t w_len = 0, w_cost = 0, agg_len = 0, agg_cost = 0;
-#pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) {
-        const uint32_t l = s_wlen[w], c = s_wcost[w];
-        if (static_cast<uint32_t>(w) < warp) { w_len += l; w_cost += c; }
-        agg_len += l; agg_cost += c;
-    }
-    const uint32_t ex_len = w_len + i_len - t_len;     // exclusive prefix of this thread inside the tile
-    const uint32_t ex_cost = w_cost + i_cost - t_cost;
+    const uint32_t chunk = s_chunk;
+    const uint32_t epoch = s_epoch;
+#ifdef DPI_PLAN_TRACE
+    if (threadIdx.x == 0) g_trace[chunk * 8 + 0] = t_start;
+#endif
+    DPI_TRACE(1, chunk);
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t tile_lo = chunk * a.tiles_per_chunk;
+    const uint32_t tile_hi = min(a.num_tiles, tile_lo + a.tiles_per_chunk);
 
-    // ---- decoupled look-back: publish aggregate, fetch predecessor prefix, publish inclusive ----
+    // ---- pass 1: aggregate of the chunk ----
+    uint32_t v[kScanItems];            // lengths of the chunk's FIRST tile stay in registers
+    uint32_t n_valid = load_items(a, tile_lo, v);
+    uint32_t t_len, t_cost;
+    thread_sums(v, n_valid, t_len, t_cost);
+    uint32_t c_len = t_len, c_cost = t_cost;
+    for (uint32_t tile = tile_lo + 1; tile < tile_hi; ++tile) {
+        uint32_t u[kScanItems], ul, uc;
+        const uint32_t nv = load_items(a, tile, u);
+        thread_sums(u, nv, ul, uc);
+        c_len += ul; c_cost += uc;
+    }
+    c_len = warp_sum(c_len);
+    c_cost = warp_sum(c_cost);
+    DPI_TRACE(2, chunk);
+    if (lane == 0) { s_wlen[0][warp] = c_len; s_wcost[0][warp] = c_cost; }
+    __syncthreads();
     if (warp == 0) {
-        if (tile == 0) {
-            if (lane == 0) {
-                st_relaxed_gpu(a.tile_len + 0, pack_status(epoch, kStateInclusive, agg_len));
-                st_relaxed_gpu(a.tile_cost + 0, pack_status(epoch, kStateInclusive, agg_cost));
-                s_pre_len = 0; s_pre_cost = 0;
-            }
-        } else {
-            if (lane == 0) {
-                st_relaxed_gpu(a.tile_len + tile, pack_status(epoch, kStateAggregate, agg_len));
-                st_relaxed_gpu(a.tile_cost + tile, pack_status(epoch, kStateAggregate, agg_cost));
-            }
-            uint32_t pl, pc;
-            lookback(a.tile_len, a.tile_cost, tile, epoch, pl, pc);
-            if (lane == 0) {
-                st_relaxed_gpu(a.tile_len + tile, pack_status(epoch, kStateInclusive, pl + agg_len));
-                st_relaxed_gpu(a.tile_cost + tile, pack_status(epoch, kStateInclusive, pc + agg_cost));
-                s_pre_len = pl; s_pre_cost = pc;
-            }
-        }
+        uint32_t agg_len = 0, agg_cost = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) { agg_len += s_wlen[0][w]; agg_cost += s_wcost[0][w]; }
+        if (lane == 0)
+            st_status(a.status + chunk, pack_status(epoch, kStateAggregate, agg_len), pack_status(epoch, kStateAggregate, agg_cost));
+        DPI_TRACE(3, chunk);
+        uint32_t pl, pc;
+        lookback_all(a.status, chunk, epoch, pl, pc);
+        DPI_TRACE(4, chunk);
+        if (lane == 0) { s_pre_len = pl; s_pre_cost = pc; }
     }
     __syncthreads();
     // Let a dependent (PDL) lookup kernel start its prologue; it still waits for this grid to finish
     // and flush before it reads the plan.
     asm volatile("griddepcontrol.launch_dependents;");
 
-    if (n_valid == 0) return;
-    uint32_t off = s_pre_len + ex_len;    // offsets[base]
-    uint32_t c = s_pre_cost + ex_cost;    // C[base]
-
-    // ---- a1: offsets ----
-    if (n_valid == kScanItems) {
-        int4 o0, o1;
-        uint32_t r = off;
-        o0.x = r; r += v[0]; o0.y = r; r += v[1]; o0.z = r; r += v[2]; o0.w = r; r += v[3];
-        o1.x = r; r += v[4]; o1.y = r; r += v[5]; o1.z = r; r += v[6]; o1.w = r;
-        reinterpret_cast<int4*>(a.offsets + base)[0] = o0;   // offsets is 256-B aligned (cudaMalloc), base % 8 == 0
-        reinterpret_cast<int4*>(a.offsets + base)[1] = o1;
-    } else {
-        uint32_t r = off;
+    // ---- pass 2: scan the chunk tile by tile from its prefix ----
+    uint32_t run_len = s_pre_len, run_cost = s_pre_cost;   // offsets / C at the first bag of the current tile
+    for (uint32_t tile = tile_lo; tile < tile_hi; ++tile) {
+        const int sb = (tile - tile_lo) & 1;               // double-buffered scratch: one barrier per tile
+        uint32_t u[kScanItems];                            // next tile's lengths, requested before this tile is scanned
+        uint32_t nv_next = 0;
+        const bool has_next = tile + 1 < tile_hi;
+        if (has_next) nv_next = load_items(a, tile + 1, u);
+        uint32_t i_len = t_len, i_cost = t_cost;
 #pragma unroll
-        for (int i = 0; i < kScanItems; ++i) {
-            if (static_cast<uint32_t>(i) < n_valid) a.offsets[base + i] = r;
-            r += v[i];
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t ul = __shfl_up_sync(0xffffffffu, i_len, d);
+            const uint32_t uc = __shfl_up_sync(0xffffffffu, i_cost, d);
+            if (lane >= static_cast<uint32_t>(d)) { i_len += ul; i_cost += uc; }
+        }
+        if (lane == 31) { s_wlen[sb][warp] = i_len; s_wcost[sb][warp] = i_cost; }
+        __syncthreads();
+        uint32_t w_len = 0, w_cost = 0, agg_len = 0, agg_cost = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) {
+            const uint32_t l = s_wlen[sb][w], c = s_wcost[sb][w];
+            if (static_cast<uint32_t>(w) < warp) { w_len += l; w_cost += c; }
+            agg_len += l; agg_cost += c;
+        }
+        const uint32_t base = tile * kScanTile + threadIdx.x * kScanItems;
+        const uint32_t off = run_len + w_len + i_len - t_len;     // offsets[base]
+        uint32_t c = run_cost + w_cost + i_cost - t_cost;         // C[base]
+        run_len += agg_len;
+        run_cost += agg_cost;
+        if (n_valid != 0) {
+            // ---- a1: offsets ----
+            if (n_valid == kScanItems) {
+                int4 o0, o1;
+                uint32_t r = off;
+                o0.x = r; r += v[0]; o0.y = r; r += v[1]; o0.z = r; r += v[2]; o0.w = r; r += v[3];
+                o1.x = r; r += v[4]; o1.y = r; r += v[5]; o1.z = r; r += v[6]; o1.w = r;
+                reinterpret_cast<int4*>(a.offsets + base)[0] = o0;   // offsets is 256-B aligned (cudaMalloc), base % 8 == 0
+                reinterpret_cast<int4*>(a.offsets + base)[1] = o1;
+            } else {
+                uint32_t r = off;
+#pragma unroll
+                for (int i = 0; i < kScanItems; ++i) {
+                    if (static_cast<uint32_t>(i) < n_valid) a.offsets[base + i] = r;
+                    r += v[i];
+                }
+            }
+
+            // ---- a2: every quantum boundary s*K inside (C[g], C[g+1]] belongs to bag g -> seg_bag[s] = g+1 ----
+            // One division per thread; after that the next boundary (q+1)*K is carried along (64-bit: it may pass 2^32).
+            if (base == 0) a.seg[0] = make_int2(0, 0);      // s = 0: C[0] = 0 >= 0
+            uint32_t q = c / a.K;                           // boundaries <= C[base] belong to earlier bags
+            unsigned long long next_boundary = static_cast<unsigned long long>(q + 1) * a.K;
+            uint32_t run = off;
+#pragma unroll
+            for (int i = 0; i < kScanItems; ++i) {
+                if (static_cast<uint32_t>(i) < n_valid) {
+                    c += max(v[i], 1u);
+                    run += v[i];                             // offsets[base + i + 1]
+                    while (c >= next_boundary) {
+                        ++q;
+                        if (q < a.seg_cap) a.seg[q] = make_int2(base + i + 1, run);
+                        next_boundary += a.K;
+                    }
+                }
+            }
+
+            // ---- the thread that owns the last bag closes the plan ----
+            if (base + n_valid == a.G) {
+                const uint32_t n_total = run;
+                a.offsets[a.G] = n_total;
+                const uint32_t S = c / a.K + ((c % a.K) ? 1u : 0u);   // ceil(C[G]/K)
+                if ((c % a.K) != 0 && S < a.seg_cap) a.seg[S] = make_int2(a.G, n_total);  // C[G] < S*K: clamped to G
+                a.meta[META_S] = (S < a.seg_cap) ? S : 0;             // an overflowed plan must not drive a lookup
+                a.meta[META_N] = n_total;
+                a.meta[META_C] = c;
+                a.meta[META_OVERFLOW] = (n_total > a.max_indices || S >= a.seg_cap) ? 1 : 0;
+                a.meta[META_K] = a.K;
+                a.meta[META_G] = a.G;
+            }
+        }
+        if (has_next) {
+#pragma unroll
+            for (int i = 0; i < kScanItems; ++i) v[i] = u[i];
+            n_valid = nv_next;
+            thread_sums(v, n_valid, t_len, t_cost);
         }
     }
 
-    // ---- a2: every quantum boundary s*K inside (C[g], C[g+1]] belongs to bag g -> seg_bag[s] = g+1 ----
-    if (base == 0) a.seg[0] = make_int2(0, 0);      // s = 0: C[0] = 0 >= 0
-    uint32_t q_prev = c / a.K;
-    uint32_t run = off;
-#pragma unroll
-    for (int i = 0; i < kScanItems; ++i) {
-        if (static_cast<uint32_t>(i) < n_valid) {
-            c += max(v[i], 1u);
-            run += v[i];                             // offsets[base + i + 1]
-            const uint32_t q = c / a.K;
-            for (uint32_t s = q_prev + 1; s <= q; ++s)
-                if (s < a.seg_cap) a.seg[s] = make_int2(base + i + 1, run);
-            q_prev = q;
-        }
-    }
-
-    // ---- the thread that owns the last bag closes the plan ----
-    if (base + n_valid == a.G) {
-        uint32_t n_total = off;
-#pragma unroll
-        for (int i = 0; i < kScanItems; ++i) n_total += v[i];
-        a.offsets[a.G] = n_total;
-        const uint32_t S = c / a.K + ((c % a.K) ? 1u : 0u);   // ceil(C[G]/K)
-        if ((c % a.K) != 0 && S < a.seg_cap) a.seg[S] = make_int2(a.G, n_total);  // C[G] < S*K: clamped to G
-        a.meta[META_S] = (S < a.seg_cap) ? S : 0;             // an overflowed plan must not drive a lookup
-        a.meta[META_N] = n_total;
-        a.meta[META_C] = c;
-        a.meta[META_OVERFLOW] = (n_total > a.max_indices || S >= a.seg_cap) ? 1 : 0;
-        a.meta[META_K] = a.K;
-        a.meta[META_G] = a.G;
-    }
-
-    // ---- close the epoch: no thread of this CTA reads a status word past the barrier above; the last tile to
-    // get here advances the tag (a later build starts only after this grid has completed) ----
-    if (threadIdx.x == 0 && atomicInc(a.state + kStateDone, a.num_tiles - 1) == a.num_tiles - 1) {
+    DPI_TRACE(5, chunk);
+    // ---- close the epoch: no thread of this CTA reads a status record past the barrier after the look-back; the
+    // last CTA to get here advances the tag (a later build starts only after this grid has completed) ----
+    if (threadIdx.x == 0 && atomicInc(a.state + kStateDone, a.num_chunks - 1) == a.num_chunks - 1) {
         uint32_t next = epoch + 1;
-        if (next >= kEpochLimit) {  // 30-bit tag about to wrap: clear the words once and restart at 1
-            for (uint32_t i = 0; i < a.num_tiles; ++i) { a.tile_len[i] = 0ull; a.tile_cost[i] = 0ull; }
+        if (next >= kEpochLimit) {  // 30-bit tag about to wrap: clear the records once and restart at 1
+            for (uint32_t i = 0; i < a.num_chunks; ++i) a.status[i] = make_ulonglong2(0ull, 0ull);
             next = 1;
         }
         a.state[kStateEpoch] = next;
     }
+    DPI_TRACE(6, chunk);
 }
 
 __global__ void __launch_bounds__(256) check_indices_kernel(const CheckArgs a) {
@@ -254,7 +297,7 @@ __global__ void __launch_bounds__(256) check_indices_kernel(const CheckArgs a) {
 }  // namespace
 
 cudaError_t launch_plan(const PlanArgs& a, cudaStream_t stream) {
-    plan_scan_partition_kernel<<<a.num_tiles, kScanThreads, 0, stream>>>(a);
+    plan_scan_partition_kernel<<<a.num_chunks, kScanThreads, 0, stream>>>(a);
     count_launch();
     return cudaGetLastError();
 }
