@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--mode", type=int, default=0)
     ap.add_argument("--pdl", type=int, default=0)
+    ap.add_argument("--host-chunks", type=int, default=0, help="dpi_forward_host: 0 auto, 1 unpipelined, n chunks")
     ap.add_argument("--kernel", default="output_first", choices=["output_first", "input_first"],
                     help="input_first = the paper's strawman mapping (ablation, PAPER.md:172-176)")
     ap.add_argument("--graph", type=int, default=-1, help="1: time a CUDA-graph replay of the K steps; 0: stream launches; -1: auto (graph for c1-c3)")
@@ -187,6 +188,7 @@ def apply_options(plan, args, binding):
     plan.set_option(binding.OPT_BLOCKS_PER_SM, args.blocks_per_sm)
     plan.set_option(binding.OPT_MODE, args.mode)
     plan.set_option(binding.OPT_PDL, args.pdl)
+    plan.set_option(binding.OPT_HOST_CHUNKS, args.host_chunks)
 
 
 def workload_config(args):

@@ -82,6 +82,8 @@ typedef enum {
     DPI_OPT_ROW_L1_NO_ALLOC = 4,/* reserved: accepts -1 / 0 only. Rows always allocate in L1; the L1::no_allocate
                                    variant measured 17-20 % slower on B200 and was removed */
     DPI_OPT_PDL = 5,            /* 1: lookup is launched with programmatic dependent launch after the planner */
+    DPI_OPT_HOST_CHUNKS = 6,    /* dpi_forward_host only: number of sample chunks pipelined over the copy engines and the
+                                   SMs; 0 = auto (~16 MB of PCIe traffic per chunk, <= 8), 1 = no pipelining, up to 64 */
     DPI_OPT_COUNT_
 } dpi_option_t;
 
@@ -226,7 +228,11 @@ dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int
 /*
  * dpi_forward_host -- the whole path (a1+a2+a3) for callers whose sparse inputs live in HOST memory
  * (the end-to-end number of bench.py): copies lengths and indices host->device into plan-owned staging,
- * builds the plan, runs the lookup and copies the [B, T*D] block back, then synchronises `stream`.
+ * builds the plan, runs the lookup and copies the [B, T*D] block back, then synchronises `stream`. A large batch is
+ * cut into chunks of whole samples (DPI_OPT_HOST_CHUNKS); chunk c goes H2D -> plan -> lookup -> D2H on one of three
+ * internal streams ordered after `stream`, so both PCIe directions and the SMs are busy at once. Each chunk is an
+ * independent sub-batch with its own device plan (bags are independent); the host only adds up how many
+ * index entries each chunk owns, to size the copies. The result is identical to the unchunked call.
  * Tables stay resident on the device (they are the model, not a per-batch input).
  *   lengths_host int32[G]; indices_host int32 / int64 [n_indices] per the plan's index type
  *   (n_indices <= max_indices); out_host [B, sum dims].

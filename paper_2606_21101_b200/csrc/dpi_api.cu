@@ -1,5 +1,6 @@
 // dpi_api.cu -- the C ABI of include/dpi.h. Host-side validation, plan ownership and launches only:
 // every step of the path runs in plan_kernels.cu / lookup_*.cu. No CPU fallback anywhere.
+#include <algorithm>
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
@@ -66,7 +67,7 @@ struct dpi_plan_s {
     int32_t K_user = 0;      // 0 = default
     uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
     uint32_t num_tiles = 0, num_chunks = 0, tiles_per_chunk = 0;
-    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0};
+    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0, 0};
     // device
     int device = 0, num_sms = 0;
     int32_t* offsets = nullptr;
@@ -83,7 +84,18 @@ struct dpi_plan_s {
     void* stage_idx = nullptr;
     size_t stage_idx_bytes = 0;
     void* stage_out = nullptr;
+    struct HostPipeline* pipe = nullptr;   // dpi_forward_host: sample-chunked sub-plans + copy/compute streams
     bool built = false;
+};
+
+// dpi_forward_host cuts a large batch into chunks of whole samples; chunk c runs H2D -> plan -> lookup -> D2H on
+// stream c % 3, so the copy engines (both PCIe directions) and the SMs work on different chunks at the same time.
+struct HostPipeline {
+    static constexpr int kStreams = 3;
+    std::vector<dpi_plan_t*> sub;       // one plan per chunk (B_c samples each)
+    std::vector<int32_t> sample_lo;     // first sample of each chunk (+ B at the end)
+    cudaStream_t st[kStreams] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_in = nullptr, ev_done[kStreams] = {nullptr, nullptr, nullptr};
 };
 
 namespace {
@@ -116,8 +128,11 @@ dpi_status_t ensure_seg_capacity(dpi_plan_t* p, int32_t K) {
     return DPI_OK;
 }
 
+void free_pipeline(dpi_plan_t* p);
+
 void free_plan(dpi_plan_t* p) {
     if (!p) return;
+    free_pipeline(p);
     cudaFree(p->offsets); cudaFree(p->seg); cudaFree(p->meta); cudaFree(p->status);
     cudaFree(p->state); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
     cudaFree(p->tab_nvec_dev); cudaFree(p->tab_col_dev);
@@ -152,6 +167,20 @@ LookupLaunch choose_launch(const dpi_plan_t* p, const LookupArgs& a, bool genera
     if (need < l.grid) l.grid = static_cast<int>(need > 0 ? need : 1);
     l.pdl = p->opt[DPI_OPT_PDL] != 0;
     return l;
+}
+
+void free_pipeline(dpi_plan_t* p) {
+    HostPipeline* h = p->pipe;
+    if (!h) return;
+    for (dpi_plan_t* q : h->sub) free_plan(q);
+    for (int i = 0; i < HostPipeline::kStreams; ++i) {
+        if (h->st[i]) cudaStreamDestroy(h->st[i]);
+        if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
+    }
+    if (h->ev_in) cudaEventDestroy(h->ev_in);
+    (void)cudaGetLastError();
+    delete h;
+    p->pipe = nullptr;
 }
 
 struct LookupCall {
@@ -359,6 +388,7 @@ dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
         case DPI_OPT_MODE: ok = v >= 0 && v <= 3; break;
         case DPI_OPT_ROW_L1_NO_ALLOC: ok = v == -1 || v == 0; break;  // the bypass variant was removed (see dpi.h)
         case DPI_OPT_PDL: ok = v == 0 || v == 1; break;
+        case DPI_OPT_HOST_CHUNKS: ok = v >= 0 && v <= 64; break;
         default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);
     }
     if (!ok) return fail(DPI_ERR_INVALID_ARG, "value %d not supported for option %d", v, (int)opt);
@@ -511,6 +541,46 @@ dpi_status_t dpi_plan_out_width(const dpi_plan_t* p, int64_t* width) {
     return DPI_OK;
 }
 
+namespace {
+
+int host_chunks(const dpi_plan_t* p, size_t bytes_moved) {
+    if (p->bag_order == DPI_BAGS_TABLE_MAJOR) return 1;  // a chunk of samples is not a contiguous run of bags
+    int n = p->opt[DPI_OPT_HOST_CHUNKS];
+    if (n == 0) {  // auto: ~16 MB of PCIe traffic per chunk, at most 8 chunks; small batches stay in one piece
+        n = static_cast<int>(bytes_moved / (16u << 20));
+        if (n > 8) n = 8;
+        if (n < 2) n = 1;
+    }
+    if (n > p->B) n = p->B;
+    return n < 1 ? 1 : n;
+}
+
+dpi_status_t ensure_pipeline(dpi_plan_t* p, int n_chunks) {
+    if (p->pipe && static_cast<int>(p->pipe->sub.size()) == n_chunks) return DPI_OK;
+    free_pipeline(p);
+    HostPipeline* h = new (std::nothrow) HostPipeline();
+    if (!h) return fail(DPI_ERR_ALLOC, "host allocation failed");
+    p->pipe = h;
+    for (int i = 0; i < HostPipeline::kStreams; ++i) {
+        DPI_CUDA(cudaStreamCreateWithFlags(&h->st[i], cudaStreamNonBlocking));
+        DPI_CUDA(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
+    }
+    DPI_CUDA(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
+    const int32_t per = (p->B + n_chunks - 1) / n_chunks;
+    for (int32_t lo = 0; lo < p->B; lo += per) {
+        const int32_t Bc = std::min(per, p->B - lo);
+        dpi_plan_t* q = nullptr;
+        dpi_status_t st = dpi_plan_create(p->T, p->table_rows.data(), p->dims.data(), p->dtype, Bc, p->max_indices, &q);
+        if (st != DPI_OK) return st;
+        h->sub.push_back(q);
+        h->sample_lo.push_back(lo);
+    }
+    h->sample_lo.push_back(p->B);
+    return DPI_OK;
+}
+
+}  // namespace
+
 dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, const int32_t* lengths_host,
                               const void* indices_host, int64_t n_indices, const uint8_t* pooling, void* out_host,
                               void* stream) {
@@ -518,7 +588,8 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     if (n_indices < 0 || n_indices > p->max_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld outside [0, max_indices=%lld]", (long long)n_indices, (long long)p->max_indices);
     if (n_indices > 0 && !indices_host) return fail(DPI_ERR_INVALID_ARG, "indices_host is NULL");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    const size_t out_bytes = static_cast<size_t>(p->B) * p->out_width * out_elt_bytes(p);
+    const size_t oelt = out_elt_bytes(p);
+    const size_t out_bytes = static_cast<size_t>(p->B) * p->out_width * oelt;
     const size_t idx_elt = p->index_type == DPI_IDX_I64 ? 8 : 4;
     const size_t idx_bytes = (static_cast<size_t>(p->max_indices) + 4) * idx_elt;
     if (!p->stage_len) DPI_CUDA(cudaMalloc(&p->stage_len, static_cast<size_t>(p->G) * sizeof(int32_t)));
@@ -529,15 +600,75 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
         p->stage_idx_bytes = idx_bytes;
     }
     if (!p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, static_cast<size_t>(p->B) * p->out_width * 4));
-    DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
-    if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * idx_elt, cudaMemcpyHostToDevice, s));
-    dpi_status_t st = dpi_plan_build(p, p->stage_len, s);
+
+    const int n_chunks = host_chunks(p, static_cast<size_t>(p->G) * 4 + static_cast<size_t>(n_indices) * idx_elt + out_bytes);
+    if (n_chunks <= 1) {
+        DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * idx_elt, cudaMemcpyHostToDevice, s));
+        dpi_status_t st = dpi_plan_build(p, p->stage_len, s);
+        if (st != DPI_OK) return st;
+        LookupCall c;
+        c.tables = table_ptrs_dev; c.indices = p->stage_idx; c.pooling = pooling; c.out = p->stage_out;
+        st = do_lookup(p, c, s);
+        if (st != DPI_OK) return st;
+        DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
+        DPI_CUDA(cudaStreamSynchronize(s));
+        return DPI_OK;
+    }
+
+    // ---- pipelined: chunks of whole samples, each an independent sub-batch with its own device plan ----
+    dpi_status_t st = ensure_pipeline(p, n_chunks);
     if (st != DPI_OK) return st;
-    LookupCall c;
-    c.tables = table_ptrs_dev; c.indices = p->stage_idx; c.pooling = pooling; c.out = p->stage_out;
-    st = do_lookup(p, c, s);
-    if (st != DPI_OK) return st;
-    DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
+    HostPipeline* h = p->pipe;
+    const size_t n_sub = h->sub.size();
+    // Copy sizes only: how many index entries belong to each chunk (the plan itself -- offsets, segments -- is still
+    // computed on the device, per chunk).
+    std::vector<int64_t> entry_lo(n_sub + 1, 0);
+    for (size_t c = 0; c < n_sub; ++c) {
+        const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T, g1 = static_cast<size_t>(h->sample_lo[c + 1]) * p->T;
+        int64_t n = 0;
+        for (size_t g = g0; g < g1; ++g) {
+            if (lengths_host[g] < 0) return fail(DPI_ERR_INVALID_ARG, "lengths_host[%zu] is negative", g);
+            n += lengths_host[g];
+        }
+        entry_lo[c + 1] = entry_lo[c] + n;
+    }
+    if (entry_lo[n_sub] != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)entry_lo[n_sub]);
+
+    DPI_CUDA(cudaEventRecord(h->ev_in, s));
+    for (int i = 0; i < HostPipeline::kStreams; ++i) DPI_CUDA(cudaStreamWaitEvent(h->st[i], h->ev_in, 0));
+    const size_t row_bytes = static_cast<size_t>(p->out_width) * oelt;
+    for (size_t c = 0; c < n_sub; ++c) {
+        cudaStream_t cs = h->st[c % HostPipeline::kStreams];
+        dpi_plan_t* q = h->sub[c];
+        q->out_dtype = p->out_dtype;
+        q->index_type = p->index_type;
+        for (int o = 0; o < DPI_OPT_COUNT_; ++o) q->opt[o] = p->opt[o];
+        if (p->K_user && q->K != p->K_user) {
+            st = dpi_plan_set_quantum(q, p->K_user);
+            if (st != DPI_OK) return st;
+        }
+        const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T;
+        const size_t n_g = static_cast<size_t>(q->G);
+        const int64_t e0 = entry_lo[c], n_e = entry_lo[c + 1] - entry_lo[c];
+        char* idx_dev = static_cast<char*>(p->stage_idx) + static_cast<size_t>(e0) * idx_elt;
+        char* out_dev = static_cast<char*>(p->stage_out) + static_cast<size_t>(h->sample_lo[c]) * row_bytes;
+        DPI_CUDA(cudaMemcpyAsync(p->stage_len + g0, lengths_host + g0, n_g * sizeof(int32_t), cudaMemcpyHostToDevice, cs));
+        if (n_e) DPI_CUDA(cudaMemcpyAsync(idx_dev, static_cast<const char*>(indices_host) + static_cast<size_t>(e0) * idx_elt,
+                                          static_cast<size_t>(n_e) * idx_elt, cudaMemcpyHostToDevice, cs));
+        st = dpi_plan_build(q, p->stage_len + g0, cs);
+        if (st != DPI_OK) return st;
+        LookupCall lc;
+        lc.tables = table_ptrs_dev; lc.indices = idx_dev; lc.pooling = pooling; lc.out = out_dev;
+        st = do_lookup(q, lc, cs);
+        if (st != DPI_OK) return st;
+        DPI_CUDA(cudaMemcpyAsync(static_cast<char*>(out_host) + static_cast<size_t>(h->sample_lo[c]) * row_bytes, out_dev,
+                                 static_cast<size_t>(q->B) * row_bytes, cudaMemcpyDeviceToHost, cs));
+    }
+    for (int i = 0; i < HostPipeline::kStreams; ++i) {
+        DPI_CUDA(cudaEventRecord(h->ev_done[i], h->st[i]));
+        DPI_CUDA(cudaStreamWaitEvent(s, h->ev_done[i], 0));
+    }
     DPI_CUDA(cudaStreamSynchronize(s));
     return DPI_OK;
 }

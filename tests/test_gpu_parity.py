@@ -282,6 +282,18 @@ def test_forward_host_equals_device_path():
     out = torch.empty((cfg.B, cfg.T * cfg.D), dtype=torch.bfloat16).pin_memory()
     plan.forward_host(dt.ptrs, ln, idx, out, pooling=pooling)
     assert np.array_equal(out.double().numpy(), dev)
+    # the pipelined variant (chunks of whole samples over three streams) gives the same block, ragged last chunk included
+    for chunks in (2, 3, 7, 64):
+        plan.set_option(binding.OPT_HOST_CHUNKS, chunks)
+        out.fill_(float("nan"))
+        plan.forward_host(dt.ptrs, ln, idx, out, pooling=pooling)
+        assert np.array_equal(out.double().numpy(), dev), f"{chunks} chunks"
+    # pageable host memory works as well
+    out2 = torch.empty((cfg.B, cfg.T * cfg.D), dtype=torch.bfloat16)
+    plan.forward_host(dt.ptrs, torch.from_numpy(batch.lengths), torch.from_numpy(batch.indices), out2, pooling=pooling)
+    assert np.array_equal(out2.double().numpy(), dev)
+    with pytest.raises(binding.DpiError):  # lengths that do not add up to n_indices are caught before any copy
+        plan.forward_host(dt.ptrs, ln, idx[:-1].clone().pin_memory(), out, pooling=pooling)
     plan.destroy()
 
 
