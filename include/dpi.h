@@ -122,7 +122,18 @@ dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* plan, dpi_dtype_t out_dtype);
  */
 dpi_status_t dpi_plan_set_layout(dpi_plan_t* plan, dpi_bag_order_t order, dpi_index_type_t index_type);
 
-/* Elements per output row = sum of dims (T*D when every table has the same D). */
+/*
+ * dpi_plan_set_columns -- place table t's block at column columns[t] (in elements) of the output row instead of the
+ * running prefix of dims. columns: host int64[T], each columns[t]*sizeof(dtype) a multiple of 16 B; blocks must not
+ * overlap (not checked); NULL restores the default. The row width becomes max_t(columns[t] + dims[t]). This is what a
+ * rank of a table-sharded model uses to write ITS tables into the global [B, sum of all dims] row.
+ * Synchronous (one small host->device copy); call it before dpi_lookup*, not between a build and its lookup on
+ * another thread.
+ */
+dpi_status_t dpi_plan_set_columns(dpi_plan_t* plan, const int64_t* columns);
+
+/* Elements per output row = sum of dims (T*D when every table has the same D), or the span set by
+ * dpi_plan_set_columns. */
 dpi_status_t dpi_plan_out_width(const dpi_plan_t* plan, int64_t* width);
 
 /* Cost quantum K >= 1 of the balanced segments (0 = library default for this row size). Takes effect at the
@@ -196,6 +207,15 @@ dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indice
  *                one rank's column block of a table-sharded model). The pitch in bytes must keep rows 16-byte
  *                aligned (32-byte for fp32 output of 16-bit tables), else DPI_ERR_INVALID_ARG.
  *   indices_dev  int32 or int64 per the plan's index type; the other fields as in dpi_lookup.
+ *   out_peers_dev / n_peers / rows_per_peer
+ *                fused lookup + all-to-all for table-wise sharding: when out_peers_dev is
+ *                not NULL it is a device array of n_peers output base pointers -- peer-mapped memory of the other
+ *                GPUs (CUDA IPC / symmetric memory) or plain local buffers -- and sample b is stored to
+ *                out_peers_dev[b / rows_per_peer] at row b % rows_per_peer (same pitch and columns), i.e. every
+ *                rank writes its tables' column blocks straight into the batch shard of the rank that owns the
+ *                sample, over NVLink, from the same kernel that pools them: no send buffer and no separate
+ *                collective. out_dev is then ignored. n_peers*rows_per_peer must cover B. The caller orders
+ *                consumers after ALL ranks' kernels (e.g. a barrier on the stream).
  *   flags        DPI_LOOKUP_FORCE_GENERAL runs the general kernel even when the call needs none of the variants
  *                (used by the parity tests to compare the two instantiations).
  * Set struct_size = sizeof(dpi_lookup_args_t); a mismatch -> DPI_ERR_INVALID_ARG. Unused fields must be zero.
@@ -211,6 +231,9 @@ typedef struct dpi_lookup_args_s {
     const uint8_t* pooling; /* host[T] or NULL */
     void* out_dev;
     int64_t out_ld;
+    const void* const* out_peers_dev; /* NULL, or device array of n_peers output base pointers */
+    int32_t n_peers;
+    int32_t rows_per_peer;
 } dpi_lookup_args_t;
 dpi_status_t dpi_lookup_ex(const dpi_lookup_args_t* args, const dpi_plan_t* plan, void* stream);
 

@@ -25,7 +25,7 @@ IDX_I32, IDX_I64 = 0, 1
 LOOKUP_FORCE_GENERAL = 1
 
 # every symbol include/dpi.h declares (tests check the .so exports each one)
-EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "dpi_plan_out_width", "dpi_lookup_ex",
+EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "dpi_plan_set_columns", "dpi_plan_out_width", "dpi_lookup_ex",
            "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
            "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export",
            "dpi_lookup", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
@@ -36,7 +36,8 @@ class LookupArgs(ctypes.Structure):
     """dpi_lookup_args_t of include/dpi.h."""
     _fields_ = [("struct_size", ctypes.c_uint32), ("flags", ctypes.c_uint32), ("table_ptrs_dev", ctypes.c_void_p),
                 ("indices_dev", ctypes.c_void_p), ("offsets_dev", ctypes.c_void_p), ("weights_dev", ctypes.c_void_p),
-                ("pooling", ctypes.c_void_p), ("out_dev", ctypes.c_void_p), ("out_ld", ctypes.c_int64)]
+                ("pooling", ctypes.c_void_p), ("out_dev", ctypes.c_void_p), ("out_ld", ctypes.c_int64),
+                ("out_peers_dev", ctypes.c_void_p), ("n_peers", ctypes.c_int32), ("rows_per_peer", ctypes.c_int32)]
 
 
 class DpiLibraryMissing(RuntimeError):
@@ -69,6 +70,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
         "dpi_plan_set_out_dtype": (st, [vp, ctypes.c_int]),
         "dpi_plan_set_layout": (st, [vp, ctypes.c_int, ctypes.c_int]),
         "dpi_plan_out_width": (st, [vp, vp]),
+        "dpi_plan_set_columns": (st, [vp, vp]),
         "dpi_lookup_ex": (st, [vp, vp, vp]),
         "dpi_plan_set_quantum": (st, [vp, i32]),
         "dpi_plan_set_option": (st, [vp, ctypes.c_int, i32]),
@@ -170,6 +172,11 @@ class Plan:
     def set_layout(self, bag_order: int = BAGS_SAMPLE_MAJOR, index_type: int = IDX_I32):
         _check(self._lib.dpi_plan_set_layout(self._h, int(bag_order), int(index_type)))
 
+    def set_columns(self, columns=None):
+        cols = None if columns is None else np.ascontiguousarray(columns, dtype=np.int64)
+        _check(self._lib.dpi_plan_set_columns(self._h, _ptr(cols)))
+        self.out_width = self.plan_out_width()
+
     def plan_out_width(self) -> int:
         w = ctypes.c_int64()
         _check(self._lib.dpi_plan_out_width(self._h, ctypes.byref(w)))
@@ -227,10 +234,11 @@ class Plan:
 
     # -- dpi_lookup_ex ----------------------------------------------------------------------------------------
     def lookup_ex(self, table_ptrs_dev, indices_dev, out_dev, pooling=None, offsets_dev=None, weights_dev=None,
-                  out_ld: int = 0, flags: int = 0, stream=None):
+                  out_ld: int = 0, flags: int = 0, out_peers_dev=None, n_peers: int = 0, rows_per_peer: int = 0, stream=None):
         pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
         a = LookupArgs(ctypes.sizeof(LookupArgs), int(flags), _ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(offsets_dev),
-                       _ptr(weights_dev), _ptr(pool), _ptr(out_dev), int(out_ld))
+                       _ptr(weights_dev), _ptr(pool), _ptr(out_dev), int(out_ld), _ptr(out_peers_dev), int(n_peers),
+                       int(rows_per_peer))
         _check(self._lib.dpi_lookup_ex(ctypes.byref(a), self._h, _stream_handle(stream)))
 
     # -- dpi_lookup_input_first (ablation) ---------------------------------------------------

@@ -52,6 +52,7 @@ struct dpi_plan_s {
     int32_t T = 0, B = 0, D = 0;   // D = the widest table's dim
     int64_t out_width = 0;         // sum of dims = elements per output row
     bool mixed_dims = false;
+    bool custom_columns = false;   // dpi_plan_set_columns: tables placed at caller-given columns
     std::vector<int32_t> dims;
     dpi_bag_order_t bag_order = DPI_BAGS_SAMPLE_MAJOR;
     dpi_index_type_t index_type = DPI_IDX_I32;
@@ -191,6 +192,9 @@ struct LookupCall {
     const uint8_t* pooling = nullptr;
     void* out = nullptr;
     int64_t out_ld = 0;     // elements; 0 = dense
+    const void* const* peers = nullptr;   // device [n_peers] output base pointers
+    int32_t n_peers = 0;
+    int32_t rows_per_peer = 0;
     bool force_general = false;
 };
 
@@ -229,7 +233,14 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
             }
         }
     }
-    const bool general = c.force_general || p->mixed_dims || a.idx_shift || a.table_major || c.weights || ld != p->out_width;
+    if (c.peers) {
+        if (c.n_peers < 1 || c.rows_per_peer < 1) return fail(DPI_ERR_INVALID_ARG, "n_peers=%d, rows_per_peer=%d", c.n_peers, c.rows_per_peer);
+        if (static_cast<int64_t>(c.n_peers) * c.rows_per_peer < p->B) return fail(DPI_ERR_INVALID_ARG, "n_peers*rows_per_peer=%lld does not cover B=%d", (long long)c.n_peers * c.rows_per_peer, p->B);
+        a.peer_out = c.peers;
+        a.rows_per_peer = static_cast<uint32_t>(c.rows_per_peer);
+    }
+    const bool general = c.force_general || p->mixed_dims || p->custom_columns || a.idx_shift || a.table_major || c.weights ||
+                         c.peers || ld != p->out_width;
     if (input_first) {
         if (general) return fail(DPI_ERR_UNSUPPORTED, "the input-first ablation kernel only takes the dense int32 sample-major layout");
         cudaError_t e = launch_input_first(a, static_cast<uint32_t>(p->B), p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, stream);
@@ -506,13 +517,15 @@ dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indice
 dpi_status_t dpi_lookup_ex(const dpi_lookup_args_t* args, const dpi_plan_t* p, void* stream) {
     if (!args) return fail(DPI_ERR_INVALID_ARG, "args is NULL");
     if (args->struct_size != sizeof(dpi_lookup_args_t)) return fail(DPI_ERR_INVALID_ARG, "args->struct_size=%u, expected %zu", args->struct_size, sizeof(dpi_lookup_args_t));
-    dpi_status_t st = check_lookup_pointers(p, args->table_ptrs_dev, args->indices_dev, args->out_dev);
+    dpi_status_t st = check_lookup_pointers(p, args->table_ptrs_dev, args->indices_dev,
+                                            args->out_peers_dev ? static_cast<const void*>(args->out_peers_dev) : args->out_dev);
     if (st != DPI_OK) return st;
     if (reinterpret_cast<uintptr_t>(args->weights_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "weights_dev is not 4-byte aligned");
     if (args->out_ld < 0) return fail(DPI_ERR_INVALID_ARG, "out_ld=%lld", (long long)args->out_ld);
     LookupCall c;
     c.tables = args->table_ptrs_dev; c.indices = args->indices_dev; c.offsets = args->offsets_dev;
     c.weights = args->weights_dev; c.pooling = args->pooling; c.out = args->out_dev; c.out_ld = args->out_ld;
+    c.peers = args->out_peers_dev; c.n_peers = args->n_peers; c.rows_per_peer = args->rows_per_peer;
     c.force_general = (args->flags & DPI_LOOKUP_FORCE_GENERAL) != 0;
     return do_lookup(p, c, static_cast<cudaStream_t>(stream));
 }
@@ -532,6 +545,34 @@ dpi_status_t dpi_plan_set_layout(dpi_plan_t* p, dpi_bag_order_t order, dpi_index
     if (index_type != DPI_IDX_I32 && index_type != DPI_IDX_I64) return fail(DPI_ERR_INVALID_ARG, "unknown index type %d", (int)index_type);
     p->bag_order = order;
     p->index_type = index_type;
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_set_columns(dpi_plan_t* p, const int64_t* columns) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    const int elt = p->dtype == DPI_F32 ? 4 : 2;
+    std::vector<uint32_t> col(p->T);
+    int64_t width = 0;
+    if (columns) {
+        for (int t = 0; t < p->T; ++t) {
+            if (columns[t] < 0 || (columns[t] * elt) % 16 != 0) return fail(DPI_ERR_INVALID_ARG, "columns[%d]=%lld must be >= 0 and 16-byte aligned", t, (long long)columns[t]);
+            if (columns[t] * elt / 16 > 0x7fffffffll) return fail(DPI_ERR_INVALID_ARG, "columns[%d] too large", t);
+            col[t] = static_cast<uint32_t>(columns[t] * elt / 16);
+            width = std::max<int64_t>(width, columns[t] + p->dims[t]);
+        }
+    } else {
+        uint32_t c = 0;
+        for (int t = 0; t < p->T; ++t) {
+            col[t] = c;
+            c += static_cast<uint32_t>(static_cast<int64_t>(p->dims[t]) * elt / 16);
+            width += p->dims[t];
+        }
+    }
+    DPI_CUDA(cudaMemcpy(p->tab_col_dev, col.data(), p->T * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    p->custom_columns = columns != nullptr;
+    p->out_width = width;
+    if (p->stage_out) { DPI_CUDA(cudaFree(p->stage_out)); p->stage_out = nullptr; }
+    free_pipeline(p);
     return DPI_OK;
 }
 

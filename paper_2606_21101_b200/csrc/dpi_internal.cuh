@@ -80,6 +80,8 @@ struct LookupArgs {
     const float* __restrict__ weights;       // NULL or fp32[N]: one weight per index entry
     const uint32_t* __restrict__ tab_nvec;   // device [T] vectors per row of each table
     const uint32_t* __restrict__ tab_col;    // device [T] first output vector of each table's column block
+    const void* const* __restrict__ peer_out; // NULL, or device [n_peers] output base pointers (peer-mapped memory)
+    uint32_t rows_per_peer;                  // samples per peer when peer_out is set
     uint64_t out_pitch;                      // bytes between consecutive output rows
     uint32_t B;
     uint32_t idx_shift;                      // 0: int32 ids, 1: int64 ids (indices then points at the low words)

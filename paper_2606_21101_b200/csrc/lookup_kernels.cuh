@@ -247,7 +247,13 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
             r.tab = ti.base + sl * 16;
             r.row_bytes = ti.nvec * 16;
             r.ok = static_cast<uint32_t>(sl) < ti.nvec;
-            r.outp = out + static_cast<size_t>(b) * a.out_pitch + static_cast<size_t>(ti.col_vec) * kOutVec + sl * kOutVec;
+            char* row0 = out;
+            if (a.peer_out) {  // fused all-to-all: sample b lives on peer b / rows_per_peer (NEXT-3)
+                const uint32_t pr = b / a.rows_per_peer;
+                b -= pr * a.rows_per_peer;
+                row0 = reinterpret_cast<char*>(__ldg(reinterpret_cast<const unsigned long long*>(a.peer_out) + pr));
+            }
+            r.outp = row0 + static_cast<size_t>(b) * a.out_pitch + static_cast<size_t>(ti.col_vec) * kOutVec + sl * kOutVec;
         } else {
             r.t = g % a.T;
             r.tab = s_tab[r.t] + sl * 16;

@@ -176,3 +176,68 @@ def test_variant_argument_validation():
         plan.lookup_input_first(ptrs, idx, out)
     assert e.value.status == 2
     plan.destroy()
+
+
+# --------------------------------------------------------------------------------------------------
+# NEXT-3: table-wise sharding with the all-to-all fused into the lookup's store (dpi_lookup_ex out_peers_dev)
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("world", [1, 2, 3])
+@pytest.mark.parametrize("dtype,out", [("f32", None), ("bf16", "f32"), ("f16", None)])
+def test_table_wise_shards_scatter_into_peer_batch_shards(world, dtype, out):
+    """`world` table shards take turns on this one GPU (no kernel waits on another: each is an ordinary launch); the
+    "peers" are `world` separate device buffers, one batch shard each. Every shard's kernel stores its tables' column
+    blocks into the buffer that owns the sample; afterwards the stacked buffers must be the oracle's global block."""
+    from paper_2606_21101_b200 import sharding
+    out = out or dtype
+    dims = [16, 8, 32, 8, 16, 64, 8] if dtype == "f32" else [16, 8, 32, 8, 16, 64, 24]
+    T, B = len(dims), 203
+    rows = [50, 7, 400, 90, 3, 1000, 12]
+    cfg = W.Config("tw", T, tuple(rows), max(dims), dtype, B, ("poisson", 5.0, 30, 0.1), ("zipf", 1.1), "sum", seed=6)
+    glob = W.make_batch(cfg, np.asarray(rows, np.int64), 9)
+    host_tables = W.mixed_dim_tables(cfg.seed, dims, rows, dtype)
+    pooling = np.array([0, 1, 0, 1, 0, 1, 0], np.uint8)
+    ref = oracle.lookup_general(host_tables, W.DTYPE_CODE[dtype], B, glob.indices, host_offsets(glob.lengths).astype(np.int64), pooling)
+
+    width = int(sum(dims))
+    rows_per_rank = -(-B // world)
+    shards = [torch.full((rows_per_rank, width), float("nan"), dtype=TORCH_OUT[out], device="cuda") for _ in range(world)]
+    peers = torch.tensor([s.data_ptr() for s in shards], dtype=torch.int64, device="cuda")
+    cols = sharding.table_columns(dims)
+    parts = sharding.partition_tables(np.asarray(dims, float), world)
+    keep = []
+    for mine in parts:
+        if not mine:
+            continue
+        local = sharding.table_shard_batch(glob, T, mine)
+        tables, ptrs = harness.tables_from_host_mixed([host_tables[t] for t in mine], dtype)
+        plan = binding.Plan([rows[t] for t in mine], np.asarray([dims[t] for t in mine], np.int32), W.DTYPE_CODE[dtype], B,
+                            max(local.N, 1))
+        if out != dtype:
+            plan.set_out_dtype(W.DTYPE_CODE[out])
+        plan.set_columns(cols[mine])
+        ln = torch.from_numpy(local.lengths).cuda()
+        idx = torch.from_numpy(local.indices if local.N else np.zeros(1, np.int32)).cuda()
+        plan.build(ln)
+        plan.lookup_ex(ptrs, idx, None, pooling=pooling[mine], out_ld=width, out_peers_dev=peers, n_peers=world,
+                       rows_per_peer=rows_per_rank)
+        keep.append((plan, tables, ln, idx))
+    torch.cuda.synchronize()
+    got = torch.cat(shards, dim=0)[:B]
+    L_bt = glob.lengths.reshape(B, T)
+    assert_outputs_match_general(harness.out_to_f64(got), ref, L_bt, dims, dtype, out)
+    for plan, *_ in keep:
+        plan.destroy()
+
+
+def test_set_columns_validation_and_reset():
+    plan = binding.Plan([10, 10], np.asarray([16, 8], np.int32), 0, 4, 8)
+    assert plan.plan_out_width() == 24
+    plan.set_columns([32, 0])
+    assert plan.plan_out_width() == 48
+    with pytest.raises(binding.DpiError):
+        plan.set_columns([2, 0])       # 8-byte aligned column
+    with pytest.raises(binding.DpiError):
+        plan.set_columns([-4, 0])
+    plan.set_columns(None)
+    assert plan.plan_out_width() == 24
+    plan.destroy()

@@ -89,3 +89,89 @@ def test_world2_gloo_batch_sharded_replicas(B_global):
     assert t_max == 11.0                       # the slower rank's time, seen by every rank
     assert ranges == [sharding.shard_range(B_global, r, 2) for r in range(2)]
     assert sharding.job_throughput(100, 4, 2, 8.0) == 100 * 4 * 2 / 8e-3
+
+
+# --------------------------------------------------------------------------------------------------
+# table-wise sharding + fused all-to-all: host logic
+# --------------------------------------------------------------------------------------------------
+def test_partition_tables_is_a_balanced_partition():
+    rng = np.random.default_rng(0)
+    for T, world in ((1, 1), (5, 2), (26, 4), (100, 8), (3, 8)):
+        cost = rng.uniform(1, 100, size=T)
+        parts = sharding.partition_tables(cost, world)
+        assert len(parts) == world and sorted(sum(parts, [])) == list(range(T))
+        assert all(p == sorted(p) for p in parts)
+        loads = np.array([cost[p].sum() for p in parts])
+        assert loads.max() - loads.min() <= cost.max() + 1e-9   # LPT: no rank exceeds another by more than one table
+    assert sharding.partition_tables([5, 1, 1, 1, 4, 3], 2) == [[0, 1, 2, 3], [4, 5]]
+    assert list(sharding.table_columns([4, 8, 16])) == [0, 4, 12]
+
+
+def test_table_shard_batch_selects_whole_bags_in_order():
+    cfg = CFG.scaled(B=11)
+    rows = cfg.table_rows()
+    glob = W.make_batch(cfg, rows, 3)
+    off = host_offsets(glob.lengths)
+    for tabs in ([0], [1, 2], [0, 2], [0, 1, 2]):
+        sub = sharding.table_shard_batch(glob, cfg.T, tabs)
+        want_len, want_idx = [], []
+        for b in range(cfg.B):
+            for t in tabs:
+                g = b * cfg.T + t
+                want_len.append(glob.lengths[g])
+                want_idx.extend(glob.indices[off[g]:off[g + 1]])
+        assert np.array_equal(sub.lengths, np.array(want_len, np.int32))
+        assert np.array_equal(sub.indices, np.array(want_idx, np.int32).reshape(-1))
+
+
+def _table_worker(rank, world, port, B_global, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        dims = [16, 8, 32, 8, 16]
+        T = len(dims)
+        cfg = W.Config("tw", T, (50, 7, 400, 90, 3), 32, "f32", B_global, ("uniform", 0, 5), ("zipf", 1.1), "sum", seed=4)
+        rows = cfg.table_rows()
+        tables = W.mixed_dim_tables(cfg.seed, dims, rows, "f32")
+        glob = W.make_batch(cfg, rows, 9)
+        pooling = np.array([0, 1, 0, 1, 0], np.uint8)
+        mine = sharding.partition_tables(np.asarray(dims) * 2.5, world)[rank]
+        cols = sharding.table_columns(dims)
+        local = sharding.table_shard_batch(glob, T, mine)
+        # this rank's column blocks for EVERY sample of the global batch (the oracle stands in for the kernel)
+        blk = oracle.lookup_general([tables[t] for t in mine], oracle.F32, B_global, local.indices,
+                                    host_offsets(local.lengths).astype(np.int64), pooling[mine])
+        # the exchange the fused kernel performs by storing to peer memory: sample b -> rank b // rows_per_rank at the
+        # tables' global columns. Here: gather everybody's blocks and let each rank assemble its own batch shard.
+        rows_per_rank = -(-B_global // world)
+        got = [None] * world
+        dist.all_gather_object(got, (mine, blk))
+        lo, hi = rank * rows_per_rank, min(B_global, (rank + 1) * rows_per_rank)
+        shard = np.full((hi - lo, sum(dims)), np.nan)
+        for tabs, b in got:
+            c = 0
+            for t in tabs:
+                shard[:, cols[t]:cols[t] + dims[t]] = b[lo:hi, c:c + dims[t]]
+                c += dims[t]
+        ref = oracle.lookup_general(tables, oracle.F32, B_global, glob.indices, host_offsets(glob.lengths).astype(np.int64), pooling)
+        ok = bool(np.array_equal(shard, ref[lo:hi]))
+        oks = [None] * world
+        dist.all_gather_object(oks, ok)
+        if rank == 0:
+            q.put(all(oks))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("B_global", [37, 64])
+def test_world2_gloo_table_wise_sharding_assembles_the_global_block(B_global):
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_table_worker, args=(r, 2, port, B_global, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(120)
+        assert p.exitcode == 0
+    assert q.get(timeout=10)
