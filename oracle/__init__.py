@@ -16,6 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "dpi_oracle.c")
+_SRC_NONGEMM = os.path.join(_HERE, "nongemm_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -33,10 +34,11 @@ class OracleError(RuntimeError):
 def build(force: bool = False) -> str:
     """Compile dpi_oracle.c -> liboracle.so with gcc (-O2, no fast-math, no FMA contraction)."""
     with _lock:
-        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_NONGEMM))
+        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
             tmp = _LIB + f".tmp{os.getpid()}"
             subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared",
-                                   "-Wall", "-Wextra", "-o", tmp, _SRC])
+                                   "-Wall", "-Wextra", "-o", tmp, _SRC, _SRC_NONGEMM, "-lm"])
             os.replace(tmp, _LIB)
     return _LIB
 
@@ -58,6 +60,14 @@ def _load():
         lib.oracle_decode_f16.restype = ctypes.c_double
         lib.oracle_decode_bf16.argtypes = [ctypes.c_uint16]
         lib.oracle_decode_bf16.restype = ctypes.c_double
+        lib.oracle_fm_pairwise.argtypes = [i32, i32, i32, vp, i64, vp, vp]
+        lib.oracle_fm_pairwise.restype = ctypes.c_int
+        lib.oracle_cross_combine.argtypes = [i32, i32, vp, vp, vp, vp, vp]
+        lib.oracle_cross_combine.restype = ctypes.c_int
+        lib.oracle_bias_act.argtypes = [i32, i32, vp, vp, ctypes.c_int, vp]
+        lib.oracle_bias_act.restype = ctypes.c_int
+        lib.oracle_bfs_queue.argtypes = [i32, i32, vp, vp]
+        lib.oracle_bfs_queue.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -175,3 +185,64 @@ def decode_f16(bits: int) -> float:
 
 def decode_bf16(bits: int) -> float:
     return float(_load().oracle_decode_bf16(int(bits)))
+
+
+# ---- non-GEMM consumers of X_embed and Algorithm 2 (nongemm_oracle.c) -----------------------
+ACT_IDENTITY, ACT_RELU, ACT_SIGMOID = 0, 1, 2
+MODULE_EXPLICIT, MODULE_IMPLICIT = 0, 1
+
+
+def _f64_2d(a) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if a.ndim != 2:
+        raise ValueError("expected a [B, F] matrix")
+    return a
+
+
+def fm_pairwise(x: np.ndarray, T: int, D: int):
+    """FM second-order term by its definition (DESIGN.md 11.4 N1). x float64[B, >= T*D] ->
+    (y float64[B], v float64[B, D]) with v[b,c] = sum_{t<u} x[b,t,c] x[b,u,c] and y = v.sum(1)."""
+    x = _f64_2d(x)
+    B, ld = x.shape
+    y = np.empty(B, dtype=np.float64)
+    v = np.empty((B, D), dtype=np.float64)
+    _check(_load().oracle_fm_pairwise(B, T, D, x.ctypes.data, ld, y.ctypes.data, v.ctypes.data))
+    return y, v
+
+
+def cross_combine(x0, xl, u, bias=None) -> np.ndarray:
+    """DCNv2 cross layer, non-GEMM part (DESIGN.md 11.4 N2): x0 * (u + bias) + xl, float64[B, F]."""
+    x0, xl, u = _f64_2d(x0), _f64_2d(xl), _f64_2d(u)
+    if not (x0.shape == xl.shape == u.shape):
+        raise ValueError("shape mismatch")
+    B, F = x0.shape
+    bias = None if bias is None else np.ascontiguousarray(bias, dtype=np.float64)
+    if bias is not None and bias.shape != (F,):
+        raise ValueError("bias must be [F]")
+    out = np.empty((B, F), dtype=np.float64)
+    _check(_load().oracle_cross_combine(B, F, x0.ctypes.data, xl.ctypes.data, u.ctypes.data,
+                                        None if bias is None else bias.ctypes.data, out.ctypes.data))
+    return out
+
+
+def bias_act(u, bias=None, act: int = ACT_RELU) -> np.ndarray:
+    """MLP layer, non-GEMM part (DESIGN.md 11.4 N3): act(u + bias), float64[B, F]."""
+    u = _f64_2d(u)
+    B, F = u.shape
+    bias = None if bias is None else np.ascontiguousarray(bias, dtype=np.float64)
+    if bias is not None and bias.shape != (F,):
+        raise ValueError("bias must be [F]")
+    out = np.empty((B, F), dtype=np.float64)
+    _check(_load().oracle_bias_act(B, F, u.ctypes.data, None if bias is None else bias.ctypes.data, int(act),
+                                   out.ctypes.data))
+    return out
+
+
+def bfs_queue(n_explicit: int, n_implicit: int):
+    """Algorithm 2: launch queue as a list of (module, op index), module 0 = explicit,
+    1 = implicit."""
+    n = int(n_explicit) + int(n_implicit)
+    qm = np.empty(max(n, 1), dtype=np.int32)
+    qo = np.empty(max(n, 1), dtype=np.int32)
+    _check(_load().oracle_bfs_queue(int(n_explicit), int(n_implicit), qm.ctypes.data, qo.ctypes.data))
+    return [(int(qm[i]), int(qo[i])) for i in range(n)]
