@@ -43,6 +43,14 @@ int pow2ceil(int x) {
 
 void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
+dpi_status_t report_error(dpi_status_t st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return st;
+}
+
 }  // namespace dpi
 
 using namespace dpi;

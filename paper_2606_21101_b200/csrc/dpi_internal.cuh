@@ -113,4 +113,14 @@ cudaError_t launch_input_first(const LookupArgs& a, uint32_t B, int dtype, bool 
 
 void count_launch();
 
+// ---- NEXT-4: non-GEMM consumers of X_embed (nongemm_kernels.cu; boundary in include/dpi_nongemm.h) ---------
+cudaError_t launch_fm(const void* x, int dtype, uint32_t B, uint32_t T, uint32_t D, uint64_t x_pitch_bytes, float* y,
+                      float* v, cudaStream_t st);
+cudaError_t launch_cross_combine(const void* x0, const void* xl, const void* u, const float* bias, void* out, int dtype,
+                                 uint32_t B, uint32_t F, cudaStream_t st);
+cudaError_t launch_bias_act(const void* u, const float* bias, void* out, int dtype, uint32_t B, uint32_t F, int act,
+                            cudaStream_t st);
+// error text of the calling thread (dpi_last_error); defined in dpi_api.cu
+dpi_status_t report_error(dpi_status_t st, const char* fmt, ...);
+
 }  // namespace dpi

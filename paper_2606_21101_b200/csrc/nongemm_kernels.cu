@@ -1,0 +1,353 @@
+// nongemm_kernels.cu -- SURVEY.md 8(f) NEXT-4: the fused non-GEMM operators that consume X_embed
+// ("we combine all neighbouring non-GEMM operators into a single operator ... traverse the output
+// matrix element by element ... data reads and writes are contiguous in memory").  Boundary: include/dpi_nongemm.h.
+//
+//   fm_kernel            DeepFM FM second-order term: square, reduce-sum over fields, subtract, halve, reduce-sum over
+//                        the embedding dim -- five framework operators, one pass over X_embed, one warp per sample.
+//   cross_combine_kernel DCNv2 cross layer minus its GEMM: out = x0 * (u + bias) + xl.
+//   bias_act_kernel      MLP layer minus its GEMM: out = act(u + bias).
+// All three are streaming, HBM/L2-bound: 128-bit coalesced loads, fp32 arithmetic, one RNE cast at the store. No
+// tensor cores (no contraction here; the GEMMs between these operators are the caller's cuBLAS calls).
+#include <algorithm>
+
+#include "dpi_internal.cuh"
+#include "../../include/dpi_nongemm.h"
+
+namespace dpi {
+namespace {
+
+// ---- 16-byte vector <-> fp32 lanes -----------------------------------------------------------------------------
+template <int DT> struct Elt;
+template <> struct Elt<DPI_F32> {
+    static constexpr int kPerVec = 4;
+    __device__ static __forceinline__ void unpack(const uint4& v, float (&f)[4]) {
+        f[0] = __uint_as_float(v.x); f[1] = __uint_as_float(v.y); f[2] = __uint_as_float(v.z); f[3] = __uint_as_float(v.w);
+    }
+    __device__ static __forceinline__ uint4 pack(const float (&f)[4]) {
+        return make_uint4(__float_as_uint(f[0]), __float_as_uint(f[1]), __float_as_uint(f[2]), __float_as_uint(f[3]));
+    }
+};
+template <> struct Elt<DPI_F16> {
+    static constexpr int kPerVec = 8;
+    __device__ static __forceinline__ void unpack(const uint4& v, float (&f)[8]) {
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float2 p = __half22float2(*reinterpret_cast<const __half2*>(&w[i]));
+            f[2 * i] = p.x; f[2 * i + 1] = p.y;
+        }
+    }
+    __device__ static __forceinline__ uint4 pack(const float (&f)[8]) {
+        uint32_t w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const __half2 h = __floats2half2_rn(f[2 * i], f[2 * i + 1]);
+            w[i] = *reinterpret_cast<const uint32_t*>(&h);
+        }
+        return make_uint4(w[0], w[1], w[2], w[3]);
+    }
+};
+template <> struct Elt<DPI_BF16> {
+    static constexpr int kPerVec = 8;
+    __device__ static __forceinline__ void unpack(const uint4& v, float (&f)[8]) {
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            f[2 * i] = __uint_as_float(w[i] << 16);
+            f[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+        }
+    }
+    __device__ static __forceinline__ uint4 pack(const float (&f)[8]) {
+        uint32_t w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const __nv_bfloat162 h = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);
+            w[i] = *reinterpret_cast<const uint32_t*>(&h);
+        }
+        return make_uint4(w[0], w[1], w[2], w[3]);
+    }
+};
+
+// read once: do not keep it in L1. Coherent (no .nc) because the element-wise operators may run in place.
+__device__ __forceinline__ uint4 ld_stream16(const void* p, bool pred) {
+    uint4 r = make_uint4(0u, 0u, 0u, 0u);
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+        "@p ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];\n\t}"
+        : "+r"(r.x), "+r"(r.y), "+r"(r.z), "+r"(r.w) : "l"(p), "r"(static_cast<int>(pred)) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_stream16(void* p, const uint4& v) {
+    asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// ---- FM second-order term ---------------------------------------------------------------------------------------
+// Same lane mapping as the lookup: a field's D elements are NV 16-byte vectors, W = pow2ceil(NV) lanes hold one field
+// (lane sl < NV loads vector sl), the P = 32/W sub-warps of a warp walk fields sub, sub+P, ... of ONE sample, so a
+// warp-wide load covers P consecutive fields = a contiguous piece of the sample's row (output-first: the threads of a
+// warp share a sample). Each lane keeps sum and sum-of-squares of its columns over its fields; the
+// sub-warps are combined with log2(P) xor-shuffle steps; sub-warp 0 forms 1/2 (s^2 - q) per column, stores v and
+// reduces over the columns for y.
+struct FmArgs {
+    const char* x;
+    float* y;
+    float* v;
+    uint64_t x_pitch;  // bytes between rows
+    uint32_t B, T, D, nvec;
+};
+
+template <int DT, int W, int U>
+__global__ void __launch_bounds__(256) fm_kernel(const FmArgs a) {
+    constexpr int P = 32 / W;
+    constexpr int E = Elt<DT>::kPerVec;
+    const int lane = threadIdx.x & 31;
+    const int sub = lane / W, sl = lane % W;
+    const bool vec_ok = static_cast<uint32_t>(sl) < a.nvec;
+    const uint32_t warps_per_cta = blockDim.x >> 5;
+    const uint32_t n_warps = gridDim.x * warps_per_cta;
+    const uint32_t field_bytes = a.nvec * 16;
+
+    for (uint32_t b = blockIdx.x * warps_per_cta + (threadIdx.x >> 5); b < a.B; b += n_warps) {
+        const char* row = a.x + static_cast<size_t>(b) * a.x_pitch + sl * 16;
+        float s[E], q[E];
+#pragma unroll
+        for (int i = 0; i < E; ++i) { s[i] = 0.f; q[i] = 0.f; }
+        for (uint32_t t0 = 0; t0 < a.T; t0 += P * U) {
+            uint4 v[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const uint32_t t = t0 + u * P + sub;
+                v[u] = ld_stream16(row + static_cast<size_t>(t) * field_bytes, vec_ok && t < a.T);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {  // a predicated-off load left zeros: they add nothing to s or q
+                float f[E];
+                Elt<DT>::unpack(v[u], f);
+#pragma unroll
+                for (int i = 0; i < E; ++i) { s[i] += f[i]; q[i] = fmaf(f[i], f[i], q[i]); }
+            }
+        }
+#pragma unroll
+        for (int d = W; d < 32; d <<= 1) {
+#pragma unroll
+            for (int i = 0; i < E; ++i) {
+                s[i] += __shfl_xor_sync(0xffffffffu, s[i], d);
+                q[i] += __shfl_xor_sync(0xffffffffu, q[i], d);
+            }
+        }
+        float part = 0.f;
+        float vc[E];
+#pragma unroll
+        for (int i = 0; i < E; ++i) {
+            vc[i] = 0.5f * fmaf(s[i], s[i], -q[i]);
+            part += vc[i];
+        }
+        if (!vec_ok) part = 0.f;
+        if (a.v && sub == 0 && vec_ok) {
+            float4* pv = reinterpret_cast<float4*>(a.v + static_cast<size_t>(b) * a.D + sl * E);
+#pragma unroll
+            for (int i = 0; i < E / 4; ++i) pv[i] = make_float4(vc[4 * i], vc[4 * i + 1], vc[4 * i + 2], vc[4 * i + 3]);
+        }
+        if (a.y) {
+#pragma unroll
+            for (int d = 1; d < W; d <<= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
+            if (lane == 0) a.y[b] = part;
+        }
+    }
+}
+
+// ---- element-wise operators ---------------------------------------------------------------------------------------
+// Thread (tx, ty) of a CTA owns column vector blockIdx.x*CX + tx and rows blockIdx.y*RY + ty, +gridDim.y*RY, ...:
+// the bias of its columns is loaded once, rows are walked U at a time so U x (inputs) 16-byte loads are in flight.
+struct EwArgs {
+    const char* x0;   // cross only
+    const char* xl;   // cross only
+    const char* u;
+    const float* bias;
+    char* out;
+    uint32_t B, vpr;  // rows, 16-byte vectors per row
+    int act;
+};
+
+template <int E>
+__device__ __forceinline__ void load_bias(const float* bias, uint32_t col_vec, bool ok, float (&bv)[E]) {
+#pragma unroll
+    for (int i = 0; i < E; ++i) bv[i] = 0.f;
+    if (bias && ok) {
+        const float4* p = reinterpret_cast<const float4*>(bias + static_cast<size_t>(col_vec) * E);
+#pragma unroll
+        for (int i = 0; i < E / 4; ++i) {
+            const float4 b4 = __ldg(p + i);
+            bv[4 * i] = b4.x; bv[4 * i + 1] = b4.y; bv[4 * i + 2] = b4.z; bv[4 * i + 3] = b4.w;
+        }
+    }
+}
+
+template <int DT, int U>
+__global__ void __launch_bounds__(256) cross_combine_kernel(const EwArgs a, const uint32_t cx_log2) {
+    constexpr int E = Elt<DT>::kPerVec;
+    const uint32_t cx = 1u << cx_log2, ry = blockDim.x >> cx_log2;
+    const uint32_t tx = threadIdx.x & (cx - 1), ty = threadIdx.x >> cx_log2;
+    const uint32_t c = blockIdx.x * cx + tx;
+    const bool col_ok = c < a.vpr;
+    float bv[E];
+    load_bias<E>(a.bias, c, col_ok, bv);
+    const uint32_t r_step = gridDim.y * ry;
+    for (uint32_t r0 = blockIdx.y * ry + ty; r0 < a.B; r0 += r_step * U) {
+        uint4 vx0[U], vxl[U], vu[U];
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            const uint32_t r = r0 + k * r_step;
+            const bool ok = col_ok && r < a.B;
+            const size_t off = (static_cast<size_t>(r) * a.vpr + c) * 16;
+            vx0[k] = ld_stream16(a.x0 + off, ok);
+            vu[k] = ld_stream16(a.u + off, ok);
+            vxl[k] = ld_stream16(a.xl + off, ok);
+        }
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            const uint32_t r = r0 + k * r_step;
+            if (col_ok && r < a.B) {
+                float f0[E], fl[E], fu[E], o[E];
+                Elt<DT>::unpack(vx0[k], f0);
+                Elt<DT>::unpack(vxl[k], fl);
+                Elt<DT>::unpack(vu[k], fu);
+#pragma unroll
+                for (int i = 0; i < E; ++i) o[i] = fmaf(f0[i], fu[i] + bv[i], fl[i]);
+                st_stream16(a.out + (static_cast<size_t>(r) * a.vpr + c) * 16, Elt<DT>::pack(o));
+            }
+        }
+    }
+}
+
+template <int DT, int U>
+__global__ void __launch_bounds__(256) bias_act_kernel(const EwArgs a, const uint32_t cx_log2) {
+    constexpr int E = Elt<DT>::kPerVec;
+    const uint32_t cx = 1u << cx_log2, ry = blockDim.x >> cx_log2;
+    const uint32_t tx = threadIdx.x & (cx - 1), ty = threadIdx.x >> cx_log2;
+    const uint32_t c = blockIdx.x * cx + tx;
+    const bool col_ok = c < a.vpr;
+    float bv[E];
+    load_bias<E>(a.bias, c, col_ok, bv);
+    const uint32_t r_step = gridDim.y * ry;
+    for (uint32_t r0 = blockIdx.y * ry + ty; r0 < a.B; r0 += r_step * U) {
+        uint4 vu[U];
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            const uint32_t r = r0 + k * r_step;
+            vu[k] = ld_stream16(a.u + (static_cast<size_t>(r) * a.vpr + c) * 16, col_ok && r < a.B);
+        }
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            const uint32_t r = r0 + k * r_step;
+            if (col_ok && r < a.B) {
+                float fu[E], o[E];
+                Elt<DT>::unpack(vu[k], fu);
+#pragma unroll
+                for (int i = 0; i < E; ++i) {
+                    float s = fu[i] + bv[i];
+                    if (a.act == DPI_ACT_RELU) s = fmaxf(s, 0.f);
+                    else if (a.act == DPI_ACT_SIGMOID) s = 1.f / (1.f + expf(-s));
+                    o[i] = s;
+                }
+                st_stream16(a.out + (static_cast<size_t>(r) * a.vpr + c) * 16, Elt<DT>::pack(o));
+            }
+        }
+    }
+}
+
+int pow2ceil_i(int x) { int p = 1; while (p < x) p <<= 1; return p; }
+int log2_i(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
+
+int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+            (void)cudaGetLastError();
+            n = 148;
+        }
+    }
+    return n;
+}
+
+template <int DT>
+cudaError_t launch_fm_dt(const FmArgs& a, int W, cudaStream_t st) {
+    const int warps_per_cta = 8;
+    const long long want = (static_cast<long long>(a.B) + warps_per_cta - 1) / warps_per_cta;
+    const long long cap = static_cast<long long>(sm_count()) * 8 * 4;  // a few waves; warps stride over samples
+    const unsigned grid = static_cast<unsigned>(want < cap ? (want < 1 ? 1 : want) : cap);
+    count_launch();
+    switch (W) {
+#define DPI_FM_CASE(w) case w: fm_kernel<DT, w, 4><<<grid, 256, 0, st>>>(a); break;
+        DPI_FM_CASE(1) DPI_FM_CASE(2) DPI_FM_CASE(4) DPI_FM_CASE(8) DPI_FM_CASE(16) DPI_FM_CASE(32)
+#undef DPI_FM_CASE
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+struct EwGrid { dim3 grid; uint32_t cx_log2; };
+EwGrid ew_grid(uint32_t B, uint32_t vpr, int U) {
+    const int cx = std::min(256, pow2ceil_i(static_cast<int>(vpr)));
+    const int ry = 256 / cx;
+    EwGrid g;
+    g.cx_log2 = static_cast<uint32_t>(log2_i(cx));
+    const unsigned gx = (vpr + cx - 1) / cx;
+    const long long rows_blocks = (static_cast<long long>(B) + static_cast<long long>(ry) * U - 1) / (static_cast<long long>(ry) * U);
+    long long gy = static_cast<long long>(sm_count()) * 8 / gx;   // ~8 CTAs per SM in total
+    if (gy < 1) gy = 1;
+    if (gy > rows_blocks) gy = rows_blocks < 1 ? 1 : rows_blocks;
+    if (gy > 65535) gy = 65535;
+    g.grid = dim3(gx, static_cast<unsigned>(gy));
+    return g;
+}
+
+}  // namespace
+
+cudaError_t launch_fm(const void* x, int dtype, uint32_t B, uint32_t T, uint32_t D, uint64_t x_pitch_bytes, float* y,
+                      float* v, cudaStream_t st) {
+    const uint32_t elt = dtype == DPI_F32 ? 4u : 2u;
+    FmArgs a{static_cast<const char*>(x), y, v, x_pitch_bytes, B, T, D, D * elt / 16u};
+    const int W = pow2ceil_i(static_cast<int>(a.nvec));
+    switch (dtype) {
+        case DPI_F32: return launch_fm_dt<DPI_F32>(a, W, st);
+        case DPI_F16: return launch_fm_dt<DPI_F16>(a, W, st);
+        case DPI_BF16: return launch_fm_dt<DPI_BF16>(a, W, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+cudaError_t launch_cross_combine(const void* x0, const void* xl, const void* u, const float* bias, void* out, int dtype,
+                                 uint32_t B, uint32_t F, cudaStream_t st) {
+    const uint32_t elt = dtype == DPI_F32 ? 4u : 2u;
+    EwArgs a{static_cast<const char*>(x0), static_cast<const char*>(xl), static_cast<const char*>(u), bias,
+             static_cast<char*>(out), B, F * elt / 16u, 0};
+    constexpr int U = 4;
+    const EwGrid g = ew_grid(B, a.vpr, U);
+    count_launch();
+    switch (dtype) {
+        case DPI_F32: cross_combine_kernel<DPI_F32, U><<<g.grid, 256, 0, st>>>(a, g.cx_log2); break;
+        case DPI_F16: cross_combine_kernel<DPI_F16, U><<<g.grid, 256, 0, st>>>(a, g.cx_log2); break;
+        case DPI_BF16: cross_combine_kernel<DPI_BF16, U><<<g.grid, 256, 0, st>>>(a, g.cx_log2); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bias_act(const void* u, const float* bias, void* out, int dtype, uint32_t B, uint32_t F, int act,
+                            cudaStream_t st) {
+    const uint32_t elt = dtype == DPI_F32 ? 4u : 2u;
+    EwArgs a{nullptr, nullptr, static_cast<const char*>(u), bias, static_cast<char*>(out), B, F * elt / 16u, act};
+    constexpr int U = 8;
+    const EwGrid g = ew_grid(B, a.vpr, U);
+    count_launch();
+    switch (dtype) {
+        case DPI_F32: bias_act_kernel<DPI_F32, U><<<g.grid, 256, 0, st>>>(a, g.cx_log2); break;
+        case DPI_F16: bias_act_kernel<DPI_F16, U><<<g.grid, 256, 0, st>>>(a, g.cx_log2); break;
+        case DPI_BF16: bias_act_kernel<DPI_BF16, U><<<g.grid, 256, 0, st>>>(a, g.cx_log2); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace dpi

@@ -329,6 +329,18 @@ def full_table_storage(cfg: Config, t: int, n_rows: int, chunk: int = 1 << 18) -
     return out
 
 
+STREAM_DENSE = 97  # dense activations for the NEXT-4 operators (X_embed-shaped blocks, GEMM outputs, biases)
+
+
+def dense_values_f32(seed: int, sub: int, shape, scale: float = 0.25) -> np.ndarray:
+    """float32 array of `shape`, uniform in [-scale, scale): element i (row-major) comes from counter i of stream
+    (seed, STREAM_DENSE, sub). Stand-in for pooled embedding blocks / layer activations."""
+    n = int(np.prod(shape))
+    h = hash_u64(stream_key(seed, STREAM_DENSE, sub), np.arange(n, dtype=np.uint64))
+    x = (h >> np.uint64(40)).astype(np.float32) * np.float32(2.0 ** -24)
+    return ((x - np.float32(0.5)) * np.float32(2.0 * scale)).reshape(shape)
+
+
 # ----------------------------------------------------------------------------------------------------
 # sub-problems for sampled parity at full size
 # ----------------------------------------------------------------------------------------------------

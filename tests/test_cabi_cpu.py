@@ -36,9 +36,44 @@ def test_library_exports_every_declared_symbol(lib):
 
 
 def test_no_torch_types_in_the_boundary():
-    text = open(os.path.join(ROOT, "include", "dpi.h")).read()
-    assert "torch" not in re.sub(r"/\*.*?\*/", "", text, flags=re.S).lower()
-    assert "cuda_runtime" not in text
+    for header in ("dpi.h", "dpi_nongemm.h"):
+        text = open(os.path.join(ROOT, "include", header)).read()
+        assert "torch" not in re.sub(r"/\*.*?\*/", "", text, flags=re.S).lower()
+        assert "cuda_runtime" not in text
+
+
+def test_library_exports_every_symbol_of_the_nongemm_header(lib):
+    from paper_2606_21101_b200 import nongemm
+    text = open(os.path.join(ROOT, "include", "dpi_nongemm.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(dpi_[a-z_0-9]+)\s*\(", text)))
+    assert sorted(nongemm.EXPORTS) == declared
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_nongemm_argument_validation_and_host_schedule_need_no_device(lib):
+    from paper_2606_21101_b200 import nongemm
+    nongemm._lib()
+    buf = np.zeros(64, dtype=np.float32)
+    p = buf.ctypes.data - buf.ctypes.data % 16 + 16
+    assert lib.dpi_fm_interaction(None, 0, 4, 2, 4, 0, p, None, None) == 1          # NULL x
+    assert lib.dpi_fm_interaction(p, 0, 4, 2, 4, 0, None, None, None) == 1          # neither y nor v
+    assert lib.dpi_fm_interaction(p, 0, 4, 2, 3, 0, p, None, None) == 2             # 12-byte field
+    assert lib.dpi_fm_interaction(p, 0, 4, 2, 4, 6, p, None, None) == 1             # x_ld < T*D
+    assert lib.dpi_fm_interaction(p, 9, 4, 2, 4, 0, p, None, None) == 1             # dtype
+    assert lib.dpi_fm_interaction(p, 0, 0, 2, 4, 0, p, None, None) == 0             # B = 0: nothing to do, no launch
+    assert lib.dpi_cross_combine(p, p, None, None, p, 0, 2, 4, None) == 1
+    assert lib.dpi_cross_combine(p, p, p, None, p, 0, 2, 3, None) == 2
+    assert lib.dpi_cross_combine(p + 4, p, p, None, p, 0, 2, 4, None) == 1          # misaligned
+    assert lib.dpi_bias_act(p, None, p, 0, 2, 4, 5, None) == 1                      # unknown activation
+    assert lib.dpi_bias_act(p, None, p, 1, 2, 4, 1, None) == 2                      # 8-byte fp16 row
+    assert b"dpi_bias_act" in lib.dpi_last_error()
+    assert nongemm.bfs_schedule(2, 4) == [(1, 0), (0, 0), (1, 1), (0, 1), (1, 2), (1, 3)]   # PAPER.md Alg. 2, by hand
+    assert nongemm.bfs_schedule(0, 0) == []
+    with pytest.raises(binding.DpiError):
+        nongemm.bfs_schedule(-1, 2)
+    assert lib.dpi_launcher_run(None, None, 0, None, 0, 2, None) == 1
 
 
 def _create(lib, T, rows, dims, dtype, B, max_idx):
