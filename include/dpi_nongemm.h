@@ -61,7 +61,8 @@ typedef enum { DPI_ACT_IDENTITY = 0, DPI_ACT_RELU = 1, DPI_ACT_SIGMOID = 2 } dpi
 /*
  * dpi_bias_act -- the non-GEMM part of one MLP layer: out[b,f] = act(u[b,f] + bias[f]) ("GEMM and
  * activation operators"). u_dev, out_dev [B, F] dense of `dtype` (may alias); bias_dev NULL or fp32[F];
- * F*sizeof(elt) a multiple of 16. Sigmoid is 1 / (1 + exp(-s)) in fp32 (expf, not the fast intrinsic).
+ * F*sizeof(elt) a multiple of 16. Sigmoid is 1 / (1 + exp(-s)) in fp32 with the hardware ex2 / rcp approximations
+ * (absolute error <= 2^-21 before the output cast; the precise expf + IEEE division made the operator ALU-bound).
  */
 dpi_status_t dpi_bias_act(const void* u_dev, const float* bias_dev, void* out_dev, dpi_dtype_t dtype, int32_t B,
                           int32_t F, dpi_act_t act, void* stream);

@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(256) bias_act_kernel(const EwArgs a, const uin
                 for (int i = 0; i < E; ++i) {
                     float s = fu[i] + bv[i];
                     if (a.act == DPI_ACT_RELU) s = fmaxf(s, 0.f);
-                    else if (a.act == DPI_ACT_SIGMOID) s = 1.f / (1.f + expf(-s));
+                    else if (a.act == DPI_ACT_SIGMOID) s = __fdividef(1.f, 1.f + __expf(-s));  // ex2.approx + rcp.approx: a few fp32 ulps
                     o[i] = s;
                 }
                 st_stream16(a.out + (static_cast<size_t>(r) * a.vpr + c) * 16, Elt<DT>::pack(o));
