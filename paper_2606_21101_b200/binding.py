@@ -280,7 +280,7 @@ def dpi_lookup(table_ptrs_dev, indices_dev, offsets_dev, plan: Plan, pooling, ou
 _synth = None
 
 
-def synth_fill_table(dst_dev, n_elems: int, dtype: int, key: int, stream=None):
+def _synth_lib():
     global _synth
     if _synth is None:
         path = _build.lib_path("libdpi_synth.so")
@@ -290,6 +290,25 @@ def synth_fill_table(dst_dev, n_elems: int, dtype: int, key: int, stream=None):
         _synth.dpi_synth_fill_table.restype = ctypes.c_int
         _synth.dpi_synth_fill_table.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int, ctypes.c_uint64,
                                                 ctypes.c_void_p]
+        _synth.dpi_synth_row_read_probe.restype = ctypes.c_int
+        _synth.dpi_synth_row_read_probe.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint64,
+                                                    ctypes.c_uint64, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                    ctypes.c_void_p, ctypes.c_void_p]
+    return _synth
+
+
+def synth_row_read_probe(base_dev, span_rows: int, row_bytes: int, n_rows: int, key: int, random: bool, unroll: int,
+                         ctas_per_sm: int, sink_dev, stream=None):
+    """Bench context only: read n_rows whole rows at hashed (or consecutive) positions of a span_rows-row buffer."""
+    rc = _synth_lib().dpi_synth_row_read_probe(_ptr(base_dev), int(span_rows), int(row_bytes), int(n_rows), int(key),
+                                               int(bool(random)), int(unroll), int(ctas_per_sm), _ptr(sink_dev),
+                                               _stream_handle(stream))
+    if rc != 0:
+        raise RuntimeError(f"dpi_synth_row_read_probe failed with cudaError {rc}")
+
+
+def synth_fill_table(dst_dev, n_elems: int, dtype: int, key: int, stream=None):
+    _synth = _synth_lib()
     rc = _synth.dpi_synth_fill_table(_ptr(dst_dev), int(n_elems), int(dtype), int(key), _stream_handle(stream))
     if rc != 0:
         raise RuntimeError(f"dpi_synth_fill_table failed with cudaError {rc}")

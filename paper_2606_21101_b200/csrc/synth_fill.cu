@@ -73,3 +73,55 @@ extern "C" int dpi_synth_fill_table(void* dst, uint64_t n_elems, int dtype, uint
     }
     return (int)cudaGetLastError();
 }
+
+// ---- gather ceiling probe (bench context, not part of the method) -----------------------------------------------------
+// What can this box sustain for independent reads of whole `row_bytes`-byte rows at random (or consecutive) positions of
+// a `span_rows`-row buffer, with no indices to fetch, no pooling and no output? That is the ceiling the fused lookup's
+// row stream can be compared with (SURVEY.md 8(d) "random-access ceiling"): W = row_bytes/16 lanes read one row with one
+// 128-bit load each, U rows in flight per lane, row ids from a counter hash (random) or the counter itself (sequential).
+namespace {
+template <int U>
+__global__ void __launch_bounds__(256) row_read_probe_kernel(const char* __restrict__ base, unsigned long long span_rows,
+                                                             unsigned int row_bytes, unsigned long long n_rows,
+                                                             unsigned long long key, int random, unsigned int* sink) {
+    const unsigned int W = row_bytes / 16;                     // lanes per row (power of two <= 32)
+    const unsigned int lane = threadIdx.x & 31, sl = lane % W, sub = lane / W, P = 32 / W;
+    const unsigned long long warp = (blockIdx.x * static_cast<unsigned long long>(blockDim.x) + threadIdx.x) >> 5;
+    const unsigned long long n_warps = (gridDim.x * static_cast<unsigned long long>(blockDim.x)) >> 5;
+    unsigned int acc = 0;
+    for (unsigned long long i0 = warp * (P * U); i0 < n_rows; i0 += n_warps * (P * U)) {
+        uint4 v[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const unsigned long long i = i0 + u * P + sub;
+            // hash -> [0, span_rows) by multiply-high (a 64-bit modulo costs more than the load it feeds)
+            const unsigned long long r = random ? __umul64hi(fmix64(key + i * 0x9E3779B97F4A7C15ull), span_rows)
+                                                : (i < span_rows ? i : i - span_rows * (i / span_rows));
+            v[u] = __ldg(reinterpret_cast<const uint4*>(base + r * row_bytes + sl * 16));
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+    }
+    if (acc == 0x9E3779B9u) *sink = acc;                       // keeps the loads alive; practically never taken
+}
+}  // namespace
+
+// Reads n_rows rows of row_bytes (16..512, power of two) from base[span_rows * row_bytes]. unroll in {2, 4, 8}.
+extern "C" int dpi_synth_row_read_probe(const void* base, uint64_t span_rows, uint32_t row_bytes, uint64_t n_rows,
+                                        uint64_t key, int random, int unroll, int ctas_per_sm, void* sink_dev, void* stream) {
+    if (!base || !sink_dev || span_rows == 0 || row_bytes < 16 || row_bytes > 512 || (row_bytes & (row_bytes - 1)))
+        return (int)cudaErrorInvalidValue;
+    int dev = 0, sms = 148;
+    (void)cudaGetDevice(&dev);
+    (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const unsigned int blocks = static_cast<unsigned int>(sms * (ctas_per_sm > 0 ? ctas_per_sm : 8));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const char* b = static_cast<const char*>(base);
+    unsigned int* sk = static_cast<unsigned int*>(sink_dev);
+    switch (unroll) {
+        case 2: row_read_probe_kernel<2><<<blocks, 256, 0, s>>>(b, span_rows, row_bytes, n_rows, key, random, sk); break;
+        case 8: row_read_probe_kernel<8><<<blocks, 256, 0, s>>>(b, span_rows, row_bytes, n_rows, key, random, sk); break;
+        default: row_read_probe_kernel<4><<<blocks, 256, 0, s>>>(b, span_rows, row_bytes, n_rows, key, random, sk); break;
+    }
+    return (int)cudaGetLastError();
+}
