@@ -263,11 +263,29 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
         }
         return r;
     };
+    // bag g_new > g_prev given the reference of g_prev: the dense layout steps the table id instead of dividing again
+    // (a 32-bit modulo by a run-time T is ~20 instructions, once per bag on the long-bag path)
+    auto bag_ref_next = [&](const BagRef& prev, uint32_t g_prev, uint32_t g_new) -> BagRef {
+        if constexpr (GEN) {
+            return bag_ref(g_new);
+        } else {
+            BagRef r = prev;
+            uint32_t t = prev.t + (g_new - g_prev);
+            if (t >= a.T) {
+                t -= a.T;
+                if (t >= a.T) t %= a.T;  // only after a run of >= T empty bags
+            }
+            r.t = t;
+            r.tab = s_tab[t] + sl * 16;
+            return r;
+        }
+    };
     auto out_of = [&](uint32_t g, const BagRef& r) -> char* {
         if constexpr (GEN) return r.outp;
         else return out + static_cast<size_t>(g) * (static_cast<size_t>(a.nvec) * kOutVec) + sl * kOutVec;
     };
-    auto idx_at = [&](const int* ip, int e) -> int { return GEN ? ip[e << ish] : ip[e]; };
+    // row ids are non-negative (precondition, dpi.h): read as uint32 so that id * row_bytes is one IMAD.WIDE.U32
+    auto idx_at = [&](const int* ip, int e) -> uint32_t { return static_cast<uint32_t>(GEN ? ip[e << ish] : ip[e]); };
     auto wgt_at = [&](const float* wp, int e) -> float { return (GEN && wp) ? wp[e] : 1.f; };
     auto accum = [&](float2 (&acc)[kAcc2], const uint4& v, float w) {
         if constexpr (GEN) Tr::fma(acc, v, make_float2(w, w));  // fma(x, 1, acc) == x + acc exactly
@@ -350,8 +368,8 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                         const bool ok = i < nb;
                         BagRef& b = br[GEN ? u : 0];
                         b = bag_ref(g_lo + (ok ? i : 0u));
-                        const int r = idx_at(ip, e_lo + (ok ? i : 0u));
-                        v[u] = ld_row16(b.tab + static_cast<size_t>(r) * b.row_bytes, ok && b.ok);
+                        const uint32_t r = idx_at(ip, e_lo + (ok ? i : 0u));
+                        v[u] = ld_row16(b.tab + static_cast<uint64_t>(r) * b.row_bytes, ok && b.ok);
                     }
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
@@ -388,9 +406,9 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                         for (int u = 0; u < U; ++u) {
                             const bool ok = j + u < hi;
                             const int e = ok ? j + u : lo;
-                            const int r = idx_at(ip, e);
+                            const uint32_t r = idx_at(ip, e);
                             w[u] = wgt_at(wp, e);
-                            v[u] = ld_row16(br.tab + static_cast<size_t>(r) * br.row_bytes, ok && br.ok);
+                            v[u] = ld_row16(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
                         }
 #pragma unroll
                         for (int u = 0; u < U; ++u) accum(acc, v[u], w[u]);
@@ -415,9 +433,9 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                             const int e = j + u * P + sub;
                             const bool ok = e < hi;
                             const int ec = ok ? e : lo;
-                            const int r = idx_at(ip, ec);
+                            const uint32_t r = idx_at(ip, ec);
                             w[u] = wgt_at(wp, ec);
-                            v[u] = ld_row16(br.tab + static_cast<size_t>(r) * br.row_bytes, ok && br.ok);
+                            v[u] = ld_row16(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
                         }
 #pragma unroll
                         for (int u = 0; u < U; ++u) accum(acc, v[u], w[u]);
@@ -457,9 +475,9 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                         const int e = j + u * P + sub;
                         const bool ok = e < hi;
                         const int ec = ok ? e : j;
-                        const int r = idx_at(ip, ec);
+                        const uint32_t r = idx_at(ip, ec);
                         if constexpr (GEN) bf.w[u] = wgt_at(wp, ec);
-                        bf.v[u] = ld_row16(br.tab + static_cast<size_t>(r) * br.row_bytes, ok && br.ok);
+                        bf.v[u] = ld_row16(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
                     }
                 };
                 uint32_t g = g_lo;
@@ -494,7 +512,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                                 store_zero(g_n);
                                 ++g_n;
                             }
-                            if (has_next) { j_n = lo_n; br_n = bag_ref(g_n); }
+                            if (has_next) { j_n = lo_n; br_n = bag_ref_next(br, g, g_n); }
                         }
                         if (has_next) issue(nv, j_n, hi_n, br_n);
 #pragma unroll
