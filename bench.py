@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--mode", type=int, default=0)
     ap.add_argument("--pdl", type=int, default=0)
     ap.add_argument("--host-chunks", type=int, default=0, help="dpi_forward_host: 0 auto, 1 unpipelined, n chunks")
+    ap.add_argument("--host-direct-out", type=int, default=0,
+                    help="dpi_forward_host: 0 auto (lookup stores straight into pinned out_host), 1 staged + D2H copy, 2 require direct")
     ap.add_argument("--kernel", default="output_first", choices=["output_first", "input_first"],
                     help="input_first = the paper's strawman mapping (ablation, PAPER.md:172-176)")
     ap.add_argument("--graph", type=int, default=-1, help="1: time a CUDA-graph replay of the K steps; 0: stream launches; -1: auto (graph for c1-c3)")
@@ -189,6 +191,7 @@ def apply_options(plan, args, binding):
     plan.set_option(binding.OPT_MODE, args.mode)
     plan.set_option(binding.OPT_PDL, args.pdl)
     plan.set_option(binding.OPT_HOST_CHUNKS, args.host_chunks)
+    plan.set_option(binding.OPT_HOST_DIRECT_OUT, args.host_direct_out)
 
 
 def workload_config(args):
@@ -416,7 +419,9 @@ def run_ours(args):
         d2h = int(out_host.numel() * out_host.element_size())
         e2e = {"value": sharding.job_throughput(cfg.G, n_e2e, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / n_e2e, "steps": n_e2e,
-               "api": "dpi_forward_host (pinned host lengths/indices in, [B,T*D] block out, tables resident)"}
+               "api": "dpi_forward_host (pinned host lengths/indices in, [B,T*D] block out, tables resident)",
+               "d2h": ("staged device block + cudaMemcpyAsync" if args.host_direct_out == 1 else
+                       "fused into the lookup's store: the kernel writes the block straight into the pinned host buffer over PCIe")}
 
     if rank != 0:
         if dist is not None:

@@ -84,6 +84,12 @@ typedef enum {
     DPI_OPT_PDL = 5,            /* 1: lookup is launched with programmatic dependent launch after the planner */
     DPI_OPT_HOST_CHUNKS = 6,    /* dpi_forward_host only: number of sample chunks pipelined over the copy engines and the
                                    SMs; 0 = auto (~16 MB of PCIe traffic per chunk, <= 8), 1 = no pipelining, up to 64 */
+    DPI_OPT_HOST_DIRECT_OUT = 7,/* dpi_forward_host only: 0 = auto, 1 = always stage (lookup -> device block -> D2H copy),
+                                   2 = require direct. Direct: when out_host is page-locked, device-mapped memory
+                                   (cudaHostAlloc / cudaHostRegister), the lookup kernel stores the pooled vectors
+                                   straight into it over PCIe -- the device->host transfer is fused into the kernel's
+                                   store, no staging block and no D2H copy. Auto uses it whenever out_host qualifies;
+                                   2 returns DPI_ERR_INVALID_ARG if it does not. */
     DPI_OPT_COUNT_
 } dpi_option_t;
 

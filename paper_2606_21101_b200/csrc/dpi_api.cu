@@ -76,7 +76,7 @@ struct dpi_plan_s {
     int32_t K_user = 0;      // 0 = default
     uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
     uint32_t num_tiles = 0, num_chunks = 0, tiles_per_chunk = 0;
-    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0, 0};
+    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0, 0, 0};
     // device
     int device = 0, num_sms = 0;
     int32_t* offsets = nullptr;
@@ -408,6 +408,7 @@ dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
         case DPI_OPT_ROW_L1_NO_ALLOC: ok = v == -1 || v == 0; break;  // the bypass variant was removed (see dpi.h)
         case DPI_OPT_PDL: ok = v == 0 || v == 1; break;
         case DPI_OPT_HOST_CHUNKS: ok = v >= 0 && v <= 64; break;
+        case DPI_OPT_HOST_DIRECT_OUT: ok = v >= 0 && v <= 2; break;
         default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);
     }
     if (!ok) return fail(DPI_ERR_INVALID_ARG, "value %d not supported for option %d", v, (int)opt);
@@ -648,19 +649,42 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
         DPI_CUDA(cudaMalloc(&p->stage_idx, idx_bytes));
         p->stage_idx_bytes = idx_bytes;
     }
-    if (!p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, static_cast<size_t>(p->B) * p->out_width * 4));
 
+    // Direct output: if out_host is page-locked and mapped into this device's address space, the lookup stores into
+    // it over PCIe and the separate device->host copy disappears (DPI_OPT_HOST_DIRECT_OUT).
+    char* out_direct = nullptr;
+    if (p->opt[DPI_OPT_HOST_DIRECT_OUT] != 1) {
+        cudaPointerAttributes pa{};
+        if (cudaPointerGetAttributes(&pa, out_host) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer &&
+            (reinterpret_cast<uintptr_t>(pa.devicePointer) & 31u) == 0) {
+            out_direct = static_cast<char*>(pa.devicePointer);
+        } else {
+            (void)cudaGetLastError();
+            if (p->opt[DPI_OPT_HOST_DIRECT_OUT] == 2)
+                return fail(DPI_ERR_INVALID_ARG, "DPI_OPT_HOST_DIRECT_OUT = 2 but out_host is not page-locked device-mapped memory (32-byte aligned)");
+        }
+    }
+    if (!out_direct && !p->stage_out) DPI_CUDA(cudaMalloc(&p->stage_out, static_cast<size_t>(p->B) * p->out_width * 4));
+    char* const out_base = out_direct ? out_direct : static_cast<char*>(p->stage_out);
+
+    // with direct output only the inputs cross PCIe as copies; the chunking then follows the input bytes alone
     const int n_chunks = host_chunks(p, static_cast<size_t>(p->G) * 4 + static_cast<size_t>(n_indices) * idx_elt + out_bytes);
     if (n_chunks <= 1) {
+        int64_t total = 0;  // same host-side check as the pipelined path: the lengths must add up to n_indices
+        for (size_t g = 0; g < static_cast<size_t>(p->G); ++g) {
+            if (lengths_host[g] < 0) return fail(DPI_ERR_INVALID_ARG, "lengths_host[%zu] is negative", g);
+            total += lengths_host[g];
+        }
+        if (total != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)total);
         DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * idx_elt, cudaMemcpyHostToDevice, s));
         dpi_status_t st = dpi_plan_build(p, p->stage_len, s);
         if (st != DPI_OK) return st;
         LookupCall c;
-        c.tables = table_ptrs_dev; c.indices = p->stage_idx; c.pooling = pooling; c.out = p->stage_out;
+        c.tables = table_ptrs_dev; c.indices = p->stage_idx; c.pooling = pooling; c.out = out_base;
         st = do_lookup(p, c, s);
         if (st != DPI_OK) return st;
-        DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
+        if (!out_direct) DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
         DPI_CUDA(cudaStreamSynchronize(s));
         return DPI_OK;
     }
@@ -701,7 +725,7 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
         const size_t n_g = static_cast<size_t>(q->G);
         const int64_t e0 = entry_lo[c], n_e = entry_lo[c + 1] - entry_lo[c];
         char* idx_dev = static_cast<char*>(p->stage_idx) + static_cast<size_t>(e0) * idx_elt;
-        char* out_dev = static_cast<char*>(p->stage_out) + static_cast<size_t>(h->sample_lo[c]) * row_bytes;
+        char* out_dev = out_base + static_cast<size_t>(h->sample_lo[c]) * row_bytes;
         DPI_CUDA(cudaMemcpyAsync(p->stage_len + g0, lengths_host + g0, n_g * sizeof(int32_t), cudaMemcpyHostToDevice, cs));
         if (n_e) DPI_CUDA(cudaMemcpyAsync(idx_dev, static_cast<const char*>(indices_host) + static_cast<size_t>(e0) * idx_elt,
                                           static_cast<size_t>(n_e) * idx_elt, cudaMemcpyHostToDevice, cs));
@@ -711,8 +735,9 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
         lc.tables = table_ptrs_dev; lc.indices = idx_dev; lc.pooling = pooling; lc.out = out_dev;
         st = do_lookup(q, lc, cs);
         if (st != DPI_OK) return st;
-        DPI_CUDA(cudaMemcpyAsync(static_cast<char*>(out_host) + static_cast<size_t>(h->sample_lo[c]) * row_bytes, out_dev,
-                                 static_cast<size_t>(q->B) * row_bytes, cudaMemcpyDeviceToHost, cs));
+        if (!out_direct)
+            DPI_CUDA(cudaMemcpyAsync(static_cast<char*>(out_host) + static_cast<size_t>(h->sample_lo[c]) * row_bytes, out_dev,
+                                     static_cast<size_t>(q->B) * row_bytes, cudaMemcpyDeviceToHost, cs));
     }
     for (int i = 0; i < HostPipeline::kStreams; ++i) {
         DPI_CUDA(cudaEventRecord(h->ev_done[i], h->st[i]));

@@ -288,6 +288,20 @@ def test_forward_host_equals_device_path():
         out.fill_(float("nan"))
         plan.forward_host(dt.ptrs, ln, idx, out, pooling=pooling)
         assert np.array_equal(out.double().numpy(), dev), f"{chunks} chunks"
+    # output path: staged block + D2H copy (1) and the lookup storing straight into the pinned host block (2, and what
+    # auto picked above) give the same bytes, pipelined or not
+    for direct in (1, 2):
+        plan.set_option(binding.OPT_HOST_DIRECT_OUT, direct)
+        for chunks in (1, 5):
+            plan.set_option(binding.OPT_HOST_CHUNKS, chunks)
+            out.fill_(float("nan"))
+            plan.forward_host(dt.ptrs, ln, idx, out, pooling=pooling)
+            assert np.array_equal(out.double().numpy(), dev), f"direct_out={direct}, {chunks} chunks"
+    pageable = torch.empty((cfg.B, cfg.T * cfg.D), dtype=torch.bfloat16)
+    with pytest.raises(binding.DpiError):   # "require direct" on memory the device cannot store into
+        plan.forward_host(dt.ptrs, ln, idx, pageable, pooling=pooling)
+    plan.set_option(binding.OPT_HOST_DIRECT_OUT, 0)
+    plan.set_option(binding.OPT_HOST_CHUNKS, 0)
     # pageable host memory works as well
     out2 = torch.empty((cfg.B, cfg.T * cfg.D), dtype=torch.bfloat16)
     plan.forward_host(dt.ptrs, torch.from_numpy(batch.lengths), torch.from_numpy(batch.indices), out2, pooling=pooling)
