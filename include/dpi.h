@@ -244,6 +244,20 @@ typedef struct dpi_lookup_args_s {
 dpi_status_t dpi_lookup_ex(const dpi_lookup_args_t* args, const dpi_plan_t* plan, void* stream);
 
 /*
+ * dpi_lookup_onehot -- Algorithm 1 itself: the one-hot case, where every (sample, table) bag holds
+ * exactly one id. The workload is then pure arithmetic, so this call needs NO built plan (the plan object only supplies
+ * T, B, the common dim and the dtype): ONE launch copies row ids_dev[b*T + t] of table t to out[b, t*D .. (t+1)*D).
+ * Bit-identical to dpi_plan_build on all-ones lengths + dpi_lookup (sum or mean pooling: a bag of length 1 is its row).
+ *   ids_dev  device int32[B*T] (int64 when the plan's index type is DPI_IDX_I64), sample-major, per-table local row ids
+ *            in [0, table_rows[t]) (precondition, as in dpi_lookup)
+ *   out_dev  device [B, T*D] of the TABLE dtype, 16-byte aligned
+ * Equal dims, sample-major bags, default columns and table-dtype output only: anything else -> DPI_ERR_UNSUPPORTED
+ * (use dpi_lookup_ex). Asynchronous on `stream`.
+ */
+dpi_status_t dpi_lookup_onehot(const void* const* table_ptrs_dev, const void* ids_dev, const dpi_plan_t* plan,
+                               void* out_dev, void* stream);
+
+/*
  * dpi_lookup_input_first -- ABLATION, not the product path: the same lookup with the paper's strawman
  * "input-first" workload allocation (different samples on different threads, so table reads
  * and output writes of a warp are random), kept to measure the paper's Fig. 11 claim (output-first up to 10.3x

@@ -28,7 +28,7 @@ LOOKUP_FORCE_GENERAL = 1
 EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "dpi_plan_set_columns", "dpi_plan_out_width", "dpi_lookup_ex",
            "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
            "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export",
-           "dpi_lookup", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
+           "dpi_lookup", "dpi_lookup_onehot", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
            "dpi_version", "dpi_status_string", "dpi_last_error"]
 
 
@@ -82,6 +82,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
         "dpi_plan_export": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_lookup": (st, [vp, vp, vp, vp, vp, vp, vp]),
         "dpi_lookup_input_first": (st, [vp, vp, vp, vp, vp, vp, vp]),
+        "dpi_lookup_onehot": (st, [vp, vp, vp, vp, vp]),
         "dpi_forward_host": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_check_indices": (st, [vp, vp, vp, vp]),
         "dpi_plan_destroy": (st, [vp]),
@@ -246,6 +247,11 @@ class Plan:
         pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
         _check(self._lib.dpi_lookup_input_first(_ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(offsets_dev), self._h,
                                                 _ptr(pool), _ptr(out_dev), _stream_handle(stream)))
+
+    # -- dpi_lookup_onehot (Algorithm 1, no built plan needed) ------------------------------------------------
+    def lookup_onehot(self, table_ptrs_dev, ids_dev, out_dev, stream=None):
+        _check(self._lib.dpi_lookup_onehot(_ptr(table_ptrs_dev), _ptr(ids_dev), self._h, _ptr(out_dev),
+                                           _stream_handle(stream)))
 
     # -- dpi_forward_host -----------------------------------------------------------------------------------
     def forward_host(self, table_ptrs_dev, lengths_host, indices_host, out_host, pooling=None, stream=None):

@@ -548,6 +548,21 @@ dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int
     return do_lookup(p, c, static_cast<cudaStream_t>(stream), true);
 }
 
+dpi_status_t dpi_lookup_onehot(const void* const* table_ptrs_dev, const void* ids_dev, const dpi_plan_t* p, void* out_dev,
+                               void* stream) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (!table_ptrs_dev || !ids_dev || !out_dev) return fail(DPI_ERR_INVALID_ARG, "table_ptrs_dev/ids_dev/out_dev is NULL");
+    if (p->mixed_dims || p->custom_columns || p->bag_order != DPI_BAGS_SAMPLE_MAJOR || p->out_dtype != p->dtype)
+        return fail(DPI_ERR_UNSUPPORTED, "dpi_lookup_onehot covers equal dims, sample-major ids, default columns and table-dtype output only");
+    if (reinterpret_cast<uintptr_t>(out_dev) & 15u) return fail(DPI_ERR_INVALID_ARG, "out_dev is not 16-byte aligned");
+    const bool i64 = p->index_type == DPI_IDX_I64;
+    if (reinterpret_cast<uintptr_t>(ids_dev) & (i64 ? 7u : 3u)) return fail(DPI_ERR_INVALID_ARG, "ids_dev is misaligned");
+    cudaError_t e = launch_onehot(table_ptrs_dev, ids_dev, i64 ? 1u : 0u, out_dev, p->G, static_cast<uint32_t>(p->T), p->nvec,
+                                  p->lanes, p->num_sms, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e, "onehot_kernel launch");
+    return DPI_OK;
+}
+
 dpi_status_t dpi_plan_set_layout(dpi_plan_t* p, dpi_bag_order_t order, dpi_index_type_t index_type) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
     if (order != DPI_BAGS_SAMPLE_MAJOR && order != DPI_BAGS_TABLE_MAJOR) return fail(DPI_ERR_INVALID_ARG, "unknown bag order %d", (int)order);

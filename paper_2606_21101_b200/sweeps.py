@@ -12,6 +12,8 @@ one-hot workload with c2's recipe (26 fields, heights log-uniform in [10, 1e6], 
 the sweep fixes the shape itself. Three timings per point, CUDA events on one stream, after warm-up:
 
 * ``output_first``  dpi_lookup (the product kernel), per launch, and plan + lookup as a replayed CUDA graph
+* ``alg1_direct``   dpi_lookup_onehot: Algorithm 1 as one plan-free launch (the workload is one-hot, so the plan is pure
+                    arithmetic), per launch and as a replayed CUDA graph
 * ``input_first``   dpi_lookup_input_first (the ablation kernel, same plan, same results bit for bit)
 * ``per_table``     context only: one ``torch.nn.functional.embedding`` launch per table and a ``torch.cat``
                     -- the k-serial-lookups-plus-concat structure the paper starts from,
@@ -91,6 +93,12 @@ def run_point(cfg, n_iter: int = 200, rotating: int = 4, with_torch: bool = True
     res["input_first"] = _time_calls(lambda: plan.lookup_input_first(dt.ptrs, nxt().indices, out, pooling=pooling, stream=stream),
                                      stream, max(20, n_iter // 4))
 
+    res["alg1_direct"] = _time_calls(lambda: plan.lookup_onehot(dt.ptrs, nxt().indices, out, stream=stream), stream, n_iter)
+    res["alg1_direct_graph_us"] = _time_graph(lambda i, s: plan.lookup_onehot(dt.ptrs, batches[i % rotating].indices, out, stream=s),
+                                              stream, n_iter)
+    res["lookup_graph_us"] = _time_graph(lambda i, s: plan.lookup(dt.ptrs, batches[i % rotating].indices, out, pooling=pooling, stream=s),
+                                         stream, n_iter)
+
     def step(i, s):
         b = batches[i % rotating]
         plan.build(b.lengths, s)
@@ -150,8 +158,9 @@ def to_markdown(results: Dict[str, List[dict]]) -> str:
     for name, pts in results.items():
         lines += [f"## {name}", "",
                   "| " + pts[0]["axis"] + " | T | B | D | alg. MB | output-first us (avg / min) | GB/s | input-first us | GB/s | "
-                  "input/output | plan+lookup graph us | stream us | per-table torch us | per-table/ours(stream) |",
-                  "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
+                  "input/output | plan+lookup graph us | stream us | per-table torch us | per-table/ours(stream) | "
+                  "lookup only, graph us | alg1 direct us (avg / min) | alg1 direct, graph us |",
+                  "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
         for p in pts:
             of, inf = p["output_first"], p["input_first"]
             pt = p.get("per_table", {}).get("avg_us")
@@ -159,7 +168,9 @@ def to_markdown(results: Dict[str, List[dict]]) -> str:
             lines.append(f"| {p['axis_value']} | {p['T']} | {p['B']} | {p['D']} | {p['algorithmic_MB']:.2f} | "
                          f"{of['avg_us']:.1f} / {of['min_us']:.1f} | {p['output_first_GBs']:.0f} | {inf['avg_us']:.1f} | "
                          f"{p['input_first_GBs']:.0f} | {inf['avg_us'] / of['avg_us']:.2f}x | {p['plan_plus_lookup_graph_us']:.1f} | "
-                         f"{st:.1f} | " + (f"{pt:.1f} | {pt / st:.1f}x |" if pt else "- | - |"))
+                         f"{st:.1f} | " + (f"{pt:.1f} | {pt / st:.1f}x |" if pt else "- | - |") +
+                         (f" {p['lookup_graph_us']:.1f} | {p['alg1_direct']['avg_us']:.1f} / {p['alg1_direct']['min_us']:.1f} | "
+                          f"{p['alg1_direct_graph_us']:.1f} |" if "alg1_direct" in p else " - | - | - |"))
         lines.append("")
     return "\n".join(lines)
 

@@ -371,3 +371,68 @@ def test_c5_full_size_sampled():
     if free < 90e9:
         pytest.fail(f"config 5 needs ~82 GB of tables; only {free / 1e9:.0f} GB free on this device")
     _sampled_full_size(W.C5, 4096)
+
+
+# --------------------------------------------------------------------------------------------------
+# dpi_lookup_onehot: Algorithm 1 itself, no built plan
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype,D", [("f32", 4), ("f32", 16), ("f32", 24), ("f32", 64), ("f32", 128), ("f16", 8), ("f16", 32),
+                                     ("bf16", 40), ("bf16", 64), ("bf16", 256)])
+@pytest.mark.parametrize("B,T", [(1, 1), (5, 3), (333, 26), (2049, 7)])
+def test_lookup_onehot_is_alg1_bit_exact(dtype, D, B, T):
+    rows = tuple(int(r) for r in (np.arange(T) * 37 % 211 + 1))
+    cfg = W.Config("oh", T, rows, D, dtype, B, ("const", 1), ("uniform",), "sum", 3)
+    host_tables = [W.full_table_storage(cfg, t, rows[t]) for t in range(T)]
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, np.asarray(rows, np.int64))
+    ids = batch.indices.reshape(B, T)
+    plan = harness.make_plan(cfg, dt.rows, batch.N)          # never built: Alg. 1 needs no plan
+    out = harness.new_output(cfg, fill_nan=True)
+    plan.lookup_onehot(dt.ptrs, torch.from_numpy(batch.indices).cuda(), out)
+    torch.cuda.synchronize()
+    want = oracle.alg1_onehot(host_tables, W.DTYPE_CODE[dtype], ids)
+    assert np.array_equal(harness.out_to_f64(out), want)
+    plan.destroy()
+
+
+def test_lookup_onehot_c2_full_size_int64_ids_and_equals_the_planned_path():
+    cfg = W.C2
+    dt = harness.make_device_tables(cfg)
+    batch = W.make_batch(cfg, dt.rows)
+    host_tables = [W.full_table_storage(cfg, t, int(dt.rows[t])) for t in range(cfg.T)]
+    want = oracle.alg1_onehot(host_tables, oracle.F32, batch.indices.reshape(cfg.B, cfg.T))
+    planned = _run_gpu(cfg, dt, batch, cfg.pooling_modes())
+    assert np.array_equal(planned, want)
+    plan = harness.make_plan(cfg, dt.rows, batch.N)
+    out = harness.new_output(cfg, fill_nan=True)
+    plan.lookup_onehot(dt.ptrs, torch.from_numpy(batch.indices).cuda(), out)
+    torch.cuda.synchronize()
+    assert np.array_equal(harness.out_to_f64(out), want)
+    plan.set_layout(binding.BAGS_SAMPLE_MAJOR, binding.IDX_I64)
+    out.fill_(float("nan"))
+    plan.lookup_onehot(dt.ptrs, torch.from_numpy(batch.indices.astype(np.int64)).cuda(), out)
+    torch.cuda.synchronize()
+    assert np.array_equal(harness.out_to_f64(out), want)
+    plan.destroy()
+
+
+def test_lookup_onehot_rejects_what_it_does_not_cover():
+    cfg = W.Config("ohv", 2, (10, 10), 16, "bf16", 4, ("const", 1), ("uniform",), "sum", 3)
+    dt = harness.make_device_tables(cfg)
+    ids = torch.zeros(8, dtype=torch.int32, device="cuda")
+    out = harness.new_output(cfg)
+    plan = harness.make_plan(cfg, dt.rows, 8)
+    plan.set_out_dtype(W.DTYPE_CODE["f32"])
+    with pytest.raises(binding.DpiError) as e:
+        plan.lookup_onehot(dt.ptrs, ids, out)
+    assert e.value.status == 2
+    plan.set_out_dtype(W.DTYPE_CODE["bf16"])
+    plan.set_layout(binding.BAGS_TABLE_MAJOR, binding.IDX_I32)
+    with pytest.raises(binding.DpiError):
+        plan.lookup_onehot(dt.ptrs, ids, out)
+    plan.set_layout(binding.BAGS_SAMPLE_MAJOR, binding.IDX_I32)
+    with pytest.raises(binding.DpiError):
+        plan.lookup_onehot(dt.ptrs, None, out)
+    plan.lookup_onehot(dt.ptrs, ids, out)
+    torch.cuda.synchronize()
+    plan.destroy()
