@@ -436,3 +436,80 @@ def test_lookup_onehot_rejects_what_it_does_not_cover():
     plan.lookup_onehot(dt.ptrs, ids, out)
     torch.cuda.synchronize()
     plan.destroy()
+
+
+# --------------------------------------------------------------------------------------------------
+# maximum sizes of the boundary (include/dpi.h): T = DPI_MAX_TABLES, table_rows = 2^31 - 1, 512-byte rows
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 0, 3)])
+def test_max_table_count_2048(lengths):
+    """DPI_MAX_TABLES tables: the per-table pointer block in shared memory (16 KB), the 2048-bit pooling mask passed by
+    value, the table id stepping across bags; B = 3 keeps the oracle quick. Mixed sum / mean pooling."""
+    T = 2048
+    rows = tuple(int(r) for r in (np.arange(T) * 7 % 13 + 1))
+    cfg = W.Config("t2048", T, rows, 16, "f32", 3, lengths, ("uniform",), "half", seed=21)
+    _full_parity(cfg)
+    _full_parity(cfg.scaled(dtype="bf16", D=8, out_dtype="f32"), K=64)
+    if lengths[0] == "const":       # Alg. 1 plan-free kernel at the same table count
+        host_tables = [W.full_table_storage(cfg, t, rows[t]) for t in range(T)]
+        dt = harness.tables_from_host(cfg, host_tables)
+        batch = W.make_batch(cfg, np.asarray(rows, np.int64))
+        plan = harness.make_plan(cfg, dt.rows, batch.N)
+        out = harness.new_output(cfg, fill_nan=True)
+        plan.lookup_onehot(dt.ptrs, torch.from_numpy(batch.indices).cuda(), out)
+        torch.cuda.synchronize()
+        assert np.array_equal(harness.out_to_f64(out), oracle.alg1_onehot(host_tables, oracle.F32, batch.indices.reshape(3, T)))
+        plan.destroy()
+
+
+def test_one_table_more_than_the_limit_is_refused():
+    with pytest.raises(binding.DpiError) as e:
+        binding.Plan([5] * 2049, np.full(2049, 16, np.int32), 0, 2, 10)
+    assert e.value.status == 2
+
+
+def test_max_table_height_row_ids_up_to_2_pow_31_minus_2():
+    """One table of 2^31 - 1 rows x 16 B (34 GB): row ids need all 31 bits and byte offsets 35 bits. Only the referenced
+    rows are given values on the device; the oracle sees the same rows compacted (ids remapped), so nothing it reads
+    comes from the CUDA path. A second, small table checks the column block order next to it."""
+    n_big = 2 ** 31 - 1
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40 * 2 ** 30:
+        pytest.skip("needs 40 GB of free device memory")
+    D, B, T = 4, 64, 2
+    big = torch.empty((n_big, D), dtype=torch.float32, device="cuda")      # uninitialised except the referenced rows
+    small32 = W.dense_values_f32(3, 1, (10, D), 0.05)
+    small = torch.from_numpy(small32).cuda()
+    h = W.hash_u64(W.stream_key(8, W.STREAM_DENSE, 0), np.arange(3 * B, dtype=np.uint64))
+    ids_big = (h % np.uint64(n_big)).astype(np.int64)
+    ids_big[:6] = [0, 1, n_big - 1, n_big - 2, 2 ** 30, 2 ** 31 - 4097]     # the corners
+    uniq, inv = np.unique(ids_big, return_inverse=True)
+    vals32 = W.dense_values_f32(3, 2, (uniq.shape[0], D), 0.05)
+    big[torch.from_numpy(uniq).cuda()] = torch.from_numpy(vals32).cuda()
+    lengths = np.tile(np.array([3, 2], np.int32), B)                      # bag (b, big) has 3 entries, (b, small) 2
+    ids_small = (W.hash_u64(W.stream_key(8, W.STREAM_DENSE, 1), np.arange(2 * B, dtype=np.uint64)) % np.uint64(10)).astype(np.int64)
+    gpu_idx = np.empty(5 * B, np.int32)
+    ora_idx = np.empty(5 * B, np.int32)
+    for b in range(B):
+        gpu_idx[5 * b: 5 * b + 3] = ids_big[3 * b: 3 * b + 3]
+        ora_idx[5 * b: 5 * b + 3] = inv[3 * b: 3 * b + 3]
+        gpu_idx[5 * b + 3: 5 * b + 5] = ora_idx[5 * b + 3: 5 * b + 5] = ids_small[2 * b: 2 * b + 2]
+    ptrs = torch.tensor([big.data_ptr(), small.data_ptr()], dtype=torch.int64, device="cuda")
+    pooling = np.array([1, 0], np.uint8)
+    plan = binding.Plan([n_big, 10], np.array([D, D], np.int32), 0, B, 5 * B)
+    plan.build(torch.from_numpy(lengths).cuda())
+    idx_dev = torch.from_numpy(gpu_idx).cuda()
+    assert plan.check_indices(idx_dev) == 0
+    out = torch.full((B, T * D), float("nan"), device="cuda")
+    plan.lookup(ptrs, idx_dev, out, pooling=pooling)
+    torch.cuda.synchronize()
+    ref = oracle_reference([vals32, small32], "f32", B, lengths, ora_idx, pooling)
+    assert_outputs_match(harness.out_to_f64(out), ref, lengths, T, D, "f32")
+    plan.destroy()
+    del big
+
+
+def test_widest_rows_512_bytes_full_warp_per_row():
+    cfg = W.Config("w512", 3, (300, 5, 2000), 128, "f32", 515, ("poisson", 9.0, 60, 0.1), ("zipf", 1.05), "half", seed=5)
+    _full_parity(cfg)
+    _full_parity(cfg.scaled(dtype="f16", D=256, out_dtype="f32"))

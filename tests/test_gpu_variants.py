@@ -241,3 +241,13 @@ def test_set_columns_validation_and_reset():
     plan.set_columns(None)
     assert plan.plan_out_width() == 24
     plan.destroy()
+
+
+def test_general_kernel_at_the_maximum_table_count():
+    """T = DPI_MAX_TABLES with mixed dims, weights and int64 ids: 32 KB of per-table records + the per-warp staging
+    exceed the default 48 KB of dynamic shared memory, so this also covers the opt-in path of the launch."""
+    T = 2048
+    dims = [8 if t % 3 else 16 for t in range(T)]
+    rows = [int(t * 5 % 11 + 1) for t in range(T)]
+    _run(dims, rows, 3, "bf16", ("uniform", 0, 3), out_dtype="f32", idx64=True, weighted=True, K=64)
+    _run([d // 2 for d in dims], rows, 2, "f32", ("const", 1), table_major=True, pooling=[t & 1 for t in range(T)])
