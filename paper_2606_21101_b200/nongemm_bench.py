@@ -206,13 +206,37 @@ def bench_launcher(lines):
     lines.append("")
 
 
+def profile_pass():
+    """Three plain launches of each operator at a 65 536-row shape (no graphs, no timing): the target of an
+    `ncu --set full -k regex:"fm_kernel|cross_combine|bias_act"` capture."""
+    B, T, D, F = 65536, 8, 64, 512
+    x = [dense(1, r, (B, T * D), "f32") for r in range(3)]
+    y = torch.empty((B,), device="cuda")
+    x0, xl, u = (dense(2 + i, 0, (B, F), "f32") for i in range(3))
+    out = torch.empty((B, F), device="cuda")
+    bias = torch.from_numpy(W.dense_values_f32(5, 0, (F,), 1.0)).cuda()
+    for r in range(3):
+        nongemm.fm_interaction(x[r], 0, B, T, D, y=y)
+    for r in range(3):
+        nongemm.cross_combine(x0, xl, u, bias, out, 0, B, F)
+    for r in range(3):
+        nongemm.bias_act(u, bias, out, 0, B, F, nongemm.ACT_RELU)
+    for r in range(3):
+        nongemm.bias_act(u, bias, out, 0, B, F, nongemm.ACT_SIGMOID)
+    torch.cuda.synchronize()
+    print("profile pass done: 3 launches each of fm_kernel, cross_combine_kernel, bias_act_kernel (relu, sigmoid)")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default="")
     ap.add_argument("--skip-launcher", action="store_true")
+    ap.add_argument("--profile", action="store_true", help="only launch each operator three times (for ncu)")
     args = ap.parse_args()
     harness.require_cuda()
     torch.cuda.set_device(0)
+    if args.profile:
+        return profile_pass()
     lines = ["# NEXT-4 measurements (python -m paper_2606_21101_b200.nongemm_bench)", "",
              f"Device: {torch.cuda.get_device_name(0)}. CUDA events on the launching stream, after warm-up. Synthetic seeded inputs.", ""]
     bench_operators(lines)
