@@ -66,6 +66,8 @@ def _load():
         lib.oracle_cross_combine.restype = ctypes.c_int
         lib.oracle_bias_act.argtypes = [i32, i32, vp, vp, ctypes.c_int, vp]
         lib.oracle_bias_act.restype = ctypes.c_int
+        lib.oracle_lr_first_order.argtypes = [i32, i32, vp, vp, vp, vp, ctypes.c_double, vp]
+        lib.oracle_lr_first_order.restype = ctypes.c_int
         lib.oracle_bfs_queue.argtypes = [i32, i32, vp, vp]
         lib.oracle_bfs_queue.restype = ctypes.c_int
         _lib = lib
@@ -236,6 +238,22 @@ def bias_act(u, bias=None, act: int = ACT_RELU) -> np.ndarray:
     _check(_load().oracle_bias_act(B, F, u.ctypes.data, None if bias is None else bias.ctypes.data, int(act),
                                    out.ctypes.data))
     return out
+
+
+def lr_first_order(weights: Sequence[np.ndarray], B: int, indices: np.ndarray, offsets=None, bias: float = 0.0) -> np.ndarray:
+    """DeepFM first-order (logistic-regression) term (DESIGN.md 11.4 N7): weights[t] is float64[rows_t]; sample-major CSR
+    bags as in lookup(); offsets=None means one-hot. Returns float64[B]."""
+    keep = [np.ascontiguousarray(w, dtype=np.float64).reshape(-1) for w in weights]
+    T = len(keep)
+    ptrs = (ctypes.c_void_p * T)(*[a.ctypes.data for a in keep])
+    rows = np.asarray([a.shape[0] for a in keep], dtype=np.int64)
+    indices = np.ascontiguousarray(indices, dtype=np.int32)
+    off = None if offsets is None else np.ascontiguousarray(offsets, dtype=np.int32)
+    y = np.empty(B, dtype=np.float64)
+    _check(_load().oracle_lr_first_order(B, T, ctypes.cast(ptrs, ctypes.c_void_p), rows.ctypes.data, indices.ctypes.data,
+                                         None if off is None else off.ctypes.data, float(bias), y.ctypes.data))
+    del keep
+    return y
 
 
 def bfs_queue(n_explicit: int, n_implicit: int):

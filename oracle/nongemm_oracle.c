@@ -13,6 +13,8 @@
  *                              pairwise, not the square-of-sum rearrangement the GPU kernel uses)
  *       oracle_cross_combine   out = x0 * (u + bias) + xl                     (DCNv2 layer, u = W xl from the GEMM)
  *       oracle_bias_act        out = act(u + bias), act in {identity, relu, sigmoid}
+ *       oracle_lr_first_order  y[b] = bias + sum_t sum_{j in bag(b,t)} w_t[indices[j]]   (DeepFM's logistic-regression
+ *                              part: "table lookup ... and reduce-sum"; N7)
  *   - Algorithm 2 "Breadth-first Stream Scheduling", step by step in the paper's order:
  *       oracle_bfs_queue
  * Arithmetic: float64 throughout, results unrounded.
@@ -22,7 +24,8 @@
  * permutation, degree-2 homogeneity, hand-worked fixture tests/golden/nongemm_examples.txt.  Cross -- W = 0, b = 0 is
  * the identity layer; x0 = 0 gives xl; the scalar recurrence x_{l+1} = x0 (w x_l + b) + x_l in exact rationals;
  * fixture.  bias_act -- relu is idempotent and equals (v + |v|)/2; sigmoid(0) = 1/2, sigmoid(-v) = 1 - sigmoid(v),
- * scipy.special.expit.  BFS queue -- the three hand-expanded cases of Algorithm 2 in the fixture, alternation,
+ * scipy.special.expit.  LR -- constant weights give bias + kappa * (entries of the sample), one-hot is numpy take + sum,
+ * equality with the (separately pinned) oracle_lookup on width-1 tables summed over the row, hand fixture.  BFS queue -- the three hand-expanded cases of Algorithm 2 in the fixture, alternation,
  * longer-module-first, per-module order preserved, every op exactly once.
  */
 #include <stdint.h>
@@ -87,6 +90,31 @@ int oracle_bias_act(int32_t B, int32_t F, const double *u, const double *bias, i
             else if (act == NG_ACT_SIGMOID) s = 1.0 / (1.0 + exp(-s));
             out[i] = s;
         }
+    return NG_OK;
+}
+
+/*
+ * DeepFM logistic-regression (first-order) term (DESIGN.md 11.4 N7): one scalar weight per feature,
+ *   y[b] = bias + sum_t sum_{j in [offsets[b*T+t], offsets[b*T+t+1])} w_t[indices[j]]
+ * Bags are sample-major CSR exactly as in oracle_lookup; offsets == NULL means one-hot (bag g is entry g).
+ */
+int oracle_lr_first_order(int32_t B, int32_t T, const double *const *w, const int64_t *table_rows,
+                          const int32_t *indices, const int32_t *offsets, double bias, double *y)
+{
+    if (B < 0 || T <= 0 || !w || !table_rows || !y) return NG_BAD_ARG;
+    for (int32_t b = 0; b < B; ++b) {
+        double acc = bias;
+        for (int32_t t = 0; t < T; ++t) {
+            int64_t g = (int64_t)b * T + t;
+            int64_t lo = offsets ? offsets[g] : g, hi = offsets ? offsets[g + 1] : g + 1;
+            for (int64_t j = lo; j < hi; ++j) {
+                int64_t r = indices[j];
+                if (r < 0 || r >= table_rows[t]) return NG_BAD_ARG;
+                acc += w[t][r];
+            }
+        }
+        y[b] = acc;
+    }
     return NG_OK;
 }
 

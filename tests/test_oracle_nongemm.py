@@ -156,6 +156,50 @@ def test_sigmoid_against_library_and_symmetry():
     assert oracle.bias_act(np.zeros((1, 1)), None, oracle.ACT_SIGMOID)[0, 0] == 0.5
 
 
+# ---------------------------------------------------------------------------------------------------------------
+# DeepFM first-order (logistic regression) term
+# ---------------------------------------------------------------------------------------------------------------
+LR_W = [np.array([1.0, 2, 3]), np.array([10.0, 20]), np.array([100.0, 200, 300, 400])]
+
+
+def test_lr_hand_worked_fixture():
+    ln = np.array(GOLD["lr.lengths"]).reshape(-1).astype(np.int64)
+    idx = np.concatenate([np.array(r) for r in GOLD["lr.indices"]]).astype(np.int32)
+    off = np.concatenate(([0], np.cumsum(ln))).astype(np.int32)
+    assert np.array_equal(oracle.lr_first_order(LR_W, 2, idx, off, bias=0.5), np.array(GOLD["lr.y"][0]))
+    ids = np.array(GOLD["lr.onehot_ids"]).reshape(-1).astype(np.int32)
+    assert np.array_equal(oracle.lr_first_order(LR_W, 2, ids, None, bias=0.5), np.array(GOLD["lr.onehot_y"][0]))
+
+
+def test_lr_closed_forms_and_library_routines():
+    rng = np.random.default_rng(7)
+    T, B = 6, 40
+    rows = [5, 1, 300, 17, 64, 9]
+    ln = rng.integers(0, 5, size=B * T)
+    off = np.concatenate(([0], np.cumsum(ln))).astype(np.int32)
+    idx = np.concatenate([rng.integers(0, rows[g % T], size=ln[g]) for g in range(B * T)]).astype(np.int32)
+    # constant weights kappa_t = 2^t: y = bias + sum_t 2^t * len(b, t), exactly
+    w = [np.full(rows[t], 2.0 ** t) for t in range(T)]
+    y = oracle.lr_first_order(w, B, idx, off, bias=-3.0)
+    assert np.array_equal(y, -3.0 + (ln.reshape(B, T) * 2.0 ** np.arange(T)).sum(axis=1))
+    # integer weights: numpy take + add.reduceat-free brute force in Python ints
+    wi = [rng.integers(-50, 51, size=rows[t]).astype(np.float64) for t in range(T)]
+    y = oracle.lr_first_order(wi, B, idx, off)
+    for b in range(B):
+        tot = 0
+        for t in range(T):
+            g = b * T + t
+            tot += int(sum(int(wi[t][r]) for r in idx[off[g]:off[g + 1]]))
+        assert y[b] == tot
+    # one-hot: numpy take per table, summed over tables
+    ids = np.stack([rng.integers(0, rows[t], size=B) for t in range(T)], axis=1).astype(np.int32)
+    y1 = oracle.lr_first_order(wi, B, ids.reshape(-1), None, bias=1.0)
+    assert np.array_equal(y1, 1.0 + sum(np.take(wi[t], ids[:, t]) for t in range(T)))
+    # the same thing through the separately pinned pooled lookup: width-1 tables, sum pooling, then a row sum
+    ref = oracle.lookup([w_.astype(np.float32).reshape(-1, 1) for w_ in wi], oracle.F32, B, idx, off, np.zeros(T, np.uint8))
+    assert np.array_equal(y, ref.sum(axis=1))
+
+
 def test_bad_arguments_are_rejected():
     with pytest.raises(oracle.OracleError):
         oracle.bias_act(np.zeros((1, 1)), None, 7)
