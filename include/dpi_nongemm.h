@@ -56,6 +56,21 @@ dpi_status_t dpi_fm_interaction(const void* x_dev, dpi_dtype_t dtype, int32_t B,
 dpi_status_t dpi_cross_combine(const void* x0_dev, const void* xl_dev, const void* u_dev, const float* bias_dev,
                                void* out_dev, dpi_dtype_t dtype, int32_t B, int32_t F, void* stream);
 
+/*
+ * dpi_lr_first_order -- DeepFM's logistic-regression (first-order) term, "table lookup ... and reduce-sum"
+ * (DESIGN.md 11.4 N7): one scalar weight per feature,
+ *     y[b] = bias + sum_t sum_{j in bag(b,t)} w_t[indices[j]]          (or y[b] += ... when accumulate != 0)
+ * fused into ONE launch (T lookups + T-way reduce-sum + bias): one warp per sample, lanes over its T bags.
+ *   w_ptrs_dev   device array of T device pointers, w_ptrs_dev[t] = fp32[table_rows[t]]
+ *   indices_dev  device int32, sample-major CSR bags exactly as dpi_lookup reads them (per-table local ids, range is a
+ *                precondition); offsets_dev device int32[B*T+1] (e.g. the plan's, dpi_plan_device_views), or NULL for
+ *                one-hot input (bag g is entry g: indices_dev = IDs[B*T])
+ *   y_dev        device fp32[B]; accumulate != 0 adds to what is there (e.g. the FM term), bias included once
+ * fp32 accumulation; an empty sample gives bias.
+ */
+dpi_status_t dpi_lr_first_order(const void* const* w_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,
+                                int32_t B, int32_t T, float bias, float* y_dev, int32_t accumulate, void* stream);
+
 typedef enum { DPI_ACT_IDENTITY = 0, DPI_ACT_RELU = 1, DPI_ACT_SIGMOID = 2 } dpi_act_t;
 
 /*

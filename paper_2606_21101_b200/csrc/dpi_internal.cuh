@@ -120,6 +120,8 @@ void count_launch();
 // ---- NEXT-4: non-GEMM consumers of X_embed (nongemm_kernels.cu; boundary in include/dpi_nongemm.h) ---------
 cudaError_t launch_fm(const void* x, int dtype, uint32_t B, uint32_t T, uint32_t D, uint64_t x_pitch_bytes, float* y,
                       float* v, cudaStream_t st);
+cudaError_t launch_lr(const void* const* w, const int32_t* indices, const int32_t* offsets, uint32_t B, uint32_t T, float bias,
+                      float* y, int accumulate, cudaStream_t st);
 cudaError_t launch_cross_combine(const void* x0, const void* xl, const void* u, const float* bias, void* out, int dtype,
                                  uint32_t B, uint32_t F, cudaStream_t st);
 cudaError_t launch_bias_act(const void* u, const float* bias, void* out, int dtype, uint32_t B, uint32_t F, int act,

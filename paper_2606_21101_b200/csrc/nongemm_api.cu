@@ -48,6 +48,20 @@ dpi_status_t dpi_fm_interaction(const void* x_dev, dpi_dtype_t dtype, int32_t B,
                        "fm_kernel launch");
 }
 
+dpi_status_t dpi_lr_first_order(const void* const* w_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,
+                                int32_t B, int32_t T, float bias, float* y_dev, int32_t accumulate, void* stream) {
+    if (!w_ptrs_dev || !indices_dev || !y_dev) return report_error(DPI_ERR_INVALID_ARG, "dpi_lr_first_order: NULL pointer");
+    if (B < 0 || T <= 0) return report_error(DPI_ERR_INVALID_ARG, "dpi_lr_first_order: B=%d T=%d", B, T);
+    if ((reinterpret_cast<uintptr_t>(w_ptrs_dev) & 7u) || (reinterpret_cast<uintptr_t>(indices_dev) & 3u) ||
+        (reinterpret_cast<uintptr_t>(offsets_dev) & 3u) || (reinterpret_cast<uintptr_t>(y_dev) & 3u))
+        return report_error(DPI_ERR_INVALID_ARG, "dpi_lr_first_order: misaligned pointer");
+    if (static_cast<int64_t>(B) * T > 0x7fffffffll) return report_error(DPI_ERR_UNSUPPORTED, "dpi_lr_first_order: B*T exceeds 2^31 - 1");
+    if (B == 0) return DPI_OK;
+    return cuda_status(launch_lr(w_ptrs_dev, indices_dev, offsets_dev, static_cast<uint32_t>(B), static_cast<uint32_t>(T), bias, y_dev,
+                                 accumulate != 0, static_cast<cudaStream_t>(stream)),
+                       "lr_kernel launch");
+}
+
 static dpi_status_t check_ew(const char* who, int dtype, int32_t B, int32_t F) {
     if (!dtype_ok(dtype)) return report_error(DPI_ERR_INVALID_ARG, "%s: bad dtype %d", who, dtype);
     if (B < 0 || F <= 0) return report_error(DPI_ERR_INVALID_ARG, "%s: B=%d F=%d", who, B, F);

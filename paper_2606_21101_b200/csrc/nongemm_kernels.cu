@@ -255,6 +255,42 @@ __global__ void __launch_bounds__(256) bias_act_kernel(const EwArgs a, const uin
     }
 }
 
+// ---- DeepFM first-order (logistic regression) term -------------------------------------------------------------------
+// One warp per sample; lane l owns bags t = l, l + 32, ... of the sample (their offsets are consecutive words, their
+// index entries consecutive runs), gathers the scalar weights of its bags and the warp tree-reduces. T lookups, the
+// T-way reduce-sum and the bias add of the framework graph in one launch.
+struct LrArgs {
+    const float* const* w;
+    const int32_t* indices;
+    const int32_t* offsets;  // NULL: one-hot
+    float* y;
+    float bias;
+    uint32_t B, T;
+    int accumulate;
+};
+
+__global__ void __launch_bounds__(256) lr_kernel(const LrArgs a) {
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t warps_per_cta = blockDim.x >> 5;
+    const uint32_t n_warps = gridDim.x * warps_per_cta;
+    for (uint32_t b = blockIdx.x * warps_per_cta + (threadIdx.x >> 5); b < a.B; b += n_warps) {
+        const size_t g0 = static_cast<size_t>(b) * a.T;
+        float acc = 0.f;
+        for (uint32_t t = lane; t < a.T; t += 32) {
+            const float* wt = reinterpret_cast<const float*>(__ldg(reinterpret_cast<const unsigned long long*>(a.w) + t));
+            if (a.offsets) {
+                const int lo = __ldg(a.offsets + g0 + t), hi = __ldg(a.offsets + g0 + t + 1);
+                for (int j = lo; j < hi; ++j) acc += __ldg(wt + static_cast<uint32_t>(__ldg(a.indices + j)));
+            } else {
+                acc += __ldg(wt + static_cast<uint32_t>(__ldg(a.indices + g0 + t)));
+            }
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+        if (lane == 0) a.y[b] = (a.accumulate ? a.y[b] : 0.f) + (a.bias + acc);
+    }
+}
+
 int pow2ceil_i(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 int log2_i(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
 
@@ -315,6 +351,17 @@ cudaError_t launch_fm(const void* x, int dtype, uint32_t B, uint32_t T, uint32_t
         case DPI_BF16: return launch_fm_dt<DPI_BF16>(a, W, st);
         default: return cudaErrorInvalidValue;
     }
+}
+
+cudaError_t launch_lr(const void* const* w, const int32_t* indices, const int32_t* offsets, uint32_t B, uint32_t T, float bias,
+                      float* y, int accumulate, cudaStream_t st) {
+    LrArgs a{reinterpret_cast<const float* const*>(w), indices, offsets, y, bias, B, T, accumulate};
+    const long long want = (static_cast<long long>(B) + 7) / 8;
+    const long long cap = static_cast<long long>(sm_count()) * 8 * 4;
+    const unsigned grid = static_cast<unsigned>(want < cap ? (want < 1 ? 1 : want) : cap);
+    count_launch();
+    lr_kernel<<<grid, 256, 0, st>>>(a);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_cross_combine(const void* x0, const void* xl, const void* u, const float* bias, void* out, int dtype,

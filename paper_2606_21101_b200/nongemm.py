@@ -13,7 +13,7 @@ import numpy as np
 from . import binding
 from .binding import _check, _ptr, _stream_handle
 
-EXPORTS = ["dpi_fm_interaction", "dpi_cross_combine", "dpi_bias_act", "dpi_bfs_schedule", "dpi_launcher_create",
+EXPORTS = ["dpi_fm_interaction", "dpi_lr_first_order", "dpi_cross_combine", "dpi_bias_act", "dpi_bfs_schedule", "dpi_launcher_create",
            "dpi_launcher_destroy", "dpi_launcher_run"]
 
 ACT_IDENTITY, ACT_RELU, ACT_SIGMOID = 0, 1, 2
@@ -38,6 +38,7 @@ def _lib() -> ctypes.CDLL:
         sig = {
             "dpi_fm_interaction": (st, [vp, ctypes.c_int, i32, i32, i32, i64, vp, vp, vp]),
             "dpi_cross_combine": (st, [vp, vp, vp, vp, vp, ctypes.c_int, i32, i32, vp]),
+            "dpi_lr_first_order": (st, [vp, vp, vp, i32, i32, ctypes.c_float, vp, i32, vp]),
             "dpi_bias_act": (st, [vp, vp, vp, ctypes.c_int, i32, i32, ctypes.c_int, vp]),
             "dpi_bfs_schedule": (st, [i32, i32, vp, vp]),
             "dpi_launcher_create": (st, [vp]),
@@ -56,6 +57,13 @@ def fm_interaction(x, dtype: int, B: int, T: int, D: int, y=None, v=None, x_ld: 
     """dpi_fm_interaction: x [B, x_ld] device tensor of `dtype`; y fp32[B] and / or v fp32[B, D] device tensors."""
     _check(_lib().dpi_fm_interaction(_ptr(x), int(dtype), int(B), int(T), int(D), int(x_ld), _ptr(y), _ptr(v),
                                      _stream_handle(stream)))
+
+
+def lr_first_order(w_ptrs, indices, offsets, B: int, T: int, bias: float, y, accumulate: bool = False, stream=None) -> None:
+    """dpi_lr_first_order: y[b] (+)= bias + sum of the scalar weights of sample b's entries. w_ptrs: device int64[T] of
+    pointers to fp32 weight vectors; indices int32 (CSR, sample-major); offsets int32[B*T+1] or None (one-hot)."""
+    _check(_lib().dpi_lr_first_order(_ptr(w_ptrs), _ptr(indices), _ptr(offsets), int(B), int(T), float(bias), _ptr(y),
+                                     int(bool(accumulate)), _stream_handle(stream)))
 
 
 def cross_combine(x0, xl, u, bias, out, dtype: int, B: int, F: int, stream=None) -> None:

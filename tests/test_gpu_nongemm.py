@@ -292,3 +292,84 @@ def test_launcher_is_graph_capturable():
     torch.cuda.synchronize()
     assert (a == 5).all() and (b == 15).all()
     L.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# DeepFM first-order (logistic regression) term
+# ---------------------------------------------------------------------------------------------------------------
+def _lr_problem(T, B, lengths, seed=17):
+    rows = tuple(int(r) for r in (np.arange(T) * 131 % 997 + 1))
+    cfg = W.Config("lr", T, rows, 4, "f32", B, lengths, ("zipf", 1.05), "sum", seed)
+    batch = W.make_batch(cfg, np.asarray(rows, np.int64))
+    w32 = [W.dense_values_f32(seed, 100 + t, (rows[t],), 0.5) for t in range(T)]
+    w_dev = [torch.from_numpy(w).cuda() for w in w32]
+    ptrs = torch.tensor([w.data_ptr() for w in w_dev], dtype=torch.int64, device="cuda")
+    return batch, w32, w_dev, ptrs
+
+
+@pytest.mark.parametrize("T,B", [(1, 1), (3, 5), (26, 1037), (39, 333), (100, 77)])
+@pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 0, 4), ("poisson", 20.0, 100, 0.05)])
+def test_lr_first_order_matches_the_oracle(T, B, lengths):
+    batch, w32, w_dev, ptrs = _lr_problem(T, B, lengths)
+    off = np.concatenate(([0], np.cumsum(batch.lengths.astype(np.int64)))).astype(np.int32)
+    idx_dev = torch.from_numpy(batch.indices if batch.N else np.zeros(1, np.int32)).cuda()
+    off_dev = torch.from_numpy(off).cuda()
+    y = torch.full((B,), float("nan"), device="cuda")
+    nongemm.lr_first_order(ptrs, idx_dev, off_dev, B, T, 0.25, y)
+    torch.cuda.synchronize()
+    w64 = [w.astype(np.float64) for w in w32]
+    ref = oracle.lr_first_order(w64, B, batch.indices, off, bias=0.25)
+    # fp32 sum of n terms in tree / lane order: |err| <= (n + 2) u sum|w| (+ the bias add)
+    n = batch.lengths.reshape(B, T).sum(axis=1)
+    absum = oracle.lr_first_order([np.abs(w) for w in w64], B, batch.indices, off, bias=0.25)
+    tol = (n + 2) * U32 * absum + 1e-30
+    got = f64(y)
+    assert not np.isnan(got).any()
+    assert (np.abs(got - ref) <= tol).all(), f"max err {np.abs(got - ref).max():.3e}"
+    if lengths[0] == "const":       # one-hot: the same numbers without offsets
+        y1 = torch.full((B,), float("nan"), device="cuda")
+        nongemm.lr_first_order(ptrs, idx_dev, None, B, T, 0.25, y1)
+        torch.cuda.synchronize()
+        assert torch.equal(y, y1)
+
+
+def test_lr_integer_weights_are_exact_and_accumulate_adds_onto_fm():
+    T, B, D = 26, 300, 16
+    batch, _, _, _ = _lr_problem(T, B, ("uniform", 0, 3))
+    rows = [int(r) for r in (np.arange(T) * 131 % 997 + 1)]
+    wi = [((np.arange(rows[t]) * 7 + t) % 41 - 20).astype(np.float32) for t in range(T)]
+    w_dev = [torch.from_numpy(w).cuda() for w in wi]
+    ptrs = torch.tensor([w.data_ptr() for w in w_dev], dtype=torch.int64, device="cuda")
+    off = np.concatenate(([0], np.cumsum(batch.lengths.astype(np.int64)))).astype(np.int32)
+    idx_dev, off_dev = torch.from_numpy(batch.indices).cuda(), torch.from_numpy(off).cuda()
+    y = torch.full((B,), float("nan"), device="cuda")
+    nongemm.lr_first_order(ptrs, idx_dev, off_dev, B, T, -3.0, y)
+    torch.cuda.synchronize()
+    ref = oracle.lr_first_order([w.astype(np.float64) for w in wi], B, batch.indices, off, bias=-3.0)
+    assert np.array_equal(f64(y), ref)                                   # small integers: every partial sum is exact
+    # DeepFM explicit module = FM + LR: FM writes y, LR accumulates onto it (integers again, so the sum is exact)
+    h = W.hash_u64(W.stream_key(5, W.STREAM_DENSE, 3), np.arange(B * T * D, dtype=np.uint64))
+    x = ((h % np.uint64(9)).astype(np.float32) - 4.0).reshape(B, T * D)
+    xd = torch.from_numpy(x).cuda()
+    nongemm.fm_interaction(xd, 0, B, T, D, y=y)
+    nongemm.lr_first_order(ptrs, idx_dev, off_dev, B, T, -3.0, y, accumulate=True)
+    torch.cuda.synchronize()
+    fm_ref, _ = oracle.fm_pairwise(x.astype(np.float64), T, D)
+    assert np.array_equal(f64(y), fm_ref + ref)
+
+
+def test_lr_all_empty_and_validation():
+    T, B = 4, 9
+    w_dev = [torch.ones(3, device="cuda") for _ in range(T)]
+    ptrs = torch.tensor([w.data_ptr() for w in w_dev], dtype=torch.int64, device="cuda")
+    off = torch.zeros(B * T + 1, dtype=torch.int32, device="cuda")
+    idx = torch.zeros(1, dtype=torch.int32, device="cuda")
+    y = torch.full((B,), float("nan"), device="cuda")
+    nongemm.lr_first_order(ptrs, idx, off, B, T, 1.5, y)
+    torch.cuda.synchronize()
+    assert (y == 1.5).all()
+    from paper_2606_21101_b200 import binding
+    with pytest.raises(binding.DpiError):
+        nongemm.lr_first_order(None, idx, off, B, T, 0.0, y)
+    with pytest.raises(binding.DpiError):
+        nongemm.lr_first_order(ptrs, idx, off, B, 0, 0.0, y)
