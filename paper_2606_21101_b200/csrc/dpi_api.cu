@@ -608,6 +608,19 @@ dpi_status_t dpi_plan_out_width(const dpi_plan_t* p, int64_t* width) {
 
 namespace {
 
+// Sum of lengths[g0, g1) and whether any of them is negative: branch-free so that the host compiler vectorises it (the
+// loop runs once per dpi_forward_host call over all G lengths; with an early return inside it cost 0.15 ms at G = 360 K).
+bool sum_lengths(const int32_t* lengths, size_t g0, size_t g1, int64_t* total) {
+    int64_t sum = 0;
+    int32_t sign = 0;
+    for (size_t g = g0; g < g1; ++g) {
+        sum += lengths[g];
+        sign |= lengths[g];
+    }
+    *total = sum;
+    return sign < 0;
+}
+
 int host_chunks(const dpi_plan_t* p, size_t bytes_moved) {
     if (p->bag_order == DPI_BAGS_TABLE_MAJOR) return 1;  // a chunk of samples is not a contiguous run of bags
     int n = p->opt[DPI_OPT_HOST_CHUNKS];
@@ -686,10 +699,7 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     const int n_chunks = host_chunks(p, static_cast<size_t>(p->G) * 4 + static_cast<size_t>(n_indices) * idx_elt + out_bytes);
     if (n_chunks <= 1) {
         int64_t total = 0;  // same host-side check as the pipelined path: the lengths must add up to n_indices
-        for (size_t g = 0; g < static_cast<size_t>(p->G); ++g) {
-            if (lengths_host[g] < 0) return fail(DPI_ERR_INVALID_ARG, "lengths_host[%zu] is negative", g);
-            total += lengths_host[g];
-        }
+        if (sum_lengths(lengths_host, 0, p->G, &total)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
         if (total != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)total);
         DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * idx_elt, cudaMemcpyHostToDevice, s));
@@ -715,10 +725,7 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     for (size_t c = 0; c < n_sub; ++c) {
         const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T, g1 = static_cast<size_t>(h->sample_lo[c + 1]) * p->T;
         int64_t n = 0;
-        for (size_t g = g0; g < g1; ++g) {
-            if (lengths_host[g] < 0) return fail(DPI_ERR_INVALID_ARG, "lengths_host[%zu] is negative", g);
-            n += lengths_host[g];
-        }
+        if (sum_lengths(lengths_host, g0, g1, &n)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
         entry_lo[c + 1] = entry_lo[c] + n;
     }
     if (entry_lo[n_sub] != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)entry_lo[n_sub]);
