@@ -431,7 +431,9 @@ def run_ours(args):
     peak, peak_src = measured_peak()
     lk_ms = statistics.mean(lookup_ms)
     achieved = bytes_step["lookup"] / (lk_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "lookup_kernel (a3 fused gather-and-pool)" if args.kernel == "output_first" else "input_first_kernel (ablation)", "achieved": achieved,
+    short_variant = args.kernel == "output_first" and (args.mode == 6 or (args.mode == 0 and 1 <= harness.max_bag_length(cfg) <= 8))
+    roofline = {"bound": "hbm", "kernel": ("direct_kernel (a3 fused gather-and-pool, short-bag variant)" if short_variant else
+                                           "lookup_kernel (a3 fused gather-and-pool)") if args.kernel == "output_first" else "input_first_kernel (ablation)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "frac_of_nominal_8000": achieved / 8000.0, "traffic": ncu_traffic(cfg.name),
                 "algorithmic_bytes_per_launch": bytes_step["lookup"], "kernel_ms_avg": lk_ms,
@@ -449,7 +451,11 @@ def run_ours(args):
         "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_KEY[cfg.dtype], "data": "synthetic",
         "config": describe(cfg, rows, {"parallelism": f"batch-sharded replicas x{world}, no collective",
                                        "launch": "CUDA graph replay of the K steps" if graph is not None else "stream launches",
-                                       "quantum_K": plan.info()["K"], "rows_gathered_per_step": n_mean,
+                                       "quantum_K": plan.info()["K"],
+                                       "max_bag_hint": harness.max_bag_length(cfg),
+                                       "lookup_variant": ("input-first ablation" if args.kernel == "input_first" else
+                                                          "short-bag (lane group per bag)" if (args.mode == 6 or (args.mode == 0 and 1 <= harness.max_bag_length(cfg) <= 8))
+                                                          else "balanced segments"), "rows_gathered_per_step": n_mean,
                                        "segments_per_step": s_mean}, R),
         "row_gathers_per_s": n_mean * steps * world / (total_ms * 1e-3),
         "step_algorithmic_gbs": bytes_step["total"] * world / (total_ms / steps * 1e-3) / 1e9,

@@ -78,7 +78,8 @@ typedef enum {
     DPI_OPT_BLOCK_THREADS = 1,  /* lookup CTA size: a multiple of 32 up to 256; 0 = auto */
     DPI_OPT_BLOCKS_PER_SM = 2,  /* persistent grid = SMs * this; 0 = auto (occupancy) */
     DPI_OPT_MODE = 3,           /* 0 auto per task, 1 sub-warp per bag, 2 warp per bag (single-buffered),
-                                   3 warp per bag (double-buffered batches) */
+                                   3 warp per bag (double-buffered batches), 6 short-bag variant (see
+                                   DPI_OPT_MAX_BAG_HINT) whatever the hint says */
     DPI_OPT_ROW_L1_NO_ALLOC = 4,/* reserved: accepts -1 / 0 only. Rows always allocate in L1; the L1::no_allocate
                                    variant measured 17-20 % slower on B200 and was removed */
     DPI_OPT_PDL = 5,            /* 1: lookup is launched with programmatic dependent launch after the planner */
@@ -90,6 +91,12 @@ typedef enum {
                                    straight into it over PCIe -- the device->host transfer is fused into the kernel's
                                    store, no staging block and no D2H copy. Auto uses it whenever out_host qualifies;
                                    2 returns DPI_ERR_INVALID_ARG if it does not. */
+    DPI_OPT_MAX_BAG_HINT = 8,   /* 0 = unknown (default). L >= 1: the caller's promise that no bag of the batches run with this
+                                   plan is longer than L (a schema fact in CTR serving: "at most 3 tags per item"). With
+                                   L <= 8 and DPI_OPT_MODE = 0 the dense layout runs the short-bag variant (one lane group
+                                   per bag straight from the plan's offsets, no segments; 12-17 % faster on c2 / c3) instead
+                                   of the balanced-segment kernel. A longer bag is still pooled correctly, only without
+                                   load balancing -- which is why this is a promise and not a guess from max_indices. */
     DPI_OPT_COUNT_
 } dpi_option_t;
 

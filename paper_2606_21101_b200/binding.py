@@ -19,7 +19,7 @@ STATUS_NAMES = {0: "DPI_OK", 1: "DPI_ERR_INVALID_ARG", 2: "DPI_ERR_UNSUPPORTED",
                 4: "DPI_ERR_CUDA", 5: "DPI_ERR_INDEX_RANGE"}
 DPI_F32, DPI_F16, DPI_BF16 = 0, 1, 2
 DPI_POOL_SUM, DPI_POOL_MEAN = 0, 1
-OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL, OPT_HOST_CHUNKS, OPT_HOST_DIRECT_OUT = range(8)
+OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL, OPT_HOST_CHUNKS, OPT_HOST_DIRECT_OUT, OPT_MAX_BAG_HINT = range(9)
 BAGS_SAMPLE_MAJOR, BAGS_TABLE_MAJOR = 0, 1
 IDX_I32, IDX_I64 = 0, 1
 LOOKUP_FORCE_GENERAL = 1

@@ -76,7 +76,7 @@ struct dpi_plan_s {
     int32_t K_user = 0;      // 0 = default
     uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
     uint32_t num_tiles = 0, num_chunks = 0, tiles_per_chunk = 0;
-    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0, 0, 0};
+    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 0, 0, 0, 0};
     // device
     int device = 0, num_sms = 0;
     int32_t* offsets = nullptr;
@@ -255,6 +255,13 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
         if (e != cudaSuccess) return cuda_fail(e, "input-first kernel launch");
         return DPI_OK;
     }
+    const int32_t hint = p->opt[DPI_OPT_MAX_BAG_HINT];
+    if (!general && (p->opt[DPI_OPT_MODE] == 6 || (p->opt[DPI_OPT_MODE] == 0 && hint >= 1 && hint <= 8))) {  // short-bag variant (lookup_direct.cu)
+        cudaError_t e = launch_direct(a, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->num_sms,
+                                      p->opt[DPI_OPT_PDL] != 0, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "direct lookup kernel launch");
+        return DPI_OK;
+    }
     const LookupLaunch l = choose_launch(p, a, general);
     cudaError_t e;
     switch (p->dtype) {
@@ -404,11 +411,12 @@ dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
         case DPI_OPT_UNROLL: ok = v == 0 || v == 2 || v == 4 || v == 8 || v == 16; break;
         case DPI_OPT_BLOCK_THREADS: ok = v == 0 || (v >= 32 && v <= 256 && v % 32 == 0); break;
         case DPI_OPT_BLOCKS_PER_SM: ok = v >= 0 && v <= 32; break;
-        case DPI_OPT_MODE: ok = v >= 0 && v <= 3; break;
+        case DPI_OPT_MODE: ok = (v >= 0 && v <= 3) || v == 6; break;
         case DPI_OPT_ROW_L1_NO_ALLOC: ok = v == -1 || v == 0; break;  // the bypass variant was removed (see dpi.h)
         case DPI_OPT_PDL: ok = v == 0 || v == 1; break;
         case DPI_OPT_HOST_CHUNKS: ok = v >= 0 && v <= 64; break;
         case DPI_OPT_HOST_DIRECT_OUT: ok = v >= 0 && v <= 2; break;
+        case DPI_OPT_MAX_BAG_HINT: ok = v >= 0; break;
         default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);
     }
     if (!ok) return fail(DPI_ERR_INVALID_ARG, "value %d not supported for option %d", v, (int)opt);

@@ -111,6 +111,9 @@ int lookup_occupancy_bf16(const LookupArgs& a, const LookupLaunch& l);
 // Ablation (ablation_input_first.cu): one thread per sample.
 cudaError_t launch_input_first(const LookupArgs& a, uint32_t B, int dtype, bool out32, cudaStream_t stream);
 
+// Short-bag variant of a3 (lookup_direct.cu): one lane group per bag straight from the plan's offsets, no segments.
+cudaError_t launch_direct(const LookupArgs& a, int dtype, bool out32, int lanes, int num_sms, bool pdl, cudaStream_t stream);
+
 // Algorithm 1, plan-free one-hot lookup (lookup_onehot.cu).
 cudaError_t launch_onehot(const void* const* tables, const void* ids, uint32_t idx_shift, void* out, uint32_t G, uint32_t T,
                           uint32_t nvec, int lanes, int num_sms, cudaStream_t stream);

@@ -103,10 +103,20 @@ def out_to_f64(out: torch.Tensor) -> np.ndarray:
     return out.detach().to("cpu").to(torch.float64).numpy()
 
 
-def make_plan(cfg: W.Config, rows: np.ndarray, max_indices: int) -> binding.Plan:
+def max_bag_length(cfg: W.Config) -> int:
+    """Longest bag the config's length recipe can draw (a schema fact, known before any batch exists)."""
+    kind = cfg.lengths[0]
+    return int(cfg.lengths[1]) if kind == "const" else int(cfg.lengths[2])
+
+
+def make_plan(cfg: W.Config, rows: np.ndarray, max_indices: int, bag_hint: bool = True) -> binding.Plan:
+    """bag_hint: pass the recipe's longest bag as DPI_OPT_MAX_BAG_HINT (the library then runs its short-bag variant when
+    that is <= 8: c1-c3; c4 / c5 keep the balanced-segment kernel)."""
     plan = binding.Plan(rows, cfg.D, W.DTYPE_CODE[cfg.dtype], cfg.B, max_indices)
     if cfg.out != cfg.dtype:
         plan.set_out_dtype(W.DTYPE_CODE[cfg.out])
+    if bag_hint:
+        plan.set_option(binding.OPT_MAX_BAG_HINT, max(max_bag_length(cfg), 0))
     return plan
 
 

@@ -100,7 +100,10 @@ def test_plan_overflow_is_reported_not_out_of_bounds():
 # --------------------------------------------------------------------------------------------------
 def _run_gpu(cfg, dt, batch, pooling, K=0, opts=None, via_explicit_offsets=False, input_first=False):
     db = harness.upload_batch(batch)
-    plan = harness.make_plan(cfg, dt.rows, max(batch.N, 1))
+    # no bag-length hint by default: these tests are about the balanced-segment kernel on every bag shape; the short-bag
+    # variant has its own tests (mode 6 / DPI_OPT_MAX_BAG_HINT) further down
+    plan = harness.make_plan(cfg, dt.rows, max(batch.N, 1), bag_hint=bool((opts or {}).get("bag_hint", False)))
+    opts = {k: v for k, v in (opts or {}).items() if k != "bag_hint"}
     if K:
         plan.set_quantum(K)
     for k, v in (opts or {}).items():
@@ -513,3 +516,41 @@ def test_widest_rows_512_bytes_full_warp_per_row():
     cfg = W.Config("w512", 3, (300, 5, 2000), 128, "f32", 515, ("poisson", 9.0, 60, 0.1), ("zipf", 1.05), "half", seed=5)
     _full_parity(cfg)
     _full_parity(cfg.scaled(dtype="f16", D=256, out_dtype="f32"))
+
+
+# --------------------------------------------------------------------------------------------------
+# DPI_OPT_MODE = 6: the short-bag variant (one lane group per bag straight from the plan's offsets, lookup_direct.cu)
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype,D,out", [("f32", 4, None), ("f32", 16, None), ("f32", 24, None), ("f32", 64, None), ("f32", 128, None),
+                                         ("f16", 8, None), ("f16", 32, None), ("f16", 72, "f32"), ("bf16", 64, "f32"),
+                                         ("bf16", 256, None)])
+@pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 0, 3), ("uniform", 1, 4), ("poisson", 20.0, 100, 0.05),
+                                     ("const", 0)])
+def test_direct_short_bag_variant_matches_the_oracle(dtype, D, out, lengths):
+    """Same contract as the default kernel (tolerances of tests/parity.py, bit-exact for bags of length <= 1, +0.0 for empty
+    bags), several tiles and a ragged tail; the Poisson(20) case checks that long bags are still correct here."""
+    cfg = W.Config("d", 5, (1000, 17, 4000, 1, 250), D, dtype, 333, lengths, ("zipf", 1.05), "half", seed=12, out_dtype=out)
+    _full_parity(cfg, opts={binding.OPT_MODE: 6})
+
+
+def test_direct_short_bag_variant_full_size_c3_c2_c1_and_degenerate_shapes():
+    _full_parity(W.C3, opts={binding.OPT_MODE: 6})
+    _full_parity(W.C2, opts={binding.OPT_MODE: 6})
+    _full_parity(W.C1, opts={binding.OPT_MODE: 6})
+    _full_parity(W.Config("dl", 2, (1000, 50), 64, "f32", 3, ("const", 5000), ("uniform",), "mean", 0), opts={binding.OPT_MODE: 6})
+    _full_parity(W.Config("d1", 100, ("loguniform", 10, 1000), 16, "bf16", 1, ("uniform", 0, 3), ("uniform",), "half", 2),
+                 opts={binding.OPT_MODE: 6})
+    T = 2048
+    rows = tuple(int(r) for r in (np.arange(T) * 7 % 13 + 1))
+    _full_parity(W.Config("dt", T, rows, 16, "f32", 3, ("uniform", 0, 3), ("uniform",), "half", seed=21), opts={binding.OPT_MODE: 6})
+
+
+def test_bag_length_hint_selects_the_short_bag_variant_and_a_broken_promise_is_still_correct():
+    """DPI_OPT_MAX_BAG_HINT is a promise about bag lengths; it only selects the kernel. c3 with its true bound (3), a config
+    whose bags are far longer than the promised 2 (correct, just not load-balanced), and a hint above 8 (planned kernel)."""
+    _full_parity(W.C3, opts={"bag_hint": True})
+    cfg = W.Config("hp", 3, (100, 1000, 10), 32, "f16", 500, ("poisson", 6.0, 40, 0.2), ("zipf", 1.2), "mean", 4)
+    _full_parity(cfg, opts={binding.OPT_MAX_BAG_HINT: 2})
+    _full_parity(cfg, opts={binding.OPT_MAX_BAG_HINT: 40})
+    with pytest.raises(binding.DpiError):
+        binding.Plan([5], 16, 0, 4, 10).set_option(binding.OPT_MAX_BAG_HINT, -1)
