@@ -431,7 +431,7 @@ def run_ours(args):
     peak, peak_src = measured_peak()
     lk_ms = statistics.mean(lookup_ms)
     achieved = bytes_step["lookup"] / (lk_ms * 1e-3) / 1e9
-    short_variant = args.kernel == "output_first" and (args.mode == 6 or (args.mode == 0 and 1 <= harness.max_bag_length(cfg) <= 8))
+    short_variant = args.kernel == "output_first" and harness.lookup_variant(cfg, args.mode).startswith("short-bag")
     roofline = {"bound": "hbm", "kernel": ("direct_kernel (a3 fused gather-and-pool, short-bag variant)" if short_variant else
                                            "lookup_kernel (a3 fused gather-and-pool)") if args.kernel == "output_first" else "input_first_kernel (ablation)", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
@@ -454,8 +454,7 @@ def run_ours(args):
                                        "quantum_K": plan.info()["K"],
                                        "max_bag_hint": harness.max_bag_length(cfg),
                                        "lookup_variant": ("input-first ablation" if args.kernel == "input_first" else
-                                                          "short-bag (lane group per bag)" if (args.mode == 6 or (args.mode == 0 and 1 <= harness.max_bag_length(cfg) <= 8))
-                                                          else "balanced segments"), "rows_gathered_per_step": n_mean,
+                                                          harness.lookup_variant(cfg, args.mode)), "rows_gathered_per_step": n_mean,
                                        "segments_per_step": s_mean}, R),
         "row_gathers_per_s": n_mean * steps * world / (total_ms * 1e-3),
         "step_algorithmic_gbs": bytes_step["total"] * world / (total_ms / steps * 1e-3) / 1e9,

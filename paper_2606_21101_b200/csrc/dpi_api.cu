@@ -256,7 +256,11 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
         return DPI_OK;
     }
     const int32_t hint = p->opt[DPI_OPT_MAX_BAG_HINT];
-    if (!general && (p->opt[DPI_OPT_MODE] == 6 || (p->opt[DPI_OPT_MODE] == 0 && hint >= 1 && hint <= 8))) {  // short-bag variant (lookup_direct.cu)
+    // Short-bag variant (lookup_direct.cu) when the caller promised bags of <= 8 entries. Measured on B200: with
+    // multi-hot bags (promise 2..8) it wins at every batch size; with at most ONE entry per bag the balanced-segment kernel's
+    // row-copy path overtakes it once there are more than ~4e5 bags (its index prefetch pipeline pays off at that size).
+    const bool short_bags = hint >= 2 ? hint <= 8 : (hint == 1 && p->G <= 400000u);
+    if (!general && (p->opt[DPI_OPT_MODE] == 6 || (p->opt[DPI_OPT_MODE] == 0 && short_bags))) {
         cudaError_t e = launch_direct(a, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->num_sms,
                                       p->opt[DPI_OPT_PDL] != 0, stream);
         if (e != cudaSuccess) return cuda_fail(e, "direct lookup kernel launch");
