@@ -283,6 +283,8 @@ dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int
  * internal streams ordered after `stream`, so both PCIe directions and the SMs are busy at once. Each chunk is an
  * independent sub-batch with its own device plan (bags are independent); the host only adds up how many
  * index entries each chunk owns, to size the copies. The result is identical to the unchunked call.
+ * Because the lengths are host-resident here, the longest bag of the batch is known exactly, and the call picks the a3 variant
+ * from it (as DPI_OPT_MAX_BAG_HINT would) without any promise from the caller.
  * Tables stay resident on the device (they are the model, not a per-batch input).
  *   lengths_host int32[G]; indices_host int32 / int64 [n_indices] per the plan's index type
  *   (n_indices <= max_indices); out_host [B, sum dims].

@@ -94,6 +94,7 @@ struct dpi_plan_s {
     size_t stage_idx_bytes = 0;
     void* stage_out = nullptr;
     struct HostPipeline* pipe = nullptr;   // dpi_forward_host: sample-chunked sub-plans + copy/compute streams
+    int32_t hint_override = 0;   // dpi_forward_host: longest bag of THIS batch, known exactly from the host-resident lengths
     bool built = false;
 };
 
@@ -255,7 +256,7 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
         if (e != cudaSuccess) return cuda_fail(e, "input-first kernel launch");
         return DPI_OK;
     }
-    const int32_t hint = p->opt[DPI_OPT_MAX_BAG_HINT];
+    const int32_t hint = p->hint_override > 0 ? p->hint_override : p->opt[DPI_OPT_MAX_BAG_HINT];
     // Short-bag variant (lookup_direct.cu) when the caller promised bags of <= 8 entries. Measured on B200: with
     // multi-hot bags (promise 2..8) it wins at every batch size; with at most ONE entry per bag the balanced-segment kernel's
     // row-copy path overtakes it once there are more than ~4e5 bags (its index prefetch pipeline pays off at that size).
@@ -622,14 +623,16 @@ namespace {
 
 // Sum of lengths[g0, g1) and whether any of them is negative: branch-free so that the host compiler vectorises it (the
 // loop runs once per dpi_forward_host call over all G lengths; with an early return inside it cost 0.15 ms at G = 360 K).
-bool sum_lengths(const int32_t* lengths, size_t g0, size_t g1, int64_t* total) {
+bool sum_lengths(const int32_t* lengths, size_t g0, size_t g1, int64_t* total, int32_t* longest) {
     int64_t sum = 0;
-    int32_t sign = 0;
+    int32_t sign = 0, mx = 0;
     for (size_t g = g0; g < g1; ++g) {
         sum += lengths[g];
         sign |= lengths[g];
+        mx = lengths[g] > mx ? lengths[g] : mx;
     }
     *total = sum;
+    if (*longest < mx) *longest = mx;
     return sign < 0;
 }
 
@@ -711,7 +714,8 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     const int n_chunks = host_chunks(p, static_cast<size_t>(p->G) * 4 + static_cast<size_t>(n_indices) * idx_elt + out_bytes);
     if (n_chunks <= 1) {
         int64_t total = 0;  // same host-side check as the pipelined path: the lengths must add up to n_indices
-        if (sum_lengths(lengths_host, 0, p->G, &total)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
+        int32_t longest = 0;
+        if (sum_lengths(lengths_host, 0, p->G, &total, &longest)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
         if (total != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)total);
         DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * idx_elt, cudaMemcpyHostToDevice, s));
@@ -719,7 +723,9 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
         if (st != DPI_OK) return st;
         LookupCall c;
         c.tables = table_ptrs_dev; c.indices = p->stage_idx; c.pooling = pooling; c.out = out_base;
+        p->hint_override = longest > 0 ? longest : 1;  // the lengths are on the host: the bag-length "promise" is a fact here
         st = do_lookup(p, c, s);
+        p->hint_override = 0;
         if (st != DPI_OK) return st;
         if (!out_direct) DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
         DPI_CUDA(cudaStreamSynchronize(s));
@@ -734,10 +740,11 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     // Copy sizes only: how many index entries belong to each chunk (the plan itself -- offsets, segments -- is still
     // computed on the device, per chunk).
     std::vector<int64_t> entry_lo(n_sub + 1, 0);
+    int32_t longest = 0;
     for (size_t c = 0; c < n_sub; ++c) {
         const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T, g1 = static_cast<size_t>(h->sample_lo[c + 1]) * p->T;
         int64_t n = 0;
-        if (sum_lengths(lengths_host, g0, g1, &n)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
+        if (sum_lengths(lengths_host, g0, g1, &n, &longest)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
         entry_lo[c + 1] = entry_lo[c] + n;
     }
     if (entry_lo[n_sub] != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)entry_lo[n_sub]);
@@ -767,7 +774,9 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
         if (st != DPI_OK) return st;
         LookupCall lc;
         lc.tables = table_ptrs_dev; lc.indices = idx_dev; lc.pooling = pooling; lc.out = out_dev;
+        q->hint_override = longest > 0 ? longest : 1;
         st = do_lookup(q, lc, cs);
+        q->hint_override = 0;
         if (st != DPI_OK) return st;
         if (!out_direct)
             DPI_CUDA(cudaMemcpyAsync(static_cast<char*>(out_host) + static_cast<size_t>(h->sample_lo[c]) * row_bytes, out_dev,
