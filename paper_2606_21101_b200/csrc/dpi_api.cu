@@ -261,7 +261,10 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
     // multi-hot bags (promise 2..8) it wins at every batch size; with at most ONE entry per bag the balanced-segment kernel's
     // row-copy path overtakes it once there are more than ~4e5 bags (its index prefetch pipeline pays off at that size).
     const bool short_bags = hint >= 2 ? hint <= 8 : (hint == 1 && p->G <= 400000u);
-    if (!general && (p->opt[DPI_OPT_MODE] == 6 || (p->opt[DPI_OPT_MODE] == 0 && short_bags))) {
+    // the short-bag variant also takes int64 ids (the one interface variant every framework feeds)
+    const bool general_but_ids = c.force_general || p->mixed_dims || p->custom_columns || a.table_major || c.weights || c.peers ||
+                                 ld != p->out_width;
+    if (!general_but_ids && (p->opt[DPI_OPT_MODE] == 6 || (p->opt[DPI_OPT_MODE] == 0 && short_bags))) {
         cudaError_t e = launch_direct(a, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->num_sms,
                                       p->opt[DPI_OPT_PDL] != 0, stream);
         if (e != cudaSuccess) return cuda_fail(e, "direct lookup kernel launch");

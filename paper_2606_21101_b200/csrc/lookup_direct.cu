@@ -52,7 +52,8 @@ __global__ void __launch_bounds__(256) direct_kernel(const LookupArgs a) {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const bool ok = vec_ok && j < len[u];
-                const uint32_t r = ok ? static_cast<uint32_t>(__ldg(a.indices + lo[u] + j)) : 0u;
+                // int64 ids are read through their low words (little-endian, rows < 2^31): idx_shift = 1
+                const uint32_t r = ok ? static_cast<uint32_t>(__ldg(a.indices + (static_cast<size_t>(lo[u] + j) << a.idx_shift))) : 0u;
                 v[u] = ld_row16(s_tab_direct[tt[u]] + static_cast<uint64_t>(r) * row_bytes + sl * 16, ok);
             }
 #pragma unroll

@@ -251,3 +251,13 @@ def test_general_kernel_at_the_maximum_table_count():
     rows = [int(t * 5 % 11 + 1) for t in range(T)]
     _run(dims, rows, 3, "bf16", ("uniform", 0, 3), out_dtype="f32", idx64=True, weighted=True, K=64)
     _run([d // 2 for d in dims], rows, 2, "f32", ("const", 1), table_major=True, pooling=[t & 1 for t in range(T)])
+
+
+@pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 0, 3), ("poisson", 20.0, 100, 0.05)])
+@pytest.mark.parametrize("dtype,out", [("f32", None), ("bf16", "f32"), ("f16", None)])
+def test_int64_ids_through_the_short_bag_variant(dtype, out, lengths):
+    """DPI_OPT_MODE = 6 with int64 ids: the short-bag variant reads the low words itself instead of falling back to the
+    general kernel; equal dims (the variant's precondition)."""
+    D = 16 if dtype == "f32" else 32
+    _run([D] * 7, [1000, 50, 7, 3000, 1, 640, 99], 333, dtype, lengths, out_dtype=out, idx64=True, mode=6,
+         pooling=[0, 1, 0, 1, 1, 0, 1])
