@@ -47,7 +47,7 @@ def parse_args():
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--mode", type=int, default=0)
-    ap.add_argument("--pdl", type=int, default=0)
+    ap.add_argument("--pdl", type=int, default=-1, help="-1: library default (on), 0 / 1: force")
     ap.add_argument("--host-chunks", type=int, default=0, help="dpi_forward_host: 0 auto, 1 unpipelined, n chunks")
     ap.add_argument("--host-direct-out", type=int, default=0,
                     help="dpi_forward_host: 0 auto (lookup stores straight into pinned out_host), 1 staged + D2H copy, 2 require direct")
@@ -189,7 +189,8 @@ def apply_options(plan, args, binding):
     plan.set_option(binding.OPT_BLOCK_THREADS, args.block_threads)
     plan.set_option(binding.OPT_BLOCKS_PER_SM, args.blocks_per_sm)
     plan.set_option(binding.OPT_MODE, args.mode)
-    plan.set_option(binding.OPT_PDL, args.pdl)
+    if args.pdl >= 0:
+        plan.set_option(binding.OPT_PDL, args.pdl)
     plan.set_option(binding.OPT_HOST_CHUNKS, args.host_chunks)
     plan.set_option(binding.OPT_HOST_DIRECT_OUT, args.host_direct_out)
 

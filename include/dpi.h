@@ -82,7 +82,9 @@ typedef enum {
                                    DPI_OPT_MAX_BAG_HINT) whatever the hint says */
     DPI_OPT_ROW_L1_NO_ALLOC = 4,/* reserved: accepts -1 / 0 only. Rows always allocate in L1; the L1::no_allocate
                                    variant measured 17-20 % slower on B200 and was removed */
-    DPI_OPT_PDL = 5,            /* 1: lookup is launched with programmatic dependent launch after the planner */
+    DPI_OPT_PDL = 5,            /* 1 (default): the lookup is launched with programmatic dependent launch, so its prologue
+                                   overlaps the tail of the planner (or of whatever precedes it on the stream); it still
+                                   waits for that kernel's completion before reading anything. 0: plain launch */
     DPI_OPT_HOST_CHUNKS = 6,    /* dpi_forward_host only: number of sample chunks pipelined over the copy engines and the
                                    SMs; 0 = auto (~16 MB of PCIe traffic per chunk, <= 8), 1 = no pipelining, up to 64 */
     DPI_OPT_HOST_DIRECT_OUT = 7,/* dpi_forward_host only: 0 = auto, 1 = always stage (lookup -> device block -> D2H copy),
