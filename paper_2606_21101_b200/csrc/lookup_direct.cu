@@ -75,8 +75,6 @@ cudaError_t launch_direct_t(const LookupArgs& a, int lanes, int num_sms, bool pd
     constexpr int U = 2;
     const unsigned long long lanes_needed = (static_cast<unsigned long long>(a.G) * lanes + U - 1) / U;
     unsigned long long ctas = (lanes_needed + 255) / 256;
-    const unsigned long long cap = static_cast<unsigned long long>(num_sms > 0 ? num_sms : 148) * 8;
-    if (ctas > cap) ctas = cap;
     if (ctas < 1) ctas = 1;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(static_cast<unsigned>(ctas));
@@ -89,8 +87,21 @@ cudaError_t launch_direct_t(const LookupArgs& a, int lanes, int num_sms, bool pd
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;
     count_launch();
+    // One resident wave at most: CTAs beyond SMs x occupancy would only queue behind the first wave and leave a ragged tail
+    // (c3: 1.6 waves at a fixed cap of 8 per SM cost 9 %); the kernel strides over the bags instead.
     switch (lanes) {
-#define DPI_DIRECT(w) case w: return cudaLaunchKernelEx(&cfg, direct_kernel<Tr, w, U, OUT32>, a);
+#define DPI_DIRECT(w)                                                                                                         \
+    case w: {                                                                                                                 \
+        static int occ = 0;                                                                                                   \
+        if (occ == 0 && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, direct_kernel<Tr, w, U, OUT32>, 256,             \
+                                                                       cfg.dynamicSmemBytes) != cudaSuccess || occ < 1)) {    \
+            (void)cudaGetLastError();                                                                                         \
+            occ = 4;                                                                                                          \
+        }                                                                                                                     \
+        const unsigned long long cap = static_cast<unsigned long long>(num_sms > 0 ? num_sms : 148) * occ;                    \
+        cfg.gridDim = dim3(static_cast<unsigned>(ctas > cap ? cap : ctas));                                                   \
+        return cudaLaunchKernelEx(&cfg, direct_kernel<Tr, w, U, OUT32>, a);                                                   \
+    }
         DPI_DIRECT(1) DPI_DIRECT(2) DPI_DIRECT(4) DPI_DIRECT(8) DPI_DIRECT(16) DPI_DIRECT(32)
 #undef DPI_DIRECT
         default: return cudaErrorInvalidValue;
