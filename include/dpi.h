@@ -95,7 +95,7 @@ typedef enum {
                                    2 returns DPI_ERR_INVALID_ARG if it does not. */
     DPI_OPT_MAX_BAG_HINT = 8,   /* 0 = unknown (default). L >= 1: the caller's promise that no bag of the batches run with this
                                    plan is longer than L (a schema fact in CTR serving: "at most 3 tags per item"). With
-                                   2 <= L <= 8 (or L = 1 and at most 1e6 bags) and DPI_OPT_MODE = 0 the dense layout runs the
+                                   2 <= L <= 8 (or L = 1 and at most 5e5 bags) and DPI_OPT_MODE = 0 the dense layout runs the
                                    short-bag variant (one lane group per bag straight from the plan's offsets, no
                                    segments; 12-50 % faster on such batches) instead of the balanced-segment kernel. A longer bag is still pooled correctly, only without
                                    load balancing -- which is why this is a promise and not a guess from max_indices. */

@@ -259,8 +259,8 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
     const int32_t hint = p->hint_override > 0 ? p->hint_override : p->opt[DPI_OPT_MAX_BAG_HINT];
     // Short-bag variant (lookup_direct.cu) when the caller promised bags of <= 8 entries. Measured on B200: with
     // multi-hot bags (promise 2..8) it wins at every batch size; with at most ONE entry per bag the balanced-segment kernel's
-    // row-copy path overtakes it once there are more than ~1e6 bags (its index prefetch pipeline pays off at that size).
-    const bool short_bags = hint >= 2 ? hint <= 8 : (hint == 1 && p->G <= 1000000u);
+    // row-copy path overtakes it once there are more than ~5e5 bags (its index prefetch pipeline pays off at that size).
+    const bool short_bags = hint >= 2 ? hint <= 8 : (hint == 1 && p->G <= 500000u);
     // the short-bag variant also takes int64 ids (the one interface variant every framework feeds)
     const bool general_but_ids = c.force_general || p->mixed_dims || p->custom_columns || a.table_major || c.weights || c.peers ||
                                  ld != p->out_width;

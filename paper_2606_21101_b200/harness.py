@@ -112,7 +112,7 @@ def max_bag_length(cfg: W.Config) -> int:
 def lookup_variant(cfg: W.Config, mode: int = 0, bag_hint: bool = True) -> str:
     """Which a3 kernel dpi_lookup runs for this config (mirrors the rule in dpi_api.cu::do_lookup; reporting only)."""
     L = max_bag_length(cfg) if bag_hint else 0
-    short = (2 <= L <= 8) or (L == 1 and cfg.G <= 1000000)
+    short = (2 <= L <= 8) or (L == 1 and cfg.G <= 500000)
     return "short-bag (lane group per bag)" if (mode == 6 or (mode == 0 and short)) else "balanced segments"
 
 
