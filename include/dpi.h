@@ -296,8 +296,9 @@ dpi_status_t dpi_forward_host(dpi_plan_t* plan, const void* const* table_ptrs_de
                               const int32_t* lengths_host, const void* indices_host, int64_t n_indices,
                               const uint8_t* pooling, void* out_host, void* stream);
 
-/* Off the hot path: counts indices outside [0, table_rows[t]) for the last built batch; synchronises.
- * Returns DPI_ERR_INDEX_RANGE (and *n_bad > 0) if any. */
+/* Off the hot path: checks the preconditions of dpi_lookup on the last built batch; synchronises. Counts indices outside
+ * [0, table_rows[t]) -> DPI_ERR_INDEX_RANGE (and *n_bad > 0) if any; and, when DPI_OPT_MAX_BAG_HINT = L > 0 is set, bags longer
+ * than the promised L -> DPI_ERR_INVALID_ARG (results would still be correct, only the kernel choice would be wrong). */
 dpi_status_t dpi_check_indices(const dpi_plan_t* plan, const void* indices_dev, int64_t* n_bad,
                                void* stream);
 

@@ -383,7 +383,7 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     }
     DPI_TRY(cudaMalloc(&p->table_rows_dev, T * sizeof(int64_t)));
     DPI_TRY(cudaMemcpy(p->table_rows_dev, table_rows, T * sizeof(int64_t), cudaMemcpyHostToDevice));
-    DPI_TRY(cudaMalloc(&p->n_bad_dev, sizeof(unsigned long long)));
+    DPI_TRY(cudaMalloc(&p->n_bad_dev, 2 * sizeof(unsigned long long)));
     {
         std::vector<uint32_t> nv(T), col(T);
         uint32_t c = 0;
@@ -797,12 +797,13 @@ dpi_status_t dpi_check_indices(const dpi_plan_t* p, const void* indices_dev, int
     if (!p || !n_bad) return fail(DPI_ERR_INVALID_ARG, "NULL argument");
     if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    DPI_CUDA(cudaMemsetAsync(p->n_bad_dev, 0, sizeof(unsigned long long), s));
+    DPI_CUDA(cudaMemsetAsync(p->n_bad_dev, 0, 2 * sizeof(unsigned long long), s));
     CheckArgs a{};
     a.indices = indices_dev;
     a.offsets = p->offsets;
     a.table_rows = p->table_rows_dev;
     a.n_bad = p->n_bad_dev;
+    a.max_bag = p->opt[DPI_OPT_MAX_BAG_HINT];
     a.G = p->G;
     a.T = static_cast<uint32_t>(p->T);
     a.B = static_cast<uint32_t>(p->B);
@@ -810,11 +811,12 @@ dpi_status_t dpi_check_indices(const dpi_plan_t* p, const void* indices_dev, int
     a.table_major = p->bag_order == DPI_BAGS_TABLE_MAJOR;
     cudaError_t e = launch_check_indices(a, s);
     if (e != cudaSuccess) return cuda_fail(e, "check_indices launch");
-    unsigned long long bad = 0;
-    DPI_CUDA(cudaMemcpyAsync(&bad, p->n_bad_dev, sizeof bad, cudaMemcpyDeviceToHost, s));
+    unsigned long long counts[2] = {0, 0};
+    DPI_CUDA(cudaMemcpyAsync(counts, p->n_bad_dev, sizeof counts, cudaMemcpyDeviceToHost, s));
     DPI_CUDA(cudaStreamSynchronize(s));
-    *n_bad = static_cast<int64_t>(bad);
-    if (bad) return fail(DPI_ERR_INDEX_RANGE, "%llu indices outside [0, table_rows[t])", bad);
+    *n_bad = static_cast<int64_t>(counts[0]);
+    if (counts[0]) return fail(DPI_ERR_INDEX_RANGE, "%llu indices outside [0, table_rows[t])", counts[0]);
+    if (counts[1]) return fail(DPI_ERR_INVALID_ARG, "%llu bags are longer than the promised DPI_OPT_MAX_BAG_HINT = %d", counts[1], a.max_bag);
     return DPI_OK;
 }
 

@@ -55,7 +55,8 @@ struct CheckArgs {
     const void* __restrict__ indices;        // int32 or int64 (idx64)
     const int32_t* __restrict__ offsets;
     const int64_t* __restrict__ table_rows;  // device [T]
-    unsigned long long* n_bad;
+    unsigned long long* n_bad;               // [0] indices out of range, [1] bags longer than max_bag (when max_bag > 0)
+    int32_t max_bag;                         // DPI_OPT_MAX_BAG_HINT, 0 = no promise to check
     uint32_t G;
     uint32_t T;
     uint32_t B;

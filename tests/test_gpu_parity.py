@@ -103,13 +103,18 @@ def _run_gpu(cfg, dt, batch, pooling, K=0, opts=None, via_explicit_offsets=False
     # no bag-length hint by default: these tests are about the balanced-segment kernel on every bag shape; the short-bag
     # variant has its own tests (mode 6 / DPI_OPT_MAX_BAG_HINT) further down
     plan = harness.make_plan(cfg, dt.rows, max(batch.N, 1), bag_hint=bool((opts or {}).get("bag_hint", False)))
-    opts = {k: v for k, v in (opts or {}).items() if k != "bag_hint"}
+    broken_promise = bool((opts or {}).get("broken_promise", False))   # the bag-length hint is violated on purpose
+    opts = {k: v for k, v in (opts or {}).items() if k not in ("bag_hint", "broken_promise")}
     if K:
         plan.set_quantum(K)
     for k, v in (opts or {}).items():
         plan.set_option(k, v)
     plan.build(db.lengths)
-    assert plan.check_indices(db.indices) == 0
+    if broken_promise:
+        with pytest.raises(binding.DpiError):
+            plan.check_indices(db.indices)
+    else:
+        assert plan.check_indices(db.indices) == 0
     out = harness.new_output(cfg, fill_nan=True)
     off_dev = None
     if via_explicit_offsets:
@@ -550,7 +555,21 @@ def test_bag_length_hint_selects_the_short_bag_variant_and_a_broken_promise_is_s
     whose bags are far longer than the promised 2 (correct, just not load-balanced), and a hint above 8 (planned kernel)."""
     _full_parity(W.C3, opts={"bag_hint": True})
     cfg = W.Config("hp", 3, (100, 1000, 10), 32, "f16", 500, ("poisson", 6.0, 40, 0.2), ("zipf", 1.2), "mean", 4)
-    _full_parity(cfg, opts={binding.OPT_MAX_BAG_HINT: 2})
+    _full_parity(cfg, opts={binding.OPT_MAX_BAG_HINT: 2, "broken_promise": True})
     _full_parity(cfg, opts={binding.OPT_MAX_BAG_HINT: 40})
     with pytest.raises(binding.DpiError):
         binding.Plan([5], 16, 0, 4, 10).set_option(binding.OPT_MAX_BAG_HINT, -1)
+    # the promise is checkable off the hot path, like the index range
+    rows = cfg.table_rows()
+    batch = W.make_batch(cfg, rows)
+    db = harness.upload_batch(batch)
+    plan = harness.make_plan(cfg, rows, max(batch.N, 1), bag_hint=False)
+    plan.build(db.lengths)
+    longest = int(batch.lengths.max())
+    plan.set_option(binding.OPT_MAX_BAG_HINT, longest)
+    assert plan.check_indices(db.indices) == 0
+    plan.set_option(binding.OPT_MAX_BAG_HINT, longest - 1)
+    with pytest.raises(binding.DpiError) as e:
+        plan.check_indices(db.indices)
+    assert e.value.status == 1 and "DPI_OPT_MAX_BAG_HINT" in e.value.detail
+    plan.destroy()
