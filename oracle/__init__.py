@@ -37,7 +37,8 @@ def build(force: bool = False) -> str:
         newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_NONGEMM))
         if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
             tmp = _LIB + f".tmp{os.getpid()}"
-            subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared",
+            # -fopenmp only serves oracle_lookup_par (the all-cores timing leg); every other function is a plain loop
+            subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
                                    "-Wall", "-Wextra", "-o", tmp, _SRC, _SRC_NONGEMM, "-lm"])
             os.replace(tmp, _LIB)
     return _LIB
@@ -56,6 +57,12 @@ def _load():
         lib.oracle_lookup_general.restype = ctypes.c_int
         lib.oracle_plan.argtypes = [vp, i64, i32, vp, vp, vp, i64, vp]
         lib.oracle_plan.restype = ctypes.c_int
+        lib.oracle_lookup_par.argtypes = [i32, i32, i32, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp]
+        lib.oracle_lookup_par.restype = ctypes.c_int
+        lib.oracle_plan_stats.argtypes = [vp, i64, vp, vp]
+        lib.oracle_plan_stats.restype = ctypes.c_int
+        lib.oracle_plan64.argtypes = [vp, i64, i64, vp, vp, vp, i64, vp]
+        lib.oracle_plan64.restype = ctypes.c_int
         lib.oracle_decode_f16.argtypes = [ctypes.c_uint16]
         lib.oracle_decode_f16.restype = ctypes.c_double
         lib.oracle_decode_bf16.argtypes = [ctypes.c_uint16]
@@ -134,6 +141,29 @@ def lookup(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray
     return ref
 
 
+def lookup_par(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray, offsets: np.ndarray,
+               pooling: np.ndarray):
+    """oracle_lookup on all host cores (OpenMP over samples; bit-identical block). Returns (ref float64[B, T*D],
+    threads used). bench.py's cpu_baseline timing leg; the tests pin it to lookup()."""
+    T = len(tables)
+    D = int(np.asarray(tables[0]).shape[1])
+    indices = np.ascontiguousarray(indices, dtype=np.int32)
+    offsets = np.ascontiguousarray(offsets, dtype=np.int32)
+    pooling = np.ascontiguousarray(pooling, dtype=np.uint8)
+    if offsets.shape[0] != B * T + 1 or pooling.shape[0] != T:
+        raise ValueError("offsets must be [B*T+1], pooling [T]")
+    if int(offsets[-1]) > indices.shape[0]:
+        raise ValueError("offsets[-1] exceeds len(indices)")
+    ptrs, rows, keep = _table_ptrs(tables, dtype, D)
+    ref = np.empty((B, T * D), dtype=np.float64)
+    team = ctypes.c_int32(0)
+    _check(_load().oracle_lookup_par(T, B, D, dtype, ctypes.cast(ptrs, ctypes.c_void_p), rows.ctypes.data,
+                                     indices.ctypes.data, offsets.ctypes.data, pooling.ctypes.data,
+                                     ref.ctypes.data, ctypes.byref(team)))
+    del keep
+    return ref, int(team.value)
+
+
 SAMPLE_MAJOR, TABLE_MAJOR = 0, 1
 
 
@@ -179,6 +209,29 @@ def plan(lengths: np.ndarray, K: int, with_seg_off: bool = False):
                                seg_off.ctypes.data, cap, ctypes.byref(S)))
     res = (offsets, seg_bag[: S.value + 1].copy(), int(S.value))
     return res + (seg_off[: S.value + 1].copy(),) if with_seg_off else res
+
+
+def plan_stats(lengths: np.ndarray):
+    """(min_len, max_len) of the bag-length sequence (both 0 for G == 0)."""
+    lengths = np.ascontiguousarray(lengths, dtype=np.int32)
+    lo, hi = ctypes.c_int32(0), ctypes.c_int32(0)
+    _check(_load().oracle_plan_stats(lengths.ctypes.data, lengths.shape[0], ctypes.byref(lo), ctypes.byref(hi)))
+    return int(lo.value), int(hi.value)
+
+
+def plan64(lengths: np.ndarray, K: int):
+    """The plan with 64-bit offsets (N may be >= 2^31). Returns (offsets int64[G+1], seg_bag int32[S+1], S,
+    seg_off int64[S+1])."""
+    lengths = np.ascontiguousarray(lengths, dtype=np.int32)
+    G = lengths.shape[0]
+    cap = (int(lengths.astype(np.int64).sum()) + G) // max(int(K), 1) + 3
+    offsets = np.empty(G + 1, dtype=np.int64)
+    seg_bag = np.empty(cap, dtype=np.int32)
+    seg_off = np.empty(cap, dtype=np.int64)
+    S = ctypes.c_int64(0)
+    _check(_load().oracle_plan64(lengths.ctypes.data, G, int(K), offsets.ctypes.data, seg_bag.ctypes.data,
+                                 seg_off.ctypes.data, cap, ctypes.byref(S)))
+    return offsets, seg_bag[: S.value + 1].copy(), int(S.value), seg_off[: S.value + 1].copy()
 
 
 def decode_f16(bits: int) -> float:

@@ -28,6 +28,13 @@
  * oracle_lookup_general (interface variants) is pinned in tests/test_oracle_variants.py: torch-CPU embedding_bag
  * with per_sample_weights (float64), linearity / power-of-two / zero weights, index-encoding tables with mixed
  * dims, hstack of single-table calls, and the bag-grid transpose for table-major input.
+ * oracle_plan_stats (min / max bag length, a1's "uniform-length flag") and oracle_plan64 (64-bit offsets, N >= 2^31) are
+ * pinned in tests/test_oracle_plan.py: the hand-worked fixture, closed forms for constant and arithmetic-progression
+ * lengths (incl. lengths whose sum passes 2^31), permutation / concatenation invariants, sorted-order brute force and
+ * equality with the 32-bit plan wherever both are defined.
+ * oracle_lookup_par is oracle_lookup with the two outer loops interchanged (samples outside, OpenMP over samples); every
+ * bag is pooled by the same pool_bag() in the same j -> c order, so the block is bit-identical -- pinned by exactly that
+ * equality in tests/test_oracle_lookup.py. It exists only so that bench.py can time the oracle on all host cores.
  */
 #include <stdint.h>
 #include <stddef.h>
@@ -109,6 +116,28 @@ int oracle_alg1_onehot(int32_t b, int32_t k, int32_t d, int dtype,
  * Pooled multi-hot lookup.  Bag g = b*T + t owns indices[offsets[g] .. offsets[g+1]).
  * ref is [B, T*D] row-major float64, table t at columns [t*D, (t+1)*D).
  */
+/* One bag (b, t): the inner two loops of DESIGN.md §4 (entries j in order, columns c), float64, unrounded. */
+static int pool_bag(int32_t T, int32_t D, int dtype, const void *table, int64_t rows_t, int pool_t,
+                    const int32_t *indices, const int32_t *offsets, int32_t b, int32_t t, double *ref)
+{
+    int64_t g = (int64_t)b * T + t;
+    int64_t lo = offsets[g], hi = offsets[g + 1];
+    double *acc = ref + (int64_t)b * ((int64_t)T * D) + (int64_t)t * D;
+    if (hi < lo) return ORACLE_BAD_ARG;
+    for (int32_t c = 0; c < D; ++c) acc[c] = 0.0;
+    for (int64_t j = lo; j < hi; ++j) {
+        int64_t r = indices[j];
+        if (r < 0 || r >= rows_t) return ORACLE_INDEX_RANGE;
+        for (int32_t c = 0; c < D; ++c)
+            acc[c] += element_as_double(table, dtype, r * D + c);
+    }
+    if (pool_t == ORACLE_MEAN && hi > lo) {
+        double L = (double)(hi - lo);
+        for (int32_t c = 0; c < D; ++c) acc[c] /= L;
+    }
+    return ORACLE_OK;
+}
+
 int oracle_lookup(int32_t T, int32_t B, int32_t D, int dtype,
                   const void *const *tables, const int64_t *table_rows,
                   const int32_t *indices, const int32_t *offsets,
@@ -118,24 +147,54 @@ int oracle_lookup(int32_t T, int32_t B, int32_t D, int dtype,
     if (dtype != ORACLE_F32 && dtype != ORACLE_F16 && dtype != ORACLE_BF16) return ORACLE_BAD_ARG;
     for (int32_t t = 0; t < T; ++t) {                            /* tables in order -> column block t */
         for (int32_t b = 0; b < B; ++b) {                        /* samples -> output row b */
-            int64_t g = (int64_t)b * T + t;
-            int64_t lo = offsets[g], hi = offsets[g + 1];
-            double *acc = ref + (int64_t)b * ((int64_t)T * D) + (int64_t)t * D;
-            if (hi < lo) return ORACLE_BAD_ARG;
-            for (int32_t c = 0; c < D; ++c) acc[c] = 0.0;
-            for (int64_t j = lo; j < hi; ++j) {
-                int64_t r = indices[j];
-                if (r < 0 || r >= table_rows[t]) return ORACLE_INDEX_RANGE;
-                for (int32_t c = 0; c < D; ++c)
-                    acc[c] += element_as_double(tables[t], dtype, r * D + c);
-            }
-            if (pooling[t] == ORACLE_MEAN && hi > lo) {
-                double L = (double)(hi - lo);
-                for (int32_t c = 0; c < D; ++c) acc[c] /= L;
-            }
+            int rc = pool_bag(T, D, dtype, tables[t], table_rows[t], pooling[t], indices, offsets, b, t, ref);
+            if (rc != ORACLE_OK) return rc;
         }
     }
     return ORACLE_OK;
+}
+
+/*
+ * The same lookup on all host cores, for bench.py's cpu_baseline only (SURVEY.md 8(d) "Oracle timing" (ii)): bags are
+ * independent, so the sample loop is moved outside and split over threads; each bag still goes through
+ * pool_bag() in the same entry and column order, hence the block is bit-identical to oracle_lookup's.
+ * threads_used receives the team size (may be NULL). Compiled without OpenMP this is a plain loop.
+ */
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+int oracle_lookup_par(int32_t T, int32_t B, int32_t D, int dtype,
+                      const void *const *tables, const int64_t *table_rows,
+                      const int32_t *indices, const int32_t *offsets,
+                      const uint8_t *pooling, double *ref, int32_t *threads_used)
+{
+    if (T <= 0 || B < 0 || D <= 0 || !tables || !table_rows || !offsets || !pooling || !ref) return ORACLE_BAD_ARG;
+    if (dtype != ORACLE_F32 && dtype != ORACLE_F16 && dtype != ORACLE_BF16) return ORACLE_BAD_ARG;
+    int status = ORACLE_OK;
+    int team = 1;
+#ifdef _OPENMP
+#pragma omp parallel
+    {
+#pragma omp single
+        team = omp_get_num_threads();
+#pragma omp for schedule(static)
+#endif
+        for (int32_t b = 0; b < B; ++b) {
+            for (int32_t t = 0; t < T; ++t) {
+                int rc = pool_bag(T, D, dtype, tables[t], table_rows[t], pooling[t], indices, offsets, b, t, ref);
+                if (rc != ORACLE_OK) {
+#ifdef _OPENMP
+#pragma omp critical
+#endif
+                    status = rc;
+                }
+            }
+        }
+#ifdef _OPENMP
+    }
+#endif
+    if (threads_used) *threads_used = team;
+    return status;
 }
 
 /*
@@ -230,5 +289,57 @@ int oracle_plan(const int32_t *len, int64_t G, int32_t K,
         if (seg_off) seg_off[s] = offsets[g];
     }
     *S_out = (int32_t)S;
+    return ORACLE_OK;
+}
+
+/*
+ * a1's summary of the length sequence (SURVEY.md 8(a) a1 "min/max len (uniform-length flag)"; "the overall embedding
+ * workload is deterministic and known in advance", PAPER.md:109 -- the one-hot workload of Alg. 1 is the case
+ * min_len == max_len == 1).  DESIGN.md §3:
+ *   min_len = min_{g in [0,G)} len[g],  max_len = max_{g in [0,G)} len[g];   G == 0 -> both 0.
+ */
+int oracle_plan_stats(const int32_t *len, int64_t G, int32_t *min_len, int32_t *max_len)
+{
+    if ((!len && G > 0) || G < 0 || !min_len || !max_len) return ORACLE_BAD_ARG;
+    int32_t lo = 0, hi = 0;
+    for (int64_t g = 0; g < G; ++g) {
+        if (len[g] < 0) return ORACLE_BAD_ARG;
+        if (g == 0 || len[g] < lo) lo = len[g];
+        if (g == 0 || len[g] > hi) hi = len[g];
+    }
+    *min_len = lo;
+    *max_len = hi;
+    return ORACLE_OK;
+}
+
+/*
+ * The same plan with 64-bit offsets (SURVEY.md 8(f) NEXT-2 "int64 indices/offsets"; ids and offsets reach the model as
+ * 64-bit integers): identical definition to oracle_plan, only offsets[], seg_off[] and S are
+ * int64, so N = sum len may be >= 2^31.  G < 2^31 still (seg_bag stays int32).
+ */
+int oracle_plan64(const int32_t *len, int64_t G, int64_t K,
+                  int64_t *offsets, int32_t *seg_bag, int64_t *seg_off, int64_t seg_cap, int64_t *S_out)
+{
+    if (!len || G < 0 || G > 2147483647LL || K < 1 || !offsets || !seg_bag || !S_out) return ORACLE_BAD_ARG;
+    offsets[0] = 0;
+    for (int64_t g = 0; g < G; ++g) {
+        if (len[g] < 0) return ORACLE_BAD_ARG;
+        offsets[g + 1] = offsets[g] + len[g];
+    }
+    int64_t CG = 0;
+    for (int64_t g = 0; g < G; ++g) CG += (len[g] > 1 ? len[g] : 1);
+    int64_t S = (CG + K - 1) / K;
+    if (S + 1 > seg_cap) return ORACLE_CAPACITY;
+    int64_t g = 0, Cg = 0;
+    for (int64_t s = 0; s <= S; ++s) {
+        int64_t target = s * K;
+        while (g < G && Cg < target) {
+            Cg += (len[g] > 1 ? len[g] : 1);
+            ++g;
+        }
+        seg_bag[s] = (int32_t)g;
+        if (seg_off) seg_off[s] = offsets[g];
+    }
+    *S_out = S;
     return ORACLE_OK;
 }

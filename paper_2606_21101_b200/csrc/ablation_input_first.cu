@@ -11,9 +11,13 @@
 namespace dpi {
 namespace {
 
+// Column slices are walked kGroup 16-byte vectors at a time (128 B of row), so a bag's index entries are read once for rows
+// up to 128 B and once per 128-byte slice beyond that (the accumulators of a whole 512-byte row do not fit in registers).
 template <class Tr, bool OUT32>
 __global__ void __launch_bounds__(128) input_first_kernel(const LookupArgs a, const uint32_t B) {
     constexpr int kAcc = Tr::kAcc;
+    constexpr uint32_t kGroup = 8;
+    constexpr size_t kOutVec = (OUT32 && kAcc == 8) ? 32 : 16;
     const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     const size_t row_bytes = static_cast<size_t>(a.nvec) * 16;
@@ -23,16 +27,22 @@ __global__ void __launch_bounds__(128) input_first_kernel(const LookupArgs a, co
         const int lo = __ldg(a.offsets + g), hi = __ldg(a.offsets + g + 1);
         const char* tab = static_cast<const char*>(a.tables[t]);
         const bool mean = ((a.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1;
-        for (uint32_t v = 0; v < a.nvec; ++v) {  // one 16-byte column slice of the bag at a time
-            float2 acc[kAcc / 2];
-            zero_acc(acc);
+        for (uint32_t v0 = 0; v0 < a.nvec; v0 += kGroup) {
+            float2 acc[kGroup][kAcc / 2];
+#pragma unroll
+            for (uint32_t v = 0; v < kGroup; ++v) zero_acc(acc[v]);
             for (int j = lo; j < hi; ++j) {
-                const int r = __ldg(a.indices + j);
-                Tr::add(acc, ld_row16(tab + static_cast<size_t>(r) * row_bytes + v * 16, true));
+                const char* row = tab + static_cast<size_t>(static_cast<uint32_t>(__ldg(a.indices + j))) * row_bytes + v0 * 16;
+#pragma unroll
+                for (uint32_t v = 0; v < kGroup; ++v) Tr::add(acc[v], ld_row16(row + v * 16, v0 + v < a.nvec));
             }
-            if (mean) scale_mean(acc, hi - lo);
-            constexpr size_t kOutVec = (OUT32 && kAcc == 8) ? 32 : 16;
-            store_pooled<Tr, OUT32>(out + (g * a.nvec + v) * kOutVec, acc);
+#pragma unroll
+            for (uint32_t v = 0; v < kGroup; ++v) {
+                if (v0 + v < a.nvec) {
+                    if (mean) scale_mean(acc[v], hi - lo);
+                    store_pooled<Tr, OUT32>(out + (g * a.nvec + v0 + v) * kOutVec, acc[v]);
+                }
+            }
         }
     }
 }
@@ -40,7 +50,9 @@ __global__ void __launch_bounds__(128) input_first_kernel(const LookupArgs a, co
 }  // namespace
 
 cudaError_t launch_input_first(const LookupArgs& a, uint32_t B, int dtype, bool out32, cudaStream_t stream) {
-    const dim3 block(128), grid((B + 127) / 128);
+    // one thread per sample is the scheme itself; small batches get 32-thread CTAs so that they still spread over the SMs
+    const unsigned bt = B >= 148u * 128u ? 128u : 32u;
+    const dim3 block(bt), grid((B + bt - 1) / bt);
     count_launch();
     switch (dtype) {
         case DPI_F32: input_first_kernel<F32Traits, false><<<grid, block, 0, stream>>>(a, B); break;

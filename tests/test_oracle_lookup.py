@@ -296,3 +296,34 @@ def test_out_of_range_index_is_rejected():
         with pytest.raises(oracle.OracleError):
             oracle.lookup(tables, oracle.F32, 1, np.array([bad], np.int32), np.array([0, 1], np.int32),
                           np.zeros(1, np.uint8))
+
+
+# --------------------------------------------------------------------------------------------------
+# the all-cores timing leg (bench.py cpu_baseline): same bags, same per-bag order, samples split over threads
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f32", "f16", "bf16"])
+def test_lookup_par_is_bit_identical_to_the_single_thread_oracle(dtype):
+    rng = np.random.default_rng(21)
+    T, B, D = 7, 257, 24
+    rows = [100, 7, 1000, 33, 2, 500, 64]
+    tables32, lengths, idx = _rand_problem(rng, T, B, D, rows, 12)
+    tables = [W.to_storage(t, dtype) for t in tables32]
+    off = _offsets(lengths)
+    pooling = (np.arange(T) % 2).astype(np.uint8)
+    one = oracle.lookup(tables, W.DTYPE_CODE[dtype], B, idx, off, pooling)
+    par, team = oracle.lookup_par(tables, W.DTYPE_CODE[dtype], B, idx, off, pooling)
+    assert team >= 1
+    assert np.array_equal(one.view(np.uint64), par.view(np.uint64))   # bit for bit, signed zeros included
+
+
+def test_lookup_par_golden_fig5_and_error_status():
+    g = load("fig5_shape_example.txt")
+    lengths = np.array(g["multihot.lengths"], dtype=np.int32).reshape(-1)
+    idx = np.array(sum(g["multihot.indices"], []), dtype=np.int32)
+    pooling = np.array(g["multihot.pooling"][0], dtype=np.uint8)
+    got, _ = oracle.lookup_par(fig5_tables(), oracle.F32, 2, idx, _offsets(lengths), pooling)
+    np.testing.assert_allclose(got, np.array(g["multihot.mixed"]), rtol=1e-15)
+    bad = idx.copy()
+    bad[3] = 3   # tables have rows 0..2
+    with pytest.raises(oracle.OracleError):
+        oracle.lookup_par(fig5_tables(), oracle.F32, 2, bad, _offsets(lengths), pooling)

@@ -106,3 +106,116 @@ def test_rejects_negative_length_and_overflow():
         oracle.plan(np.array([1, -1], np.int32), 4)
     with pytest.raises(oracle.OracleError):
         oracle.plan(np.full(3, 2 ** 30, np.int32), 2 ** 20)
+
+
+# --------------------------------------------------------------------------------------------------
+# a1's min / max bag length (SURVEY.md 8(a) a1 "uniform-length flag"): DESIGN.md §3
+# --------------------------------------------------------------------------------------------------
+def test_golden_fig5_plan_stats():
+    g = load("fig5_shape_example.txt")
+    lengths = np.array(g["multihot.lengths"], dtype=np.int32).reshape(-1)
+    assert oracle.plan_stats(lengths) == (int(g["plan.min_len"][0][0]), int(g["plan.max_len"][0][0]))
+    onehot = np.ones(np.array(g["onehot.ids"]).size, dtype=np.int32)   # Alg. 1: one id per (sample, field)
+    assert oracle.plan_stats(onehot) == (int(g["onehot.min_len"][0][0]), int(g["onehot.max_len"][0][0]))
+
+
+@pytest.mark.parametrize("ell", [0, 1, 7, 2 ** 31 - 1])
+def test_plan_stats_constant_lengths(ell):
+    assert oracle.plan_stats(np.full(1000, ell, np.int32)) == (ell, ell)
+
+
+def test_plan_stats_closed_forms_and_invariants():
+    # arithmetic progression a, a+1, ..., a+n-1 in any order: min = a, max = a+n-1
+    rng = np.random.default_rng(5)
+    for a, n in [(0, 1), (3, 10), (1, 4096), (100, 2049)]:
+        ln = (a + rng.permutation(n)).astype(np.int32)
+        assert oracle.plan_stats(ln) == (a, a + n - 1)
+    # the extreme sits first / last / alone
+    assert oracle.plan_stats(np.array([9, 1, 1, 1], np.int32)) == (1, 9)
+    assert oracle.plan_stats(np.array([1, 1, 1, 0], np.int32)) == (0, 1)
+    assert oracle.plan_stats(np.array([5], np.int32)) == (5, 5)
+    assert oracle.plan_stats(np.zeros(0, np.int32)) == (0, 0)
+    # brute force through a sort; invariants min <= N/G <= max; invariance under permutation; concatenation rule
+    for seed in range(5):
+        r = np.random.default_rng(seed)
+        ln = r.integers(0, 50, size=int(r.integers(1, 300))).astype(np.int32)
+        lo, hi = oracle.plan_stats(ln)
+        srt = sorted(ln.tolist())
+        assert (lo, hi) == (srt[0], srt[-1])
+        assert lo * len(ln) <= int(ln.sum()) <= hi * len(ln)
+        assert oracle.plan_stats(r.permutation(ln)) == (lo, hi)
+        other = r.integers(0, 80, size=17).astype(np.int32)
+        lo2, hi2 = oracle.plan_stats(other)
+        assert oracle.plan_stats(np.concatenate([ln, other])) == (min(lo, lo2), max(hi, hi2))
+    with pytest.raises(oracle.OracleError):
+        oracle.plan_stats(np.array([1, -2], np.int32))
+
+
+def test_plan_stats_on_the_five_configs():
+    """The recipes fix the extremes: c2 is one-hot (uniform flag), c1 U{1..4}, c3 U{1..3}, c5 U{1..64} hit both ends at
+    these batch sizes; c4 = Poisson(20) capped at 100 with 5 % empty bags -> min 0."""
+    from paper_2606_21101_b200 import workloads as W
+    assert oracle.plan_stats(W.make_lengths(W.C2, 0)) == (1, 1)
+    assert oracle.plan_stats(W.make_lengths(W.C1, 0)) == (1, 4)
+    assert oracle.plan_stats(W.make_lengths(W.C3, 0)) == (1, 3)
+    assert oracle.plan_stats(W.make_lengths(W.C5, 0)) == (1, 64)
+    lo, hi = oracle.plan_stats(W.make_lengths(W.C4, 0))
+    assert lo == 0 and 30 <= hi <= 100
+
+
+# --------------------------------------------------------------------------------------------------
+# the plan with 64-bit offsets (SURVEY.md 8(f) NEXT-2): same definition, N may pass 2^31
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(4))
+@pytest.mark.parametrize("K", [1, 3, 32, 1000])
+def test_plan64_equals_the_32_bit_plan_and_brute_force_where_both_exist(seed, K):
+    rng = np.random.default_rng(100 + seed)
+    lengths = rng.integers(0, 9, size=int(rng.integers(1, 80))).astype(np.int32)
+    off, seg, S, seg_off = oracle.plan(lengths, K, with_seg_off=True)
+    off64, seg64, S64, seg_off64 = oracle.plan64(lengths, K)
+    assert off64.dtype == np.int64 and seg_off64.dtype == np.int64
+    assert S64 == S and np.array_equal(off64, off) and np.array_equal(seg64, seg) and np.array_equal(seg_off64, seg_off)
+    bseg, bS = brute_plan(lengths.tolist(), K)
+    assert S64 == bS and seg64.tolist() == bseg
+
+
+def test_plan64_golden_fig5():
+    g = load("fig5_shape_example.txt")
+    lengths = np.array(g["multihot.lengths"], dtype=np.int32).reshape(-1)
+    off, seg, S, seg_off = oracle.plan64(lengths, int(g["plan.K"][0][0]))
+    assert off.tolist() == [int(x) for x in g["plan.offsets"][0]] and S == int(g["plan.S"][0][0])
+    assert seg.tolist() == [int(x) for x in g["plan.seg_bag"][0]]
+    assert seg_off.tolist() == [int(x) for x in g["plan.seg_off"][0]]
+
+
+@pytest.mark.parametrize("ell,G,K", [(2 ** 30, 3, 2 ** 20), (2 ** 31 - 1, 5, 2 ** 31 - 1), (3 * 2 ** 20, 1024, 12345),
+                                     (2 ** 29, 9, 2 ** 33)])
+def test_plan64_equal_lengths_closed_form_beyond_2_pow_31(ell, G, K):
+    """len == ell for every bag: offsets[g] = g*ell, C[g] = g*ell, S = ceil(G*ell/K), seg_bag[s] = min(G, ceil(s*K/ell)),
+    seg_off[s] = seg_bag[s]*ell -- with N = G*ell >= 2^31, where the 32-bit plan refuses."""
+    lengths = np.full(G, ell, np.int32)
+    assert G * ell >= 2 ** 31
+    with pytest.raises(oracle.OracleError):
+        oracle.plan(lengths, min(K, 2 ** 31 - 1))
+    off, seg, S, seg_off = oracle.plan64(lengths, K)
+    assert S == -(-G * ell // K)
+    assert off.tolist() == [g * ell for g in range(G + 1)]
+    want = [min(G, -(-s * K // ell)) for s in range(S + 1)]
+    assert seg.tolist() == want and seg_off.tolist() == [w * ell for w in want]
+
+
+def test_plan64_mixed_lengths_past_2_pow_31_invariants():
+    rng = np.random.default_rng(9)
+    G, K = 4000, 2 ** 16
+    lengths = rng.integers(0, 2 ** 21, size=G).astype(np.int32)
+    lengths[rng.random(G) < 0.1] = 0
+    off, seg, S, seg_off = oracle.plan64(lengths, K)
+    assert int(off[-1]) == int(lengths.astype(np.int64).sum()) >= 2 ** 31
+    assert np.array_equal(np.diff(off), lengths)
+    C = np.concatenate(([0], np.cumsum(np.maximum(lengths, 1).astype(np.int64))))
+    assert S == -(-int(C[G]) // K) and seg[0] == 0 and seg[S] == G and np.all(np.diff(seg) >= 0)
+    s_arr = np.arange(S + 1, dtype=np.int64) * K
+    assert np.all((C[seg] >= s_arr) | (seg == G))
+    inner = seg > 0
+    assert np.all(C[seg[inner] - 1] < s_arr[inner])
+    assert np.array_equal(seg_off, off[seg])
