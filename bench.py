@@ -75,18 +75,39 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per lookup launch from the committed `ncu --set full` capture
-    of this workload (profiles/ncu_traffic.csv, written from the .ncu-rep), or None if there is none."""
+def csrc_hash() -> str:
+    """sha256 (first 12 hex digits) over the CUDA sources and headers the library is built from: the key that ties an ncu
+    capture in profiles/ncu_traffic.csv to the kernels it was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    base = os.path.join(ROOT, "paper_2606_21101_b200", "csrc")
+    for name in sorted(os.listdir(base)) + ["../../include/dpi.h"]:
+        path = os.path.join(base, name)
+        if os.path.isfile(path):
+            h.update(name.encode())
+            with open(path, "rb") as f:
+                h.update(f.read())
+    return h.hexdigest()[:12]
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload` from the committed `ncu --set full`
+    capture (profiles/ncu_traffic.csv, written from the .ncu-rep). Each row carries the csrc hash it was captured on: a
+    capture of other sources is not reported (traffic = None) and the reason is returned beside it."""
     try:
         import csv
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
-            for row in csv.DictReader(f):
-                if row["workload"] == workload:  # one row per workload: the a3 kernel that workload runs by default
-                    return float(row["dram_bytes_per_launch"])
+            rows = [r for r in csv.DictReader(f) if r["workload"] == workload and r["kernel"] == kernel]
     except Exception:
-        pass
-    return None
+        return None, "profiles/ncu_traffic.csv unreadable"
+    if not rows:
+        return None, f"no ncu capture of {kernel} on {workload} in profiles/ncu_traffic.csv"
+    now = csrc_hash()
+    for r in rows:
+        if r.get("csrc_hash") == now:
+            return float(r["dram_bytes_per_launch"]), None
+    return None, (f"traffic_stale: the capture of {kernel} on {workload} ({rows[-1].get('source')}) was taken on csrc "
+                  f"{rows[-1].get('csrc_hash')}, the library is now built from {now}")
 
 
 class ClockSampler:
@@ -218,44 +239,110 @@ def describe(cfg, rows, extra=None, R=R_BATCHES):
 # ----------------------------------------------------------------------------------------------------
 # CPU oracle legs
 # ----------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, rows, n_samples):
-    """A bounded sample of the workload: the first n_samples samples of batch 0, tables compacted to the rows
-    they reference (the full tables do not fit on the host for c5)."""
+def host_mirror(cfg, rows, budget_bytes):
+    """Host copy of the tables for the CPU legs: the full tables when they fit the budget (c1-c4), else
+    a ROW-SCALED mirror -- the first rows_s[t] rows of every table, indices taken modulo rows_s[t] (c5: 82 GB do not fit a
+    host). With a CUDA device the values are copied D2H from tables filled by the same device generator the GPU arm reads
+    (bit-identical to the host generator, tests/test_gpu_parity.py::test_synth_fill_matches_host_generator); without one
+    they are generated on the host under a smaller budget. Returns (tables, rows_s, scaled?)."""
     from paper_2606_21101_b200 import workloads as W
-    batch = W.make_batch(cfg.scaled(B=n_samples), rows, cfg.seed)
-    sub = W.compact_subproblem(cfg.scaled(B=n_samples), batch, np.arange(n_samples))
-    return sub
+    total = int(rows.sum()) * cfg.row_bytes
+    try:
+        import torch
+        cuda = torch.cuda.is_available()
+    except Exception:
+        cuda = False
+    if not cuda:
+        budget_bytes = min(budget_bytes, 1 << 30)
+    scale = min(1.0, budget_bytes / max(total, 1))
+    rows_s = np.maximum(1, np.floor(rows * scale)).astype(np.int64) if scale < 1.0 else rows.copy()
+    tables = []
+    if cuda:
+        import torch
+        from paper_2606_21101_b200 import binding, build, harness
+        build.build()
+        for t in range(cfg.T):
+            buf = torch.empty((int(rows_s[t]), cfg.D), dtype=harness.TORCH_DTYPE[cfg.dtype], device="cuda")
+            binding.synth_fill_table(buf, buf.numel(), W.DTYPE_CODE[cfg.dtype], W.value_key(cfg.seed, t))
+            h = buf.cpu()
+            tables.append(h.view(torch.int16).numpy().view(np.uint16) if cfg.dtype == "bf16" else h.numpy())
+            del buf
+        torch.cuda.empty_cache()
+    else:
+        tables = [W.full_table_storage(cfg, t, int(rows_s[t])) for t in range(cfg.T)]
+    return tables, rows_s, scale < 1.0
 
 
 def time_oracle(cfg, rows, target_seconds, steps=None, warmup=0):
+    """The oracle as it stands on the host cores: plan (a1 + a2) + lookup (a3) on a bounded sample of batch 0 -- the first
+    n samples, n chosen so that the two legs together take about target_seconds -- against a host mirror of the tables
+    (row-scaled when the tables do not fit: c5). Two legs on the same sample: one thread (oracle_lookup) and all visible cores
+    (oracle_lookup_par, OpenMP over samples), asserted bit-identical."""
     import oracle
     from paper_2606_21101_b200 import workloads as W
     oracle.build()
-    n_samples = min(cfg.B, 1024)
-    sub = oracle_sample(cfg, rows, n_samples)
+    try:
+        avail = int(next(l for l in open("/proc/meminfo") if l.startswith("MemAvailable")).split()[1]) * 1024
+    except Exception:
+        avail = 8 << 30
+    tables, rows_s, scaled = host_mirror(cfg, rows, min(avail // 4, 16 << 30))
     pooling = cfg.pooling_modes()
     K = 32
+    code = W.DTYPE_CODE[cfg.dtype]
 
-    def one_step():
-        off, _, _ = oracle.plan(sub.lengths, K)
-        oracle.lookup(sub.tables, W.DTYPE_CODE[cfg.dtype], n_samples, sub.indices, off, pooling)
+    def sample(n):
+        sub_cfg = cfg.scaled(B=n)
+        b = W.make_batch(sub_cfg, rows, cfg.seed)      # the first n samples of batch 0 (counter-based draws)
+        idx = b.indices
+        if scaled:
+            tab = (np.repeat(np.arange(sub_cfg.G, dtype=np.int64), b.lengths) % cfg.T)
+            idx = (idx.astype(np.int64) % rows_s[tab]).astype(np.int32)
+        return b.lengths, idx
 
+    def one_step(n, ln, idx, par, out=None):
+        off, _, _ = oracle.plan(ln, K)
+        if par:
+            return oracle.lookup_par(tables, code, n, idx, off, pooling, out=out)
+        return oracle.lookup(tables, code, n, idx, off, pooling, out=out), 1
+
+    # probe on 256 samples, then size the sample for ~ target_seconds / 4 per single-thread step
+    n0 = min(cfg.B, 256)
+    ln, idx = sample(n0)
     t = time.perf_counter()
-    one_step()
-    first = time.perf_counter() - t
-    for _ in range(warmup):
-        one_step()
-    if steps is None:
-        steps = max(1, int(target_seconds / max(first, 1e-4)))
-    t = time.perf_counter()
-    for _ in range(steps):
-        one_step()
-    dt = time.perf_counter() - t
-    bags = n_samples * cfg.T * steps
-    return {"value": bags / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"first {n_samples} samples of batch 0 ({n_samples * cfg.T} bags, {int(sub.indices.size)} rows), "
-                      f"tables compacted to referenced rows; oracle plan + lookup, {steps} steps, {dt:.1f} s",
-            "seconds": dt, "ms_per_step": dt / steps * 1e3, "steps": steps}
+    one_step(n0, ln, idx, False)
+    per_sample = max((time.perf_counter() - t) / n0, 1e-7)
+    n = int(min(cfg.B, max(n0, (target_seconds / 4) / per_sample)))
+    ln, idx = sample(n)
+    ref1, _ = one_step(n, ln, idx, False)
+    refp, team = one_step(n, ln, idx, True)
+    assert np.array_equal(ref1.view(np.uint64), refp.view(np.uint64)), "all-cores oracle leg differs from the single-thread oracle"
+    del refp
+    block = ref1   # the timed steps write into one already-touched block (first-touch page faults are not the oracle)
+    legs = {}
+    for name, par in (("single_thread", False), ("all_cores", True)):
+        for _ in range(warmup):
+            one_step(n, ln, idx, par, block)
+        t = time.perf_counter()
+        one_step(n, ln, idx, par, block)
+        first = time.perf_counter() - t
+        k = steps if steps is not None else max(1, int((target_seconds / 2) / max(first, 1e-4)))
+        t = time.perf_counter()
+        for _ in range(k):
+            one_step(n, ln, idx, par, block)
+        dt = time.perf_counter() - t
+        legs[name] = {"value": n * cfg.T * k / dt, "unit": UNIT, "cores": team if par else 1, "seconds": dt, "steps": k,
+                      "ms_per_step": dt / k * 1e3}
+    mirror = (f"row-scaled host mirror ({int(rows_s.sum())} of {int(rows.sum())} rows, indices modulo the reduced heights)" if scaled
+              else "full host mirror of the tables")
+    what = (f"first {n} of {cfg.B} samples of batch 0 ({n * cfg.T} bags, {int(idx.size)} rows gathered), {mirror}; "
+            f"oracle plan + lookup per step")
+    main = legs["all_cores"]
+    return {"value": main["value"], "unit": UNIT, "cores": main["cores"], "kind": "oracle",
+            "sample": f"{what}; all-cores leg (OpenMP over samples, bit-identical to the single-thread oracle): {main['steps']} steps, {main['seconds']:.1f} s",
+            "single_thread": {"value": legs["single_thread"]["value"], "unit": UNIT, "cores": 1,
+                              "steps": legs["single_thread"]["steps"], "seconds": legs["single_thread"]["seconds"]},
+            "host_cpus_visible": len(os.sched_getaffinity(0)), "tables_row_scaled": scaled,
+            "seconds": main["seconds"], "ms_per_step": main["ms_per_step"], "steps": main["steps"]}
 
 
 def run_reference(args):
@@ -267,7 +354,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": r["steps"], "warmup": min(args.warmup or 0, 1), "ms_per_step": r["ms_per_step"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": describe(cfg, rows), "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "config": describe(cfg, rows),
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "single_thread", "host_cpus_visible", "tables_row_scaled")},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -448,8 +536,7 @@ def run_ours(args):
     cpu = None
     if not args.no_cpu_baseline:
         r = time_oracle(cfg, rows, args.cpu_seconds)
-        cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
-        cpu["host_cpus_visible"] = len(os.sched_getaffinity(0))
+        cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "single_thread", "host_cpus_visible", "tables_row_scaled")}
 
     line = {
         "metric": METRIC, "value": sharding.job_throughput(cfg.G, steps, world, total_ms), "unit": UNIT, "n_gpus": world,

@@ -37,7 +37,11 @@
  *   - Asynchronous calls (dpi_plan_build, dpi_lookup, dpi_check_indices without result read) only enqueue
  *     work; device-side faults surface at the caller's next synchronisation.
  *   - There is NO CPU fallback: without a CUDA device every call that needs one returns DPI_ERR_CUDA.
- *   - A plan is not thread-safe; distinct plans are independent.
+ *   - A plan is not thread-safe; distinct plans are independent: every launch configuration (occupancy, shared-memory
+ *     attribute) is derived when the plan is created or re-configured and stored in the plan, so two host threads may
+ *     drive two plans on two streams concurrently. A plan belongs to the device that was current in dpi_plan_create;
+ *     make that device current for every call that takes the plan. dpi_lookup / dpi_forward make no CUDA runtime call
+ *     other than the kernel launch itself.
  */
 #ifndef DPI_H_
 #define DPI_H_
@@ -82,9 +86,11 @@ typedef enum {
                                    DPI_OPT_MAX_BAG_HINT) whatever the hint says */
     DPI_OPT_ROW_L1_NO_ALLOC = 4,/* reserved: accepts -1 / 0 only. Rows always allocate in L1; the L1::no_allocate
                                    variant measured 17-20 % slower on B200 and was removed */
-    DPI_OPT_PDL = 5,            /* 1 (default): the lookup is launched with programmatic dependent launch, so its prologue
-                                   overlaps the tail of the planner (or of whatever precedes it on the stream); it still
-                                   waits for that kernel's completion before reading anything. 0: plain launch */
+    DPI_OPT_PDL = 5,            /* 1 (default): the lookup (and the fused dpi_forward kernel) is launched with programmatic
+                                   dependent launch, so its launch and scheduling overlap the tail of the planner (or of
+                                   whatever precedes it on the stream); it executes griddepcontrol.wait before its first
+                                   memory read -- table pointers included -- so inputs produced by the preceding kernel are
+                                   safe. 0: plain launch */
     DPI_OPT_HOST_CHUNKS = 6,    /* dpi_forward_host only: number of sample chunks pipelined over the copy engines and the
                                    SMs; 0 = auto (~16 MB of PCIe traffic per chunk, <= 8), 1 = no pipelining, up to 64 */
     DPI_OPT_HOST_DIRECT_OUT = 7,/* dpi_forward_host only: 0 = auto, 1 = always stage (lookup -> device block -> D2H copy),
@@ -93,12 +99,18 @@ typedef enum {
                                    straight into it over PCIe -- the device->host transfer is fused into the kernel's
                                    store, no staging block and no D2H copy. Auto uses it whenever out_host qualifies;
                                    2 returns DPI_ERR_INVALID_ARG if it does not. */
-    DPI_OPT_MAX_BAG_HINT = 8,   /* 0 = unknown (default). L >= 1: the caller's promise that no bag of the batches run with this
-                                   plan is longer than L (a schema fact in CTR serving: "at most 3 tags per item"). With
-                                   2 <= L <= 8 (or L = 1 and at most 5e5 bags) and DPI_OPT_MODE = 0 the dense layout runs the
-                                   short-bag variant (one lane group per bag straight from the plan's offsets, no
-                                   segments; 12-50 % faster on such batches) instead of the balanced-segment kernel. A longer bag is still pooled correctly, only without
-                                   load balancing -- which is why this is a promise and not a guess from max_indices. */
+    DPI_OPT_MAX_BAG_HINT = 8,   /* OPTIONAL. 0 = unknown (default): the planner measures the longest bag of every batch (a1's
+                                   max_len, meta word 7) and the lookup kernel picks its variant from it on the device --
+                                   2 <= max_len <= 8 (or max_len <= 1 and at most 5e5 bags) runs the short-bag body (one lane
+                                   group per bag straight from the plan's offsets, no segments), anything else the balanced
+                                   segments. L >= 1: the caller's promise that no bag is longer than L (a schema fact in CTR
+                                   serving: "at most 3 tags per item"); the same rule is then applied on the host and the
+                                   short-bag variant runs as its own, leaner launch. A longer bag is still pooled correctly,
+                                   only without load balancing; dpi_check_indices verifies the promise off the hot path. */
+    DPI_OPT_FUSED = 9,          /* dpi_forward / dpi_forward_host: 0 = auto (one fused launch when the layout is the dense one,
+                                   G <= DPI_OPT_FUSED_MAX_BAGS and the capacity says bags are short on average,
+                                   max_indices <= 8*G), 1 = fused whenever the layout allows, 2 = always plan + lookup */
+    DPI_OPT_FUSED_MAX_BAGS = 10,/* ceiling of the auto rule above in bags; 0 = library default (2^20) */
     DPI_OPT_COUNT_
 } dpi_option_t;
 
@@ -152,7 +164,8 @@ dpi_status_t dpi_plan_set_columns(dpi_plan_t* plan, const int64_t* columns);
 dpi_status_t dpi_plan_out_width(const dpi_plan_t* plan, int64_t* width);
 
 /* Cost quantum K >= 1 of the balanced segments (0 = library default for this row size). Takes effect at the
- * next dpi_plan_build. DPI_ERR_INVALID_ARG if K < 0. */
+ * next dpi_plan_build and invalidates the current one (the plan must be built again before dpi_lookup).
+ * DPI_ERR_INVALID_ARG if K < 0; on an allocation failure the plan keeps its previous quantum. */
 dpi_status_t dpi_plan_set_quantum(dpi_plan_t* plan, int32_t K);
 
 /* Kernel-internal tuning (see dpi_option_t). Unknown option or unsupported value -> DPI_ERR_INVALID_ARG. */
@@ -176,7 +189,8 @@ dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims,
 
 /* Borrowed device pointers into the plan, valid until the next build/destroy. Any out-pointer may be NULL.
  *   offsets_dev int32[G+1]; seg_dev int32[2*seg_capacity], interleaved pairs {seg_bag[s], seg_off[s]};
- *   meta_dev int32[8] = {S, N, C[G] low 32 bits, overflow flag, K, G, 0, 0}. */
+ *   meta_dev int32[8] = {S, N, C[G] low 32 bits, overflow flag, K, G, min_len, max_len} (min / max bag length of the
+ *   batch: a1's summary of the workload; min_len == max_len is the uniform-length flag). */
 dpi_status_t dpi_plan_device_views(const dpi_plan_t* plan, const int32_t** offsets_dev,
                                    const int32_t** seg_dev, const int32_t** meta_dev);
 
@@ -191,6 +205,11 @@ dpi_status_t dpi_plan_info(const dpi_plan_t* plan, int32_t* T, int32_t* B, int32
  * DPI_ERR_INVALID_ARG if seg_cap < S+1 or the last build overflowed max_indices. */
 dpi_status_t dpi_plan_export(const dpi_plan_t* plan, int32_t* offsets_host, int32_t* seg_bag_host,
                              int32_t* seg_off_host, int64_t seg_cap, int32_t* S, int64_t* N, void* stream);
+
+/* Parity/debug: a1's summary of the last built batch: min_len = shortest, max_len = longest bag;
+ * min_len == max_len is the uniform-length flag (1 / 1 is Alg. 1's one-hot workload). Synchronises `stream`. The device
+ * reads the same two words (meta_dev[6], meta_dev[7]) to pick the a3 variant. Either out-pointer may be NULL. */
+dpi_status_t dpi_plan_stats(const dpi_plan_t* plan, int32_t* min_len, int32_t* max_len, void* stream);
 
 /*
  * dpi_lookup -- step a3, asynchronous on `stream`, ONE kernel launch for all tables and samples.
@@ -209,6 +228,29 @@ dpi_status_t dpi_plan_export(const dpi_plan_t* plan, int32_t* offsets_host, int3
 dpi_status_t dpi_lookup(const void* const* table_ptrs_dev, const int32_t* indices_dev,
                         const int32_t* offsets_dev, const dpi_plan_t* plan, const uint8_t* pooling,
                         void* out_dev, void* stream);
+
+/*
+ * dpi_forward -- the whole path a1 + a2 + a3 on device-resident inputs in one call: dpi_plan_build followed by dpi_lookup,
+ * or -- for small / short-bag batches, where the second launch and the plan's trip through global memory are half of the
+ * step (the paper's motivation: 4.75 us of work behind 21.92 us of launch overhead; "a single parallel
+ * operation") -- ONE fused launch in which the CTA that scans a run of bags pools those bags right away.
+ * Either way the plan is left built exactly as dpi_plan_build leaves it (offsets, segments, meta: bit-identical), so
+ * dpi_plan_export / dpi_plan_device_views / later dpi_lookup calls on the same batch work unchanged, and the output block
+ * is the one dpi_lookup writes. Which way is taken depends on host-known facts only (DPI_OPT_FUSED).
+ * Arguments as in dpi_plan_build + dpi_lookup (plan's own offsets; indices int32 / int64 per the plan's index type).
+ * Asynchronous on `stream`.
+ */
+dpi_status_t dpi_forward(dpi_plan_t* plan, const int32_t* lengths_dev, const void* const* table_ptrs_dev,
+                         const void* indices_dev, const uint8_t* pooling, void* out_dev, void* stream);
+
+/*
+ * dpi_plan_status -- did any build of this plan since the last call exceed its capacity (N > max_indices)? Such a build
+ * leaves S = 0 behind, so the balanced-segment lookup that follows writes nothing; the planner also bumps a sticky device
+ * counter, which this call reads (synchronises `stream`) and clears. DPI_OK and *overflowed_builds = 0 when all builds
+ * fitted, DPI_ERR_INVALID_ARG and the count otherwise. overflowed_builds may be NULL. Off the hot path: call it once per
+ * served batch group, not per lookup.
+ */
+dpi_status_t dpi_plan_status(const dpi_plan_t* plan, int32_t* overflowed_builds, void* stream);
 
 /*
  * dpi_lookup_ex -- step a3 with the interface variants: the same fused gather-and-pool,
@@ -285,8 +327,7 @@ dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int
  * internal streams ordered after `stream`, so both PCIe directions and the SMs are busy at once. Each chunk is an
  * independent sub-batch with its own device plan (bags are independent); the host only adds up how many
  * index entries each chunk owns, to size the copies. The result is identical to the unchunked call.
- * Because the lengths are host-resident here, the longest bag of the batch is known exactly, and the call picks the a3 variant
- * from it (as DPI_OPT_MAX_BAG_HINT would) without any promise from the caller.
+ * Each chunk runs as dpi_forward does: one fused launch when eligible, else planner + lookup.
  * Tables stay resident on the device (they are the model, not a per-batch input).
  *   lengths_host int32[G]; indices_host int32 / int64 [n_indices] per the plan's index type
  *   (n_indices <= max_indices); out_host [B, sum dims].

@@ -120,9 +120,19 @@ def alg1_onehot(tables: Sequence[np.ndarray], dtype: int, ids: np.ndarray) -> np
     return out
 
 
+def _out_block(out, B: int, width: int) -> np.ndarray:
+    """The caller's float64 [B, width] block (timing loops reuse one), or a fresh one."""
+    if out is None:
+        return np.empty((B, width), dtype=np.float64)
+    if out.dtype != np.float64 or out.shape != (B, width) or not out.flags.c_contiguous:
+        raise ValueError("out must be a C-contiguous float64 [B, T*D] array")
+    return out
+
+
 def lookup(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray, offsets: np.ndarray,
-           pooling: np.ndarray) -> np.ndarray:
-    """Pooled multi-hot lookup. Returns the unrounded float64 reference [B, T*D]."""
+           pooling: np.ndarray, out: np.ndarray = None) -> np.ndarray:
+    """Pooled multi-hot lookup. Returns the unrounded float64 reference [B, T*D] (written into `out` when
+    given)."""
     T = len(tables)
     D = int(np.asarray(tables[0]).shape[1])
     indices = np.ascontiguousarray(indices, dtype=np.int32)
@@ -133,7 +143,7 @@ def lookup(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray
     if int(offsets[-1]) > indices.shape[0]:
         raise ValueError("offsets[-1] exceeds len(indices)")
     ptrs, rows, keep = _table_ptrs(tables, dtype, D)
-    ref = np.empty((B, T * D), dtype=np.float64)
+    ref = _out_block(out, B, T * D)
     _check(_load().oracle_lookup(T, B, D, dtype, ctypes.cast(ptrs, ctypes.c_void_p), rows.ctypes.data,
                                  indices.ctypes.data, offsets.ctypes.data, pooling.ctypes.data,
                                  ref.ctypes.data))
@@ -142,7 +152,7 @@ def lookup(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray
 
 
 def lookup_par(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.ndarray, offsets: np.ndarray,
-               pooling: np.ndarray):
+               pooling: np.ndarray, out: np.ndarray = None):
     """oracle_lookup on all host cores (OpenMP over samples; bit-identical block). Returns (ref float64[B, T*D],
     threads used). bench.py's cpu_baseline timing leg; the tests pin it to lookup()."""
     T = len(tables)
@@ -155,7 +165,7 @@ def lookup_par(tables: Sequence[np.ndarray], dtype: int, B: int, indices: np.nda
     if int(offsets[-1]) > indices.shape[0]:
         raise ValueError("offsets[-1] exceeds len(indices)")
     ptrs, rows, keep = _table_ptrs(tables, dtype, D)
-    ref = np.empty((B, T * D), dtype=np.float64)
+    ref = _out_block(out, B, T * D)
     team = ctypes.c_int32(0)
     _check(_load().oracle_lookup_par(T, B, D, dtype, ctypes.cast(ptrs, ctypes.c_void_p), rows.ctypes.data,
                                      indices.ctypes.data, offsets.ctypes.data, pooling.ctypes.data,

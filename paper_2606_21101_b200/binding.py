@@ -19,7 +19,7 @@ STATUS_NAMES = {0: "DPI_OK", 1: "DPI_ERR_INVALID_ARG", 2: "DPI_ERR_UNSUPPORTED",
                 4: "DPI_ERR_CUDA", 5: "DPI_ERR_INDEX_RANGE"}
 DPI_F32, DPI_F16, DPI_BF16 = 0, 1, 2
 DPI_POOL_SUM, DPI_POOL_MEAN = 0, 1
-OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL, OPT_HOST_CHUNKS, OPT_HOST_DIRECT_OUT, OPT_MAX_BAG_HINT = range(9)
+OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL, OPT_HOST_CHUNKS, OPT_HOST_DIRECT_OUT, OPT_MAX_BAG_HINT, OPT_FUSED, OPT_FUSED_MAX_BAGS = range(11)
 BAGS_SAMPLE_MAJOR, BAGS_TABLE_MAJOR = 0, 1
 IDX_I32, IDX_I64 = 0, 1
 LOOKUP_FORCE_GENERAL = 1
@@ -27,8 +27,8 @@ LOOKUP_FORCE_GENERAL = 1
 # every symbol include/dpi.h declares (tests check the .so exports each one)
 EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "dpi_plan_set_columns", "dpi_plan_out_width", "dpi_lookup_ex",
            "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
-           "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export",
-           "dpi_lookup", "dpi_lookup_onehot", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
+           "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export", "dpi_plan_stats",
+           "dpi_lookup", "dpi_forward", "dpi_plan_status", "dpi_lookup_onehot", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
            "dpi_version", "dpi_status_string", "dpi_last_error"]
 
 
@@ -80,8 +80,11 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
         "dpi_plan_device_views": (st, [vp, vp, vp, vp]),
         "dpi_plan_info": (st, [vp, vp, vp, vp, vp, vp, vp, vp]),
         "dpi_plan_export": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
+        "dpi_plan_stats": (st, [vp, vp, vp, vp]),
         "dpi_lookup": (st, [vp, vp, vp, vp, vp, vp, vp]),
         "dpi_lookup_input_first": (st, [vp, vp, vp, vp, vp, vp, vp]),
+        "dpi_forward": (st, [vp, vp, vp, vp, vp, vp, vp]),
+        "dpi_plan_status": (st, [vp, vp, vp]),
         "dpi_lookup_onehot": (st, [vp, vp, vp, vp, vp]),
         "dpi_forward_host": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_check_indices": (st, [vp, vp, vp, vp]),
@@ -151,6 +154,20 @@ class Plan:
         self.out_dtype = int(dtype)
         self.G = self.T * self.B
         self.max_indices = int(max_indices)
+
+    @classmethod
+    def _adopt(cls, handle, rows, dims, dtype, B, max_indices) -> "Plan":
+        """Wrap a handle the library already created (dpi_plan)."""
+        self = cls.__new__(cls)
+        self._lib = load_library()
+        self._h = handle
+        self.T, self.B, self.D, self.dtype = int(rows.shape[0]), int(B), int(dims.max()), int(dtype)
+        self.dims = dims.copy()
+        self.out_width = int(dims.sum())
+        self.out_dtype = int(dtype)
+        self.G = self.T * self.B
+        self.max_indices = int(max_indices)
+        return self
 
     # -- lifetime --------------------------------------------------------------------------------------
     def destroy(self):
@@ -227,11 +244,33 @@ class Plan:
         res = (offsets, seg[: S.value + 1].copy(), int(S.value), int(N.value))
         return res + (seg_off[: S.value + 1].copy(),) if with_seg_off else res
 
+    # -- dpi_plan_stats -------------------------------------------------------------------------------------
+    def stats(self, stream=None):
+        """(min_len, max_len) of the last built batch (synchronises)."""
+        lo, hi = ctypes.c_int32(), ctypes.c_int32()
+        _check(self._lib.dpi_plan_stats(self._h, ctypes.byref(lo), ctypes.byref(hi), _stream_handle(stream)))
+        return int(lo.value), int(hi.value)
+
     # -- dpi_lookup -----------------------------------------------------------------------------------------
     def lookup(self, table_ptrs_dev, indices_dev, out_dev, pooling=None, offsets_dev=None, stream=None):
         pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
         _check(self._lib.dpi_lookup(_ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(offsets_dev), self._h,
                                     _ptr(pool), _ptr(out_dev), _stream_handle(stream)))
+
+    # -- dpi_forward (a1 + a2 + a3 in one call; one fused launch on small / short-bag batches) ------------------
+    def forward(self, lengths_dev, table_ptrs_dev, indices_dev, out_dev, pooling=None, stream=None):
+        pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
+        _check(self._lib.dpi_forward(self._h, _ptr(lengths_dev), _ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(pool),
+                                     _ptr(out_dev), _stream_handle(stream)))
+
+    # -- dpi_plan_status ------------------------------------------------------------------------------------
+    def status(self, stream=None) -> int:
+        """Number of builds since the last call that overflowed the plan's capacity (synchronises; clears the count)."""
+        n = ctypes.c_int32(0)
+        st = self._lib.dpi_plan_status(self._h, ctypes.byref(n), _stream_handle(stream))
+        if st not in (DPI_OK, 1):
+            _check(st)
+        return int(n.value)
 
     # -- dpi_lookup_ex ----------------------------------------------------------------------------------------
     def lookup_ex(self, table_ptrs_dev, indices_dev, out_dev, pooling=None, offsets_dev=None, weights_dev=None,
@@ -270,10 +309,15 @@ class Plan:
 
 
 def dpi_plan(table_rows, dims, dtype: int, lengths_dev, B: int, max_indices: int, stream=None) -> Plan:
-    """north_star spelling: create + build."""
-    p = Plan(table_rows, dims, dtype, B, max_indices)
-    p.build(lengths_dev, stream)
-    return p
+    """north_star spelling, the C entry point `dpi_plan` (create + build in one call)."""
+    lib = load_library()
+    rows = np.ascontiguousarray(table_rows, dtype=np.int64)
+    T = rows.shape[0]
+    dims_a = np.ascontiguousarray(np.broadcast_to(np.asarray(dims, dtype=np.int32), (T,)))
+    handle = ctypes.c_void_p()
+    _check(lib.dpi_plan(rows.ctypes.data, T, dims_a.ctypes.data, int(dtype), _ptr(lengths_dev), int(B), int(max_indices),
+                        _stream_handle(stream), ctypes.byref(handle)))
+    return Plan._adopt(handle, rows, dims_a, dtype, B, max_indices)
 
 
 def dpi_lookup(table_ptrs_dev, indices_dev, offsets_dev, plan: Plan, pooling, out_dev, stream=None):
@@ -300,7 +344,17 @@ def _synth_lib():
         _synth.dpi_synth_row_read_probe.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint64,
                                                     ctypes.c_uint64, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                                     ctypes.c_void_p, ctypes.c_void_p]
+        _synth.dpi_synth_copy_words.restype = ctypes.c_int
+        _synth.dpi_synth_copy_words.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64]
     return _synth
+
+
+def copy_device_words(dst_dev, src_ptr: int, n_words: int):
+    """Test helper: device-to-device copy of n_words 32-bit words from a raw device address (e.g. a borrowed pointer of
+    dpi_plan_device_views) into a tensor; synchronous."""
+    rc = _synth_lib().dpi_synth_copy_words(_ptr(dst_dev), int(src_ptr), int(n_words))
+    if rc != 0:
+        raise RuntimeError(f"dpi_synth_copy_words failed with cudaError {rc}")
 
 
 def synth_row_read_probe(base_dev, span_rows: int, row_bytes: int, n_rows: int, key: int, random: bool, unroll: int,

@@ -76,7 +76,7 @@ struct dpi_plan_s {
     int32_t K_user = 0;      // 0 = default
     uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
     uint32_t num_tiles = 0, num_chunks = 0, tiles_per_chunk = 0;
-    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 1, 0, 0, 0};  // PDL on: 4-10 % per step on small batches, neutral on large ones
+    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 1, 0, 0, 0, 0, 0};  // PDL on: 4-10 % per step on small batches, neutral on large ones
     // device
     int device = 0, num_sms = 0;
     int32_t* offsets = nullptr;
@@ -94,8 +94,14 @@ struct dpi_plan_s {
     size_t stage_idx_bytes = 0;
     void* stage_out = nullptr;
     struct HostPipeline* pipe = nullptr;   // dpi_forward_host: sample-chunked sub-plans + copy/compute streams
-    int32_t hint_override = 0;   // dpi_forward_host: longest bag of THIS batch, known exactly from the host-resident lengths
     bool built = false;
+    // Launch configurations, computed when the plan is created or re-configured (prepare_launches): occupancy queries
+    // and shared-memory attributes happen there, for the plan's device -- a lookup only fills in pointers and launches.
+    LookupLaunch launch_dense{}, launch_gen{}, launch_gen_w{};   // balanced-segment kernel: dense / general / general + weights
+    int direct_grid_cap = 0;       // short-bag variant as its own launch: SMs x resident CTAs
+    uint32_t fused_chunks = 0;     // fused single-launch path: CTAs (0 = no instantiation) and bags per CTA
+    uint32_t fused_chunk_bags = 0;
+    std::vector<int64_t> columns;  // dpi_plan_set_columns, kept for the sub-plans of dpi_forward_host
 };
 
 // dpi_forward_host cuts a large batch into chunks of whole samples; chunk c runs H2D -> plan -> lookup -> D2H on
@@ -131,9 +137,10 @@ uint32_t seg_capacity_for(const dpi_plan_t* p, int32_t K) {
 dpi_status_t ensure_seg_capacity(dpi_plan_t* p, int32_t K) {
     const uint32_t need = seg_capacity_for(p, K);
     if (need <= p->seg_cap && p->seg) return DPI_OK;
-    if (p->seg) DPI_CUDA(cudaFree(p->seg));
-    p->seg = nullptr;
-    DPI_CUDA(cudaMalloc(&p->seg, static_cast<size_t>(need) * sizeof(int2)));
+    int2* fresh = nullptr;
+    DPI_CUDA(cudaMalloc(&fresh, static_cast<size_t>(need) * sizeof(int2)));   // on failure the old buffer stays in place
+    if (p->seg) (void)cudaFree(p->seg);
+    p->seg = fresh;
     p->seg_cap = need;
     return DPI_OK;
 }
@@ -151,32 +158,57 @@ void free_plan(dpi_plan_t* p) {
     delete p;
 }
 
-int occupancy(const dpi_plan_t* p, const LookupArgs& a, const LookupLaunch& l) {
+int prepare(const dpi_plan_t* p, const LookupArgs& a, const LookupLaunch& l) {
     switch (p->dtype) {
-        case DPI_F32: return lookup_occupancy_f32(a, l);
-        case DPI_F16: return lookup_occupancy_f16(a, l);
-        default: return lookup_occupancy_bf16(a, l);
+        case DPI_F32: return lookup_prepare_f32(a, l);
+        case DPI_F16: return lookup_prepare_f16(a, l);
+        default: return lookup_prepare_bf16(a, l);
     }
 }
 
-LookupLaunch choose_launch(const dpi_plan_t* p, const LookupArgs& a, bool general) {
+LookupLaunch prepare_one_launch(const dpi_plan_t* p, bool general, bool weights) {
+    LookupArgs a{};   // only T, idx_shift and weights != NULL enter the shared-memory size
+    a.T = static_cast<uint32_t>(p->T);
+    a.idx_shift = p->index_type == DPI_IDX_I64 ? 1u : 0u;
+    a.weights = weights ? reinterpret_cast<const float*>(sizeof(float)) : nullptr;
     LookupLaunch l{};
     l.lanes = p->lanes;
     l.general = general;
-    l.unroll = (p->opt[DPI_OPT_UNROLL] && !general) ? p->opt[DPI_OPT_UNROLL] : 2;  // x2 by double buffering (sweeps_r01.md)
+    l.unroll = (p->opt[DPI_OPT_UNROLL] && !general) ? p->opt[DPI_OPT_UNROLL] : 2;  // x2 by double buffering
     l.block_threads = p->opt[DPI_OPT_BLOCK_THREADS] ? p->opt[DPI_OPT_BLOCK_THREADS] : 256;
     l.out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
-    int per_sm = p->opt[DPI_OPT_BLOCKS_PER_SM];
-    if (per_sm <= 0) {
-        per_sm = occupancy(p, a, l);
-        if (per_sm <= 0) per_sm = 1;
-    }
+    int per_sm = prepare(p, a, l);   // also raises the instantiation's dynamic shared-memory limit when needed
+    if (p->opt[DPI_OPT_BLOCKS_PER_SM] > 0) per_sm = p->opt[DPI_OPT_BLOCKS_PER_SM];
+    if (per_sm <= 0) per_sm = 1;
     l.grid = p->num_sms * per_sm;  // persistent: a whole number of waves, every CTA resident
     const int64_t warps_per_cta = l.block_threads / 32;
     const int64_t need = (static_cast<int64_t>(p->seg_cap) + warps_per_cta - 1) / warps_per_cta;  // one warp per possible task
     if (need < l.grid) l.grid = static_cast<int>(need > 0 ? need : 1);
     l.pdl = p->opt[DPI_OPT_PDL] != 0;
     return l;
+}
+
+// Everything a launch needs that costs a CUDA runtime call. Runs in dpi_plan_create and in every setter that changes an
+// input of it (options, quantum, output dtype, layout) -- never in dpi_lookup / dpi_forward.
+void prepare_launches(dpi_plan_t* p) {
+    p->launch_dense = prepare_one_launch(p, false, false);
+    p->launch_gen = prepare_one_launch(p, true, false);
+    p->launch_gen_w = prepare_one_launch(p, true, true);
+    const bool out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
+    p->direct_grid_cap = p->num_sms * direct_occupancy(p->dtype, out32, p->lanes, static_cast<uint32_t>(p->T));
+    // fused single-launch path: at most one resident wave, at most kFusedMaxChunks chunks (one look-back record per
+    // thread), and no chunk smaller than one bag per lane group
+    const int occ = fused_occupancy(p->dtype, out32, p->lanes, static_cast<uint32_t>(p->T));
+    p->fused_chunks = 0;
+    p->fused_chunk_bags = 0;
+    if (occ > 0) {
+        uint64_t chunks = std::min<uint64_t>(kFusedMaxChunks, static_cast<uint64_t>(p->num_sms) * occ);
+        const uint32_t min_bags = static_cast<uint32_t>(kFusedThreads / p->lanes);
+        chunks = std::min<uint64_t>(chunks, (static_cast<uint64_t>(p->G) + min_bags - 1) / min_bags);
+        if (chunks < 1) chunks = 1;
+        p->fused_chunk_bags = static_cast<uint32_t>((p->G + chunks - 1) / chunks);
+        p->fused_chunks = (p->G + p->fused_chunk_bags - 1) / p->fused_chunk_bags;
+    }
 }
 
 void free_pipeline(dpi_plan_t* p) {
@@ -256,21 +288,22 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
         if (e != cudaSuccess) return cuda_fail(e, "input-first kernel launch");
         return DPI_OK;
     }
-    const int32_t hint = p->hint_override > 0 ? p->hint_override : p->opt[DPI_OPT_MAX_BAG_HINT];
-    // Short-bag variant (lookup_direct.cu) when the caller promised bags of <= 8 entries. Measured on B200: with
-    // multi-hot bags (promise 2..8) it wins at every batch size; with at most ONE entry per bag the balanced-segment kernel's
-    // row-copy path overtakes it once there are more than ~5e5 bags (its index prefetch pipeline pays off at that size).
-    const bool short_bags = hint >= 2 ? hint <= 8 : (hint == 1 && p->G <= 500000u);
+    // Without a hint lookup_kernel reads a1's max_len on the device and takes the short-bag body by the same rule
+    // (short_bag_rule); the OPTIONAL promise DPI_OPT_MAX_BAG_HINT (or DPI_OPT_MODE = 6) picks the short-bag variant as its own
+    // launch on the host. Measured on B200: with multi-hot bags of <= 8 entries it wins at every batch size;
+    // with at most ONE entry per bag the balanced-segment kernel's row-copy path overtakes it beyond ~5e5 bags.
+    const int32_t hint = p->opt[DPI_OPT_MAX_BAG_HINT];
+    const bool short_bags = hint >= 1 && short_bag_rule(static_cast<uint32_t>(hint), p->G);
     // the short-bag variant also takes int64 ids (the one interface variant every framework feeds)
     const bool general_but_ids = c.force_general || p->mixed_dims || p->custom_columns || a.table_major || c.weights || c.peers ||
                                  ld != p->out_width;
     if (!general_but_ids && (p->opt[DPI_OPT_MODE] == 6 || (p->opt[DPI_OPT_MODE] == 0 && short_bags))) {
-        cudaError_t e = launch_direct(a, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->num_sms,
+        cudaError_t e = launch_direct(a, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->direct_grid_cap,
                                       p->opt[DPI_OPT_PDL] != 0, stream);
         if (e != cudaSuccess) return cuda_fail(e, "direct lookup kernel launch");
         return DPI_OK;
     }
-    const LookupLaunch l = choose_launch(p, a, general);
+    const LookupLaunch& l = !general ? p->launch_dense : (c.weights ? p->launch_gen_w : p->launch_gen);
     cudaError_t e;
     switch (p->dtype) {
         case DPI_F32: e = launch_lookup_f32(a, l, stream); break;
@@ -291,6 +324,79 @@ dpi_status_t check_lookup_pointers(const dpi_plan_t* p, const void* tables, cons
     const uintptr_t idx_align = p->index_type == DPI_IDX_I64 ? 7u : 3u;
     if (reinterpret_cast<uintptr_t>(indices) & idx_align) return fail(DPI_ERR_INVALID_ARG, "indices_dev is not %d-byte aligned", (int)idx_align + 1);
     return DPI_OK;
+}
+
+PlanArgs plan_args(const dpi_plan_t* p, const int32_t* lengths_dev) {
+    PlanArgs a{};
+    a.len = lengths_dev;
+    a.offsets = p->offsets;
+    a.seg = p->seg;
+    a.meta = p->meta;
+    a.status = p->status;
+    a.state = p->state;
+    a.G = p->G;
+    a.K = static_cast<uint32_t>(p->K);
+    a.seg_cap = p->seg_cap;
+    a.num_tiles = p->num_tiles;
+    a.num_chunks = p->num_chunks;
+    a.tiles_per_chunk = p->tiles_per_chunk;
+    a.max_indices = static_cast<uint32_t>(p->max_indices);
+    return a;
+}
+
+// Default ceiling of the fused single-launch path (bags). Measured on B200: below it one launch beats
+// plan + lookup on every short-bag shape tried; above it the statically chunked CTAs lose to the persistent kernels.
+constexpr uint64_t kFusedDefaultMaxBags = 1u << 20;
+
+// May this call run as ONE launch (forward_fused.cu)? Host-known facts only: the layout is the dense one, and the plan's
+// capacity says bags are short on average (max_indices <= 8 * G) -- the fused kernel is correct for any bag length but
+// does not balance load across CTAs, so long-bag batches keep the planner + balanced-segment lookup.
+bool fused_eligible(const dpi_plan_t* p, const LookupCall& c) {
+    if (p->fused_chunks == 0 || p->opt[DPI_OPT_FUSED] == 2 || p->opt[DPI_OPT_MODE] != 0) return false;
+    if (c.force_general || p->mixed_dims || p->custom_columns || p->bag_order != DPI_BAGS_SAMPLE_MAJOR || c.weights || c.peers ||
+        c.offsets || (c.out_ld && c.out_ld != p->out_width))
+        return false;
+    if (p->opt[DPI_OPT_FUSED] == 1) return true;
+    const uint64_t max_bags = p->opt[DPI_OPT_FUSED_MAX_BAGS] > 0 ? static_cast<uint64_t>(p->opt[DPI_OPT_FUSED_MAX_BAGS]) : kFusedDefaultMaxBags;
+    return p->G <= max_bags && static_cast<uint64_t>(p->max_indices) <= 8ull * p->G;
+}
+
+dpi_status_t launch_fused_forward(dpi_plan_t* p, const int32_t* lengths_dev, const LookupCall& c, cudaStream_t stream) {
+    FusedArgs f{};
+    f.plan = plan_args(p, lengths_dev);
+    f.plan.num_chunks = p->fused_chunks;
+    f.chunk_bags = p->fused_chunk_bags;
+    LookupArgs& a = f.look;
+    a.tables = c.tables;
+    a.indices = static_cast<const int32_t*>(c.indices);
+    a.offsets = p->offsets;
+    a.seg = p->seg;
+    a.meta = p->meta;
+    a.out = c.out;
+    a.G = p->G;
+    a.T = static_cast<uint32_t>(p->T);
+    a.B = static_cast<uint32_t>(p->B);
+    a.nvec = p->nvec;
+    a.idx_shift = p->index_type == DPI_IDX_I64 ? 1u : 0u;
+    std::memset(&a.pool, 0, sizeof a.pool);
+    if (c.pooling) {
+        for (int t = 0; t < p->T; ++t) {
+            if (c.pooling[t] > 1) return fail(DPI_ERR_INVALID_ARG, "pooling[%d] = %d is not a dpi_pool_t", t, c.pooling[t]);
+            if (c.pooling[t] == DPI_POOL_MEAN) a.pool.w[t >> 5] |= 1u << (t & 31);
+        }
+    }
+    cudaError_t e = launch_fused(f, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->opt[DPI_OPT_PDL] != 0, stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fused forward kernel launch");
+    p->built = true;
+    return DPI_OK;
+}
+
+// a1 + a2 + a3 on device-resident inputs: one launch when fused_eligible(), else the planner launch followed by the lookup.
+dpi_status_t forward_device(dpi_plan_t* p, const int32_t* lengths_dev, const LookupCall& c, cudaStream_t stream) {
+    if (fused_eligible(p, c)) return launch_fused_forward(p, lengths_dev, c, stream);
+    dpi_status_t st = dpi_plan_build(p, lengths_dev, stream);
+    if (st != DPI_OK) return st;
+    return do_lookup(p, c, stream);
 }
 
 }  // namespace
@@ -374,10 +480,11 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     DPI_TRY(cudaMalloc(&p->offsets, (static_cast<size_t>(p->G) + 1) * sizeof(int32_t)));
     DPI_TRY(cudaMalloc(&p->meta, kMetaWords * sizeof(int32_t)));
     DPI_TRY(cudaMemset(p->meta, 0, kMetaWords * sizeof(int32_t)));
-    DPI_TRY(cudaMalloc(&p->status, kMaxChunks * sizeof(ulonglong2)));
-    DPI_TRY(cudaMemset(p->status, 0, kMaxChunks * sizeof(ulonglong2)));
+    DPI_TRY(cudaMalloc(&p->status, kStatusRecords * sizeof(ulonglong2)));
+    DPI_TRY(cudaMemset(p->status, 0, kStatusRecords * sizeof(ulonglong2)));
     {
-        const unsigned int init[kStateWords] = {0u, 0u, 1u, 0u};  // ticket, done, epoch = 1 (status words start at 0)
+        // ticket, done, epoch = 1 (status words start at 0), overflowed builds, running min / max length
+        const unsigned int init[kStateWords] = {0u, 0u, 1u, 0u, 0xffffffffu, 0u, 0u, 0u};
         DPI_TRY(cudaMalloc(&p->state, sizeof init));
         DPI_TRY(cudaMemcpy(p->state, init, sizeof init, cudaMemcpyHostToDevice));
     }
@@ -400,6 +507,7 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
 #undef DPI_TRY
     dpi_status_t st = ensure_seg_capacity(p, p->K);
     if (st != DPI_OK) { free_plan(p); return st; }
+    prepare_launches(p);
     *plan = p;
     return DPI_OK;
 }
@@ -407,9 +515,15 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
 dpi_status_t dpi_plan_set_quantum(dpi_plan_t* p, int32_t K) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
     if (K < 0) return fail(DPI_ERR_INVALID_ARG, "K=%d must be >= 0", K);
+    const int32_t K_new = K ? K : default_quantum(p);
+    // the segment buffer may be re-allocated and the old records describe another quantum: whatever was built is gone
+    p->built = false;
+    dpi_status_t st = ensure_seg_capacity(p, K_new);
+    if (st != DPI_OK) return st;   // K unchanged: the plan still matches its (old, intact or re-allocated larger) buffer
     p->K_user = K;
-    p->K = K ? K : default_quantum(p);
-    return ensure_seg_capacity(p, p->K);
+    p->K = K_new;
+    prepare_launches(p);           // the persistent grid is capped by the segment capacity
+    return DPI_OK;
 }
 
 dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
@@ -425,10 +539,15 @@ dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
         case DPI_OPT_HOST_CHUNKS: ok = v >= 0 && v <= 64; break;
         case DPI_OPT_HOST_DIRECT_OUT: ok = v >= 0 && v <= 2; break;
         case DPI_OPT_MAX_BAG_HINT: ok = v >= 0; break;
+        case DPI_OPT_FUSED: ok = v >= 0 && v <= 2; break;
+        case DPI_OPT_FUSED_MAX_BAGS: ok = v >= 0; break;
         default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);
     }
     if (!ok) return fail(DPI_ERR_INVALID_ARG, "value %d not supported for option %d", v, (int)opt);
+    if (p->opt[opt] == v) return DPI_OK;
     p->opt[opt] = v;
+    if (opt == DPI_OPT_UNROLL || opt == DPI_OPT_BLOCK_THREADS || opt == DPI_OPT_BLOCKS_PER_SM || opt == DPI_OPT_PDL)
+        prepare_launches(p);
     return DPI_OK;
 }
 
@@ -442,20 +561,7 @@ dpi_status_t dpi_plan_build(dpi_plan_t* p, const int32_t* lengths_dev, void* str
     if (!p || !lengths_dev) return fail(DPI_ERR_INVALID_ARG, "plan/lengths_dev is NULL");
     if (reinterpret_cast<uintptr_t>(lengths_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "lengths_dev is not 4-byte aligned");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    PlanArgs a{};
-    a.len = lengths_dev;
-    a.offsets = p->offsets;
-    a.seg = p->seg;
-    a.meta = p->meta;
-    a.status = p->status;
-    a.state = p->state;
-    a.G = p->G;
-    a.K = static_cast<uint32_t>(p->K);
-    a.seg_cap = p->seg_cap;
-    a.num_tiles = p->num_tiles;
-    a.num_chunks = p->num_chunks;
-    a.tiles_per_chunk = p->tiles_per_chunk;
-    a.max_indices = static_cast<uint32_t>(p->max_indices);
+    const PlanArgs a = plan_args(p, lengths_dev);
     cudaError_t e = launch_plan(a, s);
     if (e != cudaSuccess) return cuda_fail(e, "plan kernel launch");
     p->built = true;
@@ -523,10 +629,25 @@ dpi_status_t dpi_plan_export(const dpi_plan_t* p, int32_t* offsets_host, int32_t
     return DPI_OK;
 }
 
+dpi_status_t dpi_plan_stats(const dpi_plan_t* p, int32_t* min_len, int32_t* max_len, void* stream) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int32_t meta[kMetaWords];
+    DPI_CUDA(cudaMemcpyAsync(meta, p->meta, sizeof meta, cudaMemcpyDeviceToHost, s));
+    DPI_CUDA(cudaStreamSynchronize(s));
+    if (min_len) *min_len = meta[META_MINLEN];
+    if (max_len) *max_len = meta[META_MAXLEN];
+    return DPI_OK;
+}
+
 dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* p, dpi_dtype_t out_dtype) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
     if (out_dtype != p->dtype && out_dtype != DPI_F32) return fail(DPI_ERR_UNSUPPORTED, "output dtype %d: must be the table dtype or DPI_F32", (int)out_dtype);
-    p->out_dtype = out_dtype;
+    if (p->out_dtype != out_dtype) {
+        p->out_dtype = out_dtype;
+        prepare_launches(p);
+    }
     return DPI_OK;
 }
 
@@ -553,6 +674,33 @@ dpi_status_t dpi_lookup_ex(const dpi_lookup_args_t* args, const dpi_plan_t* p, v
     c.peers = args->out_peers_dev; c.n_peers = args->n_peers; c.rows_per_peer = args->rows_per_peer;
     c.force_general = (args->flags & DPI_LOOKUP_FORCE_GENERAL) != 0;
     return do_lookup(p, c, static_cast<cudaStream_t>(stream));
+}
+
+dpi_status_t dpi_forward(dpi_plan_t* p, const int32_t* lengths_dev, const void* const* table_ptrs_dev, const void* indices_dev,
+                         const uint8_t* pooling, void* out_dev, void* stream) {
+    if (!p || !lengths_dev) return fail(DPI_ERR_INVALID_ARG, "plan/lengths_dev is NULL");
+    if (reinterpret_cast<uintptr_t>(lengths_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "lengths_dev is not 4-byte aligned");
+    const bool was_built = p->built;
+    p->built = true;   // check_lookup_pointers only wants a plan that will be built by the time the lookup runs
+    dpi_status_t st = check_lookup_pointers(p, table_ptrs_dev, indices_dev, out_dev);
+    p->built = was_built;
+    if (st != DPI_OK) return st;
+    LookupCall c;
+    c.tables = table_ptrs_dev; c.indices = indices_dev; c.pooling = pooling; c.out = out_dev;
+    return forward_device(p, lengths_dev, c, static_cast<cudaStream_t>(stream));
+}
+
+dpi_status_t dpi_plan_status(const dpi_plan_t* p, int32_t* overflowed_builds, void* stream) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    unsigned int n = 0;
+    DPI_CUDA(cudaMemcpyAsync(&n, p->state + kStateOverflows, sizeof n, cudaMemcpyDeviceToHost, s));
+    DPI_CUDA(cudaStreamSynchronize(s));
+    if (overflowed_builds) *overflowed_builds = static_cast<int32_t>(n > 0x7fffffffu ? 0x7fffffffu : n);
+    if (n == 0) return DPI_OK;
+    DPI_CUDA(cudaMemsetAsync(p->state + kStateOverflows, 0, sizeof n, s));   // reported once
+    return fail(DPI_ERR_INVALID_ARG, "%u build(s) since the last dpi_plan_status exceeded the plan's capacity (N > max_indices=%lld): "
+                "their lookups wrote nothing", n, (long long)p->max_indices);
 }
 
 dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,
@@ -583,8 +731,10 @@ dpi_status_t dpi_plan_set_layout(dpi_plan_t* p, dpi_bag_order_t order, dpi_index
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
     if (order != DPI_BAGS_SAMPLE_MAJOR && order != DPI_BAGS_TABLE_MAJOR) return fail(DPI_ERR_INVALID_ARG, "unknown bag order %d", (int)order);
     if (index_type != DPI_IDX_I32 && index_type != DPI_IDX_I64) return fail(DPI_ERR_INVALID_ARG, "unknown index type %d", (int)index_type);
+    const bool changed = p->index_type != index_type;
     p->bag_order = order;
     p->index_type = index_type;
+    if (changed) prepare_launches(p);   // int64 ids double the staged index words of the general kernel
     return DPI_OK;
 }
 
@@ -610,6 +760,7 @@ dpi_status_t dpi_plan_set_columns(dpi_plan_t* p, const int64_t* columns) {
     }
     DPI_CUDA(cudaMemcpy(p->tab_col_dev, col.data(), p->T * sizeof(uint32_t), cudaMemcpyHostToDevice));
     p->custom_columns = columns != nullptr;
+    if (columns) p->columns.assign(columns, columns + p->T); else p->columns.clear();
     p->out_width = width;
     if (p->stage_out) { DPI_CUDA(cudaFree(p->stage_out)); p->stage_out = nullptr; }
     free_pipeline(p);
@@ -626,16 +777,14 @@ namespace {
 
 // Sum of lengths[g0, g1) and whether any of them is negative: branch-free so that the host compiler vectorises it (the
 // loop runs once per dpi_forward_host call over all G lengths; with an early return inside it cost 0.15 ms at G = 360 K).
-bool sum_lengths(const int32_t* lengths, size_t g0, size_t g1, int64_t* total, int32_t* longest) {
+bool sum_lengths(const int32_t* lengths, size_t g0, size_t g1, int64_t* total) {
     int64_t sum = 0;
-    int32_t sign = 0, mx = 0;
+    int32_t sign = 0;
     for (size_t g = g0; g < g1; ++g) {
         sum += lengths[g];
         sign |= lengths[g];
-        mx = lengths[g] > mx ? lengths[g] : mx;
     }
     *total = sum;
-    if (*longest < mx) *longest = mx;
     return sign < 0;
 }
 
@@ -649,6 +798,27 @@ int host_chunks(const dpi_plan_t* p, size_t bytes_moved) {
     }
     if (n > p->B) n = p->B;
     return n < 1 ? 1 : n;
+}
+
+// A chunk's sub-plan follows its parent's layout and options: output dtype, id width, column placement (the sub-plan writes
+// rows of the parent's width at the parent's columns), quantum and tuning knobs. Launch configurations are re-derived only
+// when something changed.
+dpi_status_t sync_subplan(const dpi_plan_t* p, dpi_plan_t* q) {
+    bool changed = q->out_dtype != p->out_dtype || q->index_type != p->index_type;
+    q->out_dtype = p->out_dtype;
+    q->index_type = p->index_type;
+    q->bag_order = p->bag_order;
+    for (int o = 0; o < DPI_OPT_COUNT_; ++o) {
+        changed |= q->opt[o] != p->opt[o];
+        q->opt[o] = p->opt[o];
+    }
+    if (p->custom_columns != q->custom_columns || p->columns != q->columns) {
+        dpi_status_t st = dpi_plan_set_columns(q, p->custom_columns ? p->columns.data() : nullptr);
+        if (st != DPI_OK) return st;
+    }
+    if (p->K_user && q->K != p->K_user) return dpi_plan_set_quantum(q, p->K_user);   // re-derives the launches as well
+    if (changed) prepare_launches(q);
+    return DPI_OK;
 }
 
 dpi_status_t ensure_pipeline(dpi_plan_t* p, int n_chunks) {
@@ -717,18 +887,13 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     const int n_chunks = host_chunks(p, static_cast<size_t>(p->G) * 4 + static_cast<size_t>(n_indices) * idx_elt + out_bytes);
     if (n_chunks <= 1) {
         int64_t total = 0;  // same host-side check as the pipelined path: the lengths must add up to n_indices
-        int32_t longest = 0;
-        if (sum_lengths(lengths_host, 0, p->G, &total, &longest)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
+        if (sum_lengths(lengths_host, 0, p->G, &total)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
         if (total != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)total);
         DPI_CUDA(cudaMemcpyAsync(p->stage_len, lengths_host, static_cast<size_t>(p->G) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         if (n_indices) DPI_CUDA(cudaMemcpyAsync(p->stage_idx, indices_host, static_cast<size_t>(n_indices) * idx_elt, cudaMemcpyHostToDevice, s));
-        dpi_status_t st = dpi_plan_build(p, p->stage_len, s);
-        if (st != DPI_OK) return st;
         LookupCall c;
         c.tables = table_ptrs_dev; c.indices = p->stage_idx; c.pooling = pooling; c.out = out_base;
-        p->hint_override = longest > 0 ? longest : 1;  // the lengths are on the host: the bag-length "promise" is a fact here
-        st = do_lookup(p, c, s);
-        p->hint_override = 0;
+        dpi_status_t st = forward_device(p, p->stage_len, c, s);   // one launch when eligible, else plan + lookup
         if (st != DPI_OK) return st;
         if (!out_direct) DPI_CUDA(cudaMemcpyAsync(out_host, p->stage_out, out_bytes, cudaMemcpyDeviceToHost, s));
         DPI_CUDA(cudaStreamSynchronize(s));
@@ -743,11 +908,10 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     // Copy sizes only: how many index entries belong to each chunk (the plan itself -- offsets, segments -- is still
     // computed on the device, per chunk).
     std::vector<int64_t> entry_lo(n_sub + 1, 0);
-    int32_t longest = 0;
     for (size_t c = 0; c < n_sub; ++c) {
         const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T, g1 = static_cast<size_t>(h->sample_lo[c + 1]) * p->T;
         int64_t n = 0;
-        if (sum_lengths(lengths_host, g0, g1, &n, &longest)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
+        if (sum_lengths(lengths_host, g0, g1, &n)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
         entry_lo[c + 1] = entry_lo[c] + n;
     }
     if (entry_lo[n_sub] != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)entry_lo[n_sub]);
@@ -758,13 +922,8 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     for (size_t c = 0; c < n_sub; ++c) {
         cudaStream_t cs = h->st[c % HostPipeline::kStreams];
         dpi_plan_t* q = h->sub[c];
-        q->out_dtype = p->out_dtype;
-        q->index_type = p->index_type;
-        for (int o = 0; o < DPI_OPT_COUNT_; ++o) q->opt[o] = p->opt[o];
-        if (p->K_user && q->K != p->K_user) {
-            st = dpi_plan_set_quantum(q, p->K_user);
-            if (st != DPI_OK) return st;
-        }
+        st = sync_subplan(p, q);
+        if (st != DPI_OK) return st;
         const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T;
         const size_t n_g = static_cast<size_t>(q->G);
         const int64_t e0 = entry_lo[c], n_e = entry_lo[c + 1] - entry_lo[c];
@@ -773,13 +932,9 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
         DPI_CUDA(cudaMemcpyAsync(p->stage_len + g0, lengths_host + g0, n_g * sizeof(int32_t), cudaMemcpyHostToDevice, cs));
         if (n_e) DPI_CUDA(cudaMemcpyAsync(idx_dev, static_cast<const char*>(indices_host) + static_cast<size_t>(e0) * idx_elt,
                                           static_cast<size_t>(n_e) * idx_elt, cudaMemcpyHostToDevice, cs));
-        st = dpi_plan_build(q, p->stage_len + g0, cs);
-        if (st != DPI_OK) return st;
         LookupCall lc;
         lc.tables = table_ptrs_dev; lc.indices = idx_dev; lc.pooling = pooling; lc.out = out_dev;
-        q->hint_override = longest > 0 ? longest : 1;
-        st = do_lookup(q, lc, cs);
-        q->hint_override = 0;
+        st = forward_device(q, p->stage_len + g0, lc, cs);
         if (st != DPI_OK) return st;
         if (!out_direct)
             DPI_CUDA(cudaMemcpyAsync(static_cast<char*>(out_host) + static_cast<size_t>(h->sample_lo[c]) * row_bytes, out_dev,

@@ -14,8 +14,16 @@
 
 namespace dpi {
 
-constexpr int kMetaWords = 8;  // meta_dev layout: {S, N, C[G] (low 32), overflow, K, G, 0, 0}
-enum MetaSlot { META_S = 0, META_N = 1, META_C = 2, META_OVERFLOW = 3, META_K = 4, META_G = 5 };
+constexpr int kMetaWords = 8;  // meta_dev layout: {S, N, C[G] (low 32), overflow, K, G, min_len, max_len}
+enum MetaSlot { META_S = 0, META_N = 1, META_C = 2, META_OVERFLOW = 3, META_K = 4, META_G = 5, META_MINLEN = 6, META_MAXLEN = 7 };
+// The device picks the a3 variant from a1's max_len: bags of 2..kShortBagMax entries run the short-bag
+// body (one lane group per bag); exactly one entry per bag runs it up to kShortOnehotMaxBags bags, beyond that the
+// balanced-segment kernel's row-copy path with its index prefetch pipeline is faster (measured).
+constexpr uint32_t kShortBagMax = 8;
+constexpr uint32_t kShortOnehotMaxBags = 500000;
+__host__ __device__ inline bool short_bag_rule(uint32_t max_len, uint32_t G) {
+    return max_len >= 2 ? max_len <= kShortBagMax : G <= kShortOnehotMaxBags;
+}
 
 constexpr int kPoolWords = DPI_MAX_TABLES / 32;
 struct PoolMask {
@@ -28,7 +36,8 @@ constexpr int kScanItems = 8;                               // consecutive bags 
 constexpr int kScanTile = kScanThreads * kScanItems;        // 2048 bags per tile
 constexpr int kMaxChunks = 320;                             // CTAs of the planner (all co-resident); multiple of 32
 
-enum PlanState { kStateTicket = 0, kStateDone = 1, kStateEpoch = 2, kStateWords = 4 };
+enum PlanState { kStateTicket = 0, kStateDone = 1, kStateEpoch = 2, kStateOverflows = 3, kStateMinLen = 4, kStateMaxLen = 5,
+                 kStateWords = 8 };
 constexpr uint32_t kEpochLimit = 1u << 30;  // status words carry a 30-bit epoch
 
 struct PlanArgs {
@@ -39,7 +48,9 @@ struct PlanArgs {
     ulonglong2* status;                // [num_chunks] look-back records {len aggregate, cost aggregate}, each half
                                        // tagged {epoch:30 | state:2 | value:32}
     unsigned int* state;               // [kStateTicket] dynamic tile id, [kStateDone] finished tiles (both
-                                       // self-resetting atomicInc), [kStateEpoch] tag of this build's status words
+                                       // self-resetting atomicInc), [kStateEpoch] tag of this build's status words,
+                                       // [kStateOverflows] builds that exceeded the capacity (sticky, dpi_plan_status),
+                                       // [kStateMinLen/MaxLen] running min / max length of the build in flight
     uint32_t G;
     uint32_t K;
     uint32_t seg_cap;
@@ -50,6 +61,12 @@ struct PlanArgs {
 };
 
 cudaError_t launch_plan(const PlanArgs& a, cudaStream_t stream);
+
+// ---- a1 + a2 + a3 in one launch (forward_fused.cu) ----
+constexpr int kFusedThreads = 512;
+constexpr int kFusedMaxChunks = 512;                        // one look-back record per thread of a CTA
+constexpr int kFusedIdxStage = 4096;                        // index entries of a 512-bag tile staged in shared memory
+constexpr int kStatusRecords = kFusedMaxChunks > kMaxChunks ? kFusedMaxChunks : kMaxChunks;
 
 struct CheckArgs {
     const void* __restrict__ indices;        // int32 or int64 (idx64)
@@ -90,6 +107,15 @@ struct LookupArgs {
     PoolMask pool;
 };
 
+// plan.num_chunks = CTAs, chunk c owns bags [c*chunk_bags, min(G, (c+1)*chunk_bags)); plan.num_tiles / tiles_per_chunk unused
+struct FusedArgs {
+    PlanArgs plan;
+    LookupArgs look;
+    uint32_t chunk_bags;
+};
+cudaError_t launch_fused(const FusedArgs& a, int dtype, bool out32, int lanes, bool pdl, cudaStream_t stream);
+int fused_occupancy(int dtype, bool out32, int lanes, uint32_t T);   // resident CTAs per SM (0: no instantiation)
+
 struct LookupLaunch {
     int lanes;          // lanes per row (power of two >= nvec)
     int unroll;         // 2, 4, 8, 16
@@ -104,16 +130,19 @@ struct LookupLaunch {
 cudaError_t launch_lookup_f32(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
 cudaError_t launch_lookup_f16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
 cudaError_t launch_lookup_bf16(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream);
-// Max resident CTAs per SM of the instantiation (0 if none).
-int lookup_occupancy_f32(const LookupArgs& a, const LookupLaunch& l);
-int lookup_occupancy_f16(const LookupArgs& a, const LookupLaunch& l);
-int lookup_occupancy_bf16(const LookupArgs& a, const LookupLaunch& l);
+// Per plan, not per lookup: raises the instantiation's dynamic shared-memory limit on the current device if needed and
+// returns its resident CTAs per SM (0 if there is no such instantiation). Only a.T, a.idx_shift and a.weights matter.
+int lookup_prepare_f32(const LookupArgs& a, const LookupLaunch& l);
+int lookup_prepare_f16(const LookupArgs& a, const LookupLaunch& l);
+int lookup_prepare_bf16(const LookupArgs& a, const LookupLaunch& l);
 
 // Ablation (ablation_input_first.cu): one thread per sample.
 cudaError_t launch_input_first(const LookupArgs& a, uint32_t B, int dtype, bool out32, cudaStream_t stream);
 
 // Short-bag variant of a3 (lookup_direct.cu): one lane group per bag straight from the plan's offsets, no segments.
-cudaError_t launch_direct(const LookupArgs& a, int dtype, bool out32, int lanes, int num_sms, bool pdl, cudaStream_t stream);
+// grid_cap = SMs x resident CTAs per SM of the instantiation (direct_occupancy, queried once per plan).
+cudaError_t launch_direct(const LookupArgs& a, int dtype, bool out32, int lanes, int grid_cap, bool pdl, cudaStream_t stream);
+int direct_occupancy(int dtype, bool out32, int lanes, uint32_t T);
 
 // Algorithm 1, plan-free one-hot lookup (lookup_onehot.cu).
 cudaError_t launch_onehot(const void* const* tables, const void* ids, uint32_t idx_shift, void* out, uint32_t G, uint32_t T,

@@ -53,6 +53,10 @@ __device__ __forceinline__ void st_out32(void* p, const float (&f)[8]) {  // sm_
                  "f"(f[3]), "f"(f[4]), "f"(f[5]), "f"(f[6]), "f"(f[7]) : "memory");
 }
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// Plan data (segments, offsets, meta) is written by the planner grid this kernel may have been launched under (PDL), so
+// it is never read through the non-coherent path (ld.global.nc assumes read-only for the kernel's lifetime): L2 loads.
+__device__ __forceinline__ int2 ld_plan(const int2* p) { return __ldcg(p); }
+__device__ __forceinline__ int ld_plan(const int32_t* p) { return __ldcg(p); }
 __device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst))),
                  "l"(gmem_src) : "memory");
@@ -163,6 +167,66 @@ __device__ __forceinline__ void store_pooled(char* p, const float2 (&acc)[Tr::kA
     }
 }
 
+// ---- short-bag body (a3 variant) -------------------------------------------------------------
+// Algorithm 1's division of labour (every thread fills its own piece of the output matrix, no shared
+// control flow) carried over to CSR bags: lane group q (W lanes = one row) of n_groups owns bags q, q + n_groups, ...; for
+// each it reads offsets[g], offsets[g+1] straight from the plan (a1), gathers and pools the bag's rows in registers and
+// stores the pooled vector; U bags per lane group are processed side by side (independent chains). No segments, no
+// staging, no per-task pipeline. Shared by direct_kernel (chosen on the host from DPI_OPT_MAX_BAG_HINT / DPI_OPT_MODE = 6)
+// and by lookup_kernel, which branches here when a1's max_len says every bag is short (no promise needed).
+// Same arithmetic as the balanced-segment path: fp32 accumulation in entry order, one RNE cast at the store, mean by
+// reciprocal, bags of length <= 1 bit-exact, empty bags +0.0. Dense layout only; int64 ids through their low words.
+template <class Tr, int W, int U, bool OUT32>
+__device__ __forceinline__ void short_bag_body(const LookupArgs& a, const char* const* s_tab, uint32_t q, uint32_t sl,
+                                               uint32_t n_groups) {
+    constexpr int kAcc2 = Tr::kAcc / 2;
+    constexpr int kOutVec = (OUT32 && Tr::kAcc == 8) ? 32 : 16;
+    const bool vec_ok = sl < a.nvec;
+    const uint32_t row_bytes = a.nvec * 16;
+    const uint32_t t_step = n_groups % a.T;
+    char* const out = static_cast<char*>(a.out);
+    uint32_t t = q % a.T;
+    for (uint32_t g0 = q; g0 < a.G; g0 += n_groups * U) {
+        int lo[U], len[U];
+        uint32_t tt[U];
+        int max_len = 0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const uint32_t g = g0 + u * n_groups;
+            const bool ok = g < a.G;
+            tt[u] = t;
+            lo[u] = ok ? __ldcg(a.offsets + g) : 0;          // plan data: coherent (L2) loads, see ld_plan()
+            len[u] = ok ? __ldcg(a.offsets + g + 1) - lo[u] : 0;
+            max_len = max(max_len, len[u]);
+            t += t_step;
+            if (t >= a.T) t -= a.T;
+        }
+        float2 acc[U][kAcc2];
+#pragma unroll
+        for (int u = 0; u < U; ++u) zero_acc(acc[u]);
+        for (int j = 0; j < max_len; ++j) {
+            uint4 v[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const bool ok = vec_ok && j < len[u];
+                // int64 ids are read through their low words (little-endian, rows < 2^31): idx_shift = 1
+                const uint32_t r = ok ? static_cast<uint32_t>(__ldg(a.indices + (static_cast<size_t>(lo[u] + j) << a.idx_shift))) : 0u;
+                v[u] = ld_row16(s_tab[tt[u]] + static_cast<uint64_t>(r) * row_bytes + sl * 16, ok);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) Tr::add(acc[u], v[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const uint32_t g = g0 + u * n_groups;
+            if (vec_ok && g < a.G) {
+                if (((a.pool.w[tt[u] >> 5] >> (tt[u] & 31)) & 1u) && len[u] > 1) scale_mean(acc[u], len[u]);
+                store_pooled<Tr, OUT32>(out + (static_cast<size_t>(g) * a.nvec + sl) * kOutVec, acc[u]);
+            }
+        }
+    }
+}
+
 // Per-table record of the general (GEN) variant, staged in shared memory.
 struct TableInfo {
     const char* base;
@@ -217,6 +281,10 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
     int* const s_warp = reinterpret_cast<int*>(smem_raw + tab_bytes) + warp_in_cta * warp_words;
     int* const s_off = s_warp + 2 * stage_idx;
     float* const s_wgt = reinterpret_cast<float*>(s_off + 2 * kStageOff);
+    // PDL: everything this kernel reads (table pointers included -- a preceding kernel may have produced them) is read
+    // after the preceding grid has completed and flushed; only the launch itself and the index arithmetic above overlap
+    // its tail. No-op for a plain launch.
+    griddep_wait();
     if constexpr (GEN) {
         TableInfo* w_info = reinterpret_cast<TableInfo*>(smem_raw);
         for (uint32_t t = threadIdx.x; t < a.T; t += blockDim.x) {
@@ -232,8 +300,17 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
     }
     __syncthreads();
 
-    griddep_wait();  // PDL: the planner's writes are visible past this point (no-op otherwise)
-    const uint32_t S = static_cast<uint32_t>(a.meta[META_S]);
+    const uint32_t S = static_cast<uint32_t>(ld_plan(a.meta + META_S));
+    if constexpr (!GEN) {
+        // The device picks the a3 variant from a1's max_len ("known in advance"): a batch
+        // whose longest bag is short runs the lane-group-per-bag body over the same persistent grid -- no promise from
+        // the caller, no extra launch. S == 0 marks an overflowed plan: nothing may be read through its offsets.
+        if (a.mode == 0 && S != 0 && short_bag_rule(static_cast<uint32_t>(ld_plan(a.meta + META_MAXLEN)), a.G)) {
+            const uint32_t lane_id = blockIdx.x * blockDim.x + threadIdx.x;
+            short_bag_body<Tr, W, 2, OUT32>(a, s_tab, lane_id / W, lane_id % W, (gridDim.x * blockDim.x) / W);
+            return;
+        }
+    }
     if (warp_id >= S) return;
 
     // bag id -> table, rows, output slot
@@ -285,7 +362,9 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
         else return out + static_cast<size_t>(g) * (static_cast<size_t>(a.nvec) * kOutVec) + sl * kOutVec;
     };
     // row ids are non-negative (precondition, dpi.h): read as uint32 so that id * row_bytes is one IMAD.WIDE.U32
-    auto idx_at = [&](const int* ip, int e) -> uint32_t { return static_cast<uint32_t>(GEN ? ip[e << ish] : ip[e]); };
+    auto idx_at = [&](const int* ip, int e) -> uint32_t {
+        return static_cast<uint32_t>(GEN ? ip[static_cast<ptrdiff_t>(e) << ish] : ip[e]);  // 64-bit: e may reach 2^30 with int64 ids
+    };
     auto wgt_at = [&](const float* wp, int e) -> float { return (GEN && wp) ? wp[e] : 1.f; };
     auto accum = [&](float2 (&acc)[kAcc2], const uint4& v, float w) {
         if constexpr (GEN) Tr::fma(acc, v, make_float2(w, w));  // fma(x, 1, acc) == x + acc exactly
@@ -315,10 +394,10 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
 
     // ---- pipeline prologue ----
     uint32_t s = warp_id;
-    int2 cur_lo = __ldg(a.seg + s), cur_hi = __ldg(a.seg + s + 1);
+    int2 cur_lo = ld_plan(a.seg + s), cur_hi = ld_plan(a.seg + s + 1);
     int2 nxt_lo = cur_lo, nxt_hi = cur_hi;
     bool have_next = s + n_warps < S;
-    if (have_next) { nxt_lo = __ldg(a.seg + s + n_warps); nxt_hi = __ldg(a.seg + s + n_warps + 1); }
+    if (have_next) { nxt_lo = ld_plan(a.seg + s + n_warps); nxt_hi = ld_plan(a.seg + s + n_warps + 1); }
     stage(cur_lo, cur_hi, 0);
     int buf = 0;
 
@@ -327,7 +406,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
         const uint32_t s2 = s + 2 * n_warps;
         const bool have_next2 = s2 < S;
         int2 n2_lo = nxt_lo, n2_hi = nxt_hi;
-        if (have_next2) { n2_lo = __ldg(a.seg + s2); n2_hi = __ldg(a.seg + s2 + 1); }
+        if (have_next2) { n2_lo = ld_plan(a.seg + s2); n2_hi = ld_plan(a.seg + s2 + 1); }
         if (have_next) {
             stage(nxt_lo, nxt_hi, buf ^ 1);
             cp_async_wait<1>();
@@ -343,7 +422,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
             const uint32_t ne = static_cast<uint32_t>(e_hi - e_lo);
             const bool staged = (nb + 1 <= static_cast<uint32_t>(kStageOff)) && (ne <= static_cast<uint32_t>(kStageIdx));
             // generic pointers indexed by ABSOLUTE entry / bag id: staged smem or the global arrays
-            const int* ip = staged ? (s_warp + buf * stage_idx - (e_lo << ish)) : a.indices;
+            const int* ip = staged ? (s_warp + buf * stage_idx - (static_cast<ptrdiff_t>(e_lo) << ish)) : a.indices;
             const int* op = staged ? (s_off + buf * kStageOff - static_cast<int>(g_lo)) : a.offsets;
             const float* wp = nullptr;
             if constexpr (GEN) {
@@ -562,20 +641,14 @@ inline size_t lookup_smem_bytes(const LookupArgs& a, bool gen, int block_threads
     return tab + static_cast<size_t>(block_threads / 32) * warp_words * sizeof(int);
 }
 
+// Launch: no CUDA runtime query and no attribute call here -- prepare_one() did both when the plan was created or
+// re-configured (dpi_api.cu::prepare_launches), for the device the plan lives on.
 template <class Tr, int W, int U, bool OUT32, bool GEN>
 cudaError_t launch_one(const LookupArgs& a, const LookupLaunch& l, cudaStream_t stream) {
-    const size_t smem = lookup_smem_bytes(a, GEN, l.block_threads);
-    static size_t smem_set = 0;  // per instantiation: raise the dynamic smem limit once (or when it grows)
-    if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(lookup_kernel<Tr, W, U, OUT32, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             static_cast<int>(smem));
-        if (e != cudaSuccess) return e;
-        smem_set = smem;
-    }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(static_cast<unsigned>(l.grid));
     cfg.blockDim = dim3(static_cast<unsigned>(l.block_threads));
-    cfg.dynamicSmemBytes = smem;
+    cfg.dynamicSmemBytes = lookup_smem_bytes(a, GEN, l.block_threads);
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -586,12 +659,17 @@ cudaError_t launch_one(const LookupArgs& a, const LookupLaunch& l, cudaStream_t 
     return cudaLaunchKernelEx(&cfg, lookup_kernel<Tr, W, U, OUT32, GEN>, a);
 }
 
+// Raises the dynamic shared-memory limit of the instantiation on the CURRENT device when it needs more than 48 KB and
+// returns its resident CTAs per SM (0 on error). Called per plan, never per lookup.
 template <class Tr, int W, int U, bool OUT32, bool GEN>
-int occupancy_one(const LookupArgs& a, int block_threads) {
+int prepare_one(const LookupArgs& a, int block_threads) {
     int n = 0;
     const size_t smem = lookup_smem_bytes(a, GEN, block_threads);
-    if (smem > 48 * 1024)
-        (void)cudaFuncSetAttribute(lookup_kernel<Tr, W, U, OUT32, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (smem > 48 * 1024 &&
+        cudaFuncSetAttribute(lookup_kernel<Tr, W, U, OUT32, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
+    }
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, lookup_kernel<Tr, W, U, OUT32, GEN>, block_threads, smem) != cudaSuccess) {
         (void)cudaGetLastError();
         return 0;

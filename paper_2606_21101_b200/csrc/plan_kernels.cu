@@ -109,21 +109,21 @@ __device__ __forceinline__ void thread_sums(const uint32_t (&v)[kScanItems], uin
         t_cost += (static_cast<uint32_t>(i) < n_valid) ? max(v[i], 1u) : 0u;
     }
 }
-
-#ifdef DPI_PLAN_TRACE
-__device__ unsigned long long g_trace[kMaxChunks * 8];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define DPI_TRACE(slot, c) do { if (threadIdx.x == 0) g_trace[(c) * 8 + (slot)] = gtime(); } while (0)
-#else
-#define DPI_TRACE(slot, c) do { } while (0)
-#endif
+// a1's summary of the lengths: running min / max over the valid items of this thread
+__device__ __forceinline__ void thread_minmax(const uint32_t (&v)[kScanItems], uint32_t n_valid, uint32_t& lo, uint32_t& hi) {
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        if (static_cast<uint32_t>(i) < n_valid) {
+            lo = min(lo, v[i]);
+            hi = max(hi, v[i]);
+        }
+    }
+}
 
 __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const PlanArgs a) {
-#ifdef DPI_PLAN_TRACE
-    const unsigned long long t_start = gtime();
-#endif
     __shared__ uint32_t s_chunk, s_epoch;
     __shared__ uint32_t s_wlen[2][kScanThreads / 32], s_wcost[2][kScanThreads / 32];
+    __shared__ uint32_t s_wmin[kScanThreads / 32], s_wmax[kScanThreads / 32];
     __shared__ uint32_t s_pre_len, s_pre_cost;
 
     // Chunk ids are handed out by a ticket, so a chunk only ever waits on chunks that already run. The epoch that
@@ -136,10 +136,6 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
     __syncthreads();
     const uint32_t chunk = s_chunk;
     const uint32_t epoch = s_epoch;
-#ifdef DPI_PLAN_TRACE
-    if (threadIdx.x == 0) g_trace[chunk * 8 + 0] = t_start;
-#endif
-    DPI_TRACE(1, chunk);
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t tile_lo = chunk * a.tiles_per_chunk;
     const uint32_t tile_hi = min(a.num_tiles, tile_lo + a.tiles_per_chunk);
@@ -149,28 +145,40 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
     uint32_t n_valid = load_items(a, tile_lo, v);
     uint32_t t_len, t_cost;
     thread_sums(v, n_valid, t_len, t_cost);
+    uint32_t len_lo = 0xffffffffu, len_hi = 0u;
+    thread_minmax(v, n_valid, len_lo, len_hi);
     uint32_t c_len = t_len, c_cost = t_cost;
     for (uint32_t tile = tile_lo + 1; tile < tile_hi; ++tile) {
         uint32_t u[kScanItems], ul, uc;
         const uint32_t nv = load_items(a, tile, u);
         thread_sums(u, nv, ul, uc);
+        thread_minmax(u, nv, len_lo, len_hi);
         c_len += ul; c_cost += uc;
     }
     c_len = warp_sum(c_len);
     c_cost = warp_sum(c_cost);
-    DPI_TRACE(2, chunk);
-    if (lane == 0) { s_wlen[0][warp] = c_len; s_wcost[0][warp] = c_cost; }
+    len_lo = __reduce_min_sync(0xffffffffu, len_lo);
+    len_hi = __reduce_max_sync(0xffffffffu, len_hi);
+    if (lane == 0) { s_wlen[0][warp] = c_len; s_wcost[0][warp] = c_cost; s_wmin[warp] = len_lo; s_wmax[warp] = len_hi; }
     __syncthreads();
     if (warp == 0) {
-        uint32_t agg_len = 0, agg_cost = 0;
+        uint32_t agg_len = 0, agg_cost = 0, agg_lo = 0xffffffffu, agg_hi = 0u;
 #pragma unroll
-        for (int w = 0; w < kScanThreads / 32; ++w) { agg_len += s_wlen[0][w]; agg_cost += s_wcost[0][w]; }
-        if (lane == 0)
+        for (int w = 0; w < kScanThreads / 32; ++w) {
+            agg_len += s_wlen[0][w]; agg_cost += s_wcost[0][w];
+            agg_lo = min(agg_lo, s_wmin[w]); agg_hi = max(agg_hi, s_wmax[w]);
+        }
+        if (lane == 0) {
             st_status(a.status + chunk, pack_status(epoch, kStateAggregate, agg_len), pack_status(epoch, kStateAggregate, agg_cost));
-        DPI_TRACE(3, chunk);
+            // min / max leave the CTA as two fire-and-forget reductions into the planner state; the last CTA to finish
+            // copies them into meta and re-arms the words for the next build
+            if (agg_lo <= agg_hi) {
+                atomicMin(a.state + kStateMinLen, agg_lo);
+                atomicMax(a.state + kStateMaxLen, agg_hi);
+            }
+        }
         uint32_t pl, pc;
         lookback_all(a.status, chunk, epoch, pl, pc);
-        DPI_TRACE(4, chunk);
         if (lane == 0) { s_pre_len = pl; s_pre_cost = pc; }
     }
     __syncthreads();
@@ -253,7 +261,9 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
                 a.meta[META_S] = (S < a.seg_cap) ? S : 0;             // an overflowed plan must not drive a lookup
                 a.meta[META_N] = n_total;
                 a.meta[META_C] = c;
-                a.meta[META_OVERFLOW] = (n_total > a.max_indices || S >= a.seg_cap) ? 1 : 0;
+                const bool overflow = n_total > a.max_indices || S >= a.seg_cap;
+                a.meta[META_OVERFLOW] = overflow ? 1 : 0;
+                if (overflow) atomicAdd(a.state + kStateOverflows, 1u);   // sticky until dpi_plan_status reads it
                 a.meta[META_K] = a.K;
                 a.meta[META_G] = a.G;
             }
@@ -265,11 +275,17 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
             thread_sums(v, n_valid, t_len, t_cost);
         }
     }
-
-    DPI_TRACE(5, chunk);
     // ---- close the epoch: no thread of this CTA reads a status record past the barrier after the look-back; the
     // last CTA to get here advances the tag (a later build starts only after this grid has completed) ----
+    if (threadIdx.x == 0) __threadfence();  // this CTA's min / max reductions (issued by this thread) before the count
     if (threadIdx.x == 0 && atomicInc(a.state + kStateDone, a.num_chunks - 1) == a.num_chunks - 1) {
+        __threadfence();
+        const uint32_t lo = *reinterpret_cast<volatile unsigned int*>(a.state + kStateMinLen);
+        const uint32_t hi = *reinterpret_cast<volatile unsigned int*>(a.state + kStateMaxLen);
+        a.meta[META_MINLEN] = lo <= hi ? lo : 0u;   // G >= 1 always, so lo <= hi; kept total for safety
+        a.meta[META_MAXLEN] = hi;
+        a.state[kStateMinLen] = 0xffffffffu;
+        a.state[kStateMaxLen] = 0u;
         uint32_t next = epoch + 1;
         if (next >= kEpochLimit) {  // 30-bit tag about to wrap: clear the records once and restart at 1
             for (uint32_t i = 0; i < a.num_chunks; ++i) a.status[i] = make_ulonglong2(0ull, 0ull);
@@ -277,7 +293,6 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
         }
         a.state[kStateEpoch] = next;
     }
-    DPI_TRACE(6, chunk);
 }
 
 __global__ void __launch_bounds__(256) check_indices_kernel(const CheckArgs a) {

@@ -125,3 +125,10 @@ extern "C" int dpi_synth_row_read_probe(const void* base, uint64_t span_rows, ui
     }
     return (int)cudaGetLastError();
 }
+
+// Test helper: copy n_words 32-bit words between two raw device addresses (how the tests read the borrowed pointers of
+// dpi_plan_device_views into a tensor); synchronous.
+extern "C" int dpi_synth_copy_words(void* dst_dev, const void* src_dev, uint64_t n_words) {
+    if (!dst_dev || !src_dev) return (int)cudaErrorInvalidValue;
+    return (int)cudaMemcpy(dst_dev, src_dev, n_words * 4, cudaMemcpyDeviceToDevice);
+}

@@ -109,16 +109,17 @@ def max_bag_length(cfg: W.Config) -> int:
     return int(cfg.lengths[1]) if kind == "const" else int(cfg.lengths[2])
 
 
-def lookup_variant(cfg: W.Config, mode: int = 0, bag_hint: bool = True) -> str:
-    """Which a3 kernel dpi_lookup runs for this config (mirrors the rule in dpi_api.cu::do_lookup; reporting only)."""
-    L = max_bag_length(cfg) if bag_hint else 0
-    short = (2 <= L <= 8) or (L == 1 and cfg.G <= 500000)
+def lookup_variant(cfg: W.Config, mode: int = 0) -> str:
+    """Which a3 body dpi_lookup ends up in for this config (mirrors short_bag_rule in dpi_internal.cuh, which the device
+    applies to a1's max_len; reporting only)."""
+    L = max_bag_length(cfg)
+    short = (2 <= L <= 8) or (L <= 1 and cfg.G <= 500000)
     return "short-bag (lane group per bag)" if (mode == 6 or (mode == 0 and short)) else "balanced segments"
 
 
-def make_plan(cfg: W.Config, rows: np.ndarray, max_indices: int, bag_hint: bool = True) -> binding.Plan:
-    """bag_hint: pass the recipe's longest bag as DPI_OPT_MAX_BAG_HINT (the library then runs its short-bag variant when
-    that is <= 8: c1-c3; c4 / c5 keep the balanced-segment kernel)."""
+def make_plan(cfg: W.Config, rows: np.ndarray, max_indices: int, bag_hint: bool = False) -> binding.Plan:
+    """bag_hint: pass the recipe's longest bag as the OPTIONAL promise DPI_OPT_MAX_BAG_HINT (the short-bag variant then runs as
+    its own launch, chosen on the host). Default: no hint -- the device picks from a1's max_len."""
     plan = binding.Plan(rows, cfg.D, W.DTYPE_CODE[cfg.dtype], cfg.B, max_indices)
     if cfg.out != cfg.dtype:
         plan.set_out_dtype(W.DTYPE_CODE[cfg.out])

@@ -50,6 +50,8 @@ def _plan_parity(lengths: np.ndarray, T: int, B: int, K: int, max_indices=None):
         assert np.array_equal(off, o_off)
         assert np.array_equal(seg, o_seg)
         assert np.array_equal(seg_off, o_seg_off)
+        assert plan.stats() == oracle.plan_stats(lengths)      # a1's min / max bag length
+        assert plan.status() == 0                              # nothing overflowed
     plan.destroy()
 
 
@@ -93,6 +95,14 @@ def test_plan_overflow_is_reported_not_out_of_bounds():
     with pytest.raises(binding.DpiError) as e:
         plan.export()
     assert e.value.status == 1 and "max_indices" in e.value.detail
+    # ... and without exporting anything: the sticky device counter (dpi_plan_status) counts overflowed builds once
+    plan.build(torch.from_numpy(ln).cuda())
+    assert plan.status() == 2
+    assert plan.status() == 0
+    ok = np.full(100, 5, np.int32)
+    plan.build(torch.from_numpy(ok).cuda())
+    assert plan.status() == 0 and plan.export()[3] == 500
+    plan.destroy()
 
 
 # --------------------------------------------------------------------------------------------------
@@ -379,6 +389,36 @@ def test_c5_full_size_sampled():
     if free < 90e9:
         pytest.fail(f"config 5 needs ~82 GB of tables; only {free / 1e9:.0f} GB free on this device")
     _sampled_full_size(W.C5, 4096)
+
+
+def _every_sample_full_size(cfg, samples_per_pass):
+    """Every output element of one full-size batch against the oracle. The tables do not fit on the host (c5) or are slow to
+    mirror (c4), so the oracle works through the batch in passes of `samples_per_pass` samples, each on tables compacted to
+    the rows that pass references (values recomputed from the counter-based generator, never read back from the device)."""
+    dt = harness.make_device_tables(cfg)
+    batch = W.make_batch(cfg, dt.rows, cfg.seed)
+    pooling = cfg.pooling_modes()
+    got = _run_gpu(cfg, dt, batch, pooling)
+    worst = 0.0
+    for lo in range(0, cfg.B, samples_per_pass):
+        samples = np.arange(lo, min(cfg.B, lo + samples_per_pass))
+        sub = W.compact_subproblem(cfg, batch, samples)
+        ref = oracle.lookup(sub.tables, W.DTYPE_CODE[cfg.dtype], len(samples), sub.indices, host_offsets(sub.lengths), pooling)
+        worst = max(worst, assert_outputs_match(got[samples], ref, sub.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out))
+    del dt
+    torch.cuda.empty_cache()
+    return worst
+
+
+def test_c4_full_size_every_sample():
+    _every_sample_full_size(W.C4, 1024)
+
+
+def test_c5_full_size_every_sample():
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.fail(f"config 5 needs ~82 GB of tables; only {free / 1e9:.0f} GB free on this device")
+    _every_sample_full_size(W.C5, 8192)
 
 
 # --------------------------------------------------------------------------------------------------
