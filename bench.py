@@ -59,6 +59,7 @@ def parse_args():
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--fused", type=int, default=-1, help="dpi_forward: -1 library default (auto), 0 auto, 1 fused whenever the layout allows, 2 always planner + lookup")
     ap.add_argument("--rows-scale", type=float, default=1.0, help="debug: scale table heights (invalidates the run)")
     return ap.parse_args()
 
@@ -364,6 +365,44 @@ def run_reference(args):
 # ----------------------------------------------------------------------------------------------------
 # CUDA path
 # ----------------------------------------------------------------------------------------------------
+def link_floor(h2d_bytes: int, d2h_bytes: int, device: str, reps: int = 5) -> dict:
+    """Host-link ceiling for one e2e step, measured in this run: pinned-memory cudaMemcpyAsync of exactly the step's byte
+    counts -- H2D alone, D2H alone, and both at once on two streams (one copy per direction). The floor of an e2e step is
+    the concurrent figure: no schedule can beat both directions streaming flat out."""
+    import torch
+    hi = torch.empty(max(h2d_bytes, 1), dtype=torch.uint8).pin_memory()
+    ho = torch.empty(max(d2h_bytes, 1), dtype=torch.uint8).pin_memory()
+    di = torch.empty(max(h2d_bytes, 1), dtype=torch.uint8, device=device)
+    do = torch.empty(max(d2h_bytes, 1), dtype=torch.uint8, device=device)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+
+    def run(h2d, d2h):
+        best = None
+        for _ in range(reps + 1):
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            j = torch.cuda.Event()
+            a.record(s1)
+            s2.wait_event(a)
+            if h2d:
+                with torch.cuda.stream(s1):
+                    di.copy_(hi, non_blocking=True)
+            if d2h:
+                with torch.cuda.stream(s2):
+                    ho.copy_(do, non_blocking=True)
+            j.record(s2)
+            s1.wait_event(j)
+            b.record(s1)
+            torch.cuda.synchronize()
+            t = a.elapsed_time(b)
+            best = t if best is None else min(best, t)
+        return best
+
+    h, d, both = run(True, False), run(False, True), run(True, True)
+    return {"h2d_ms": h, "d2h_ms": d, "both_ms": both, "h2d_gbs": h2d_bytes / h / 1e6, "d2h_gbs": d2h_bytes / d / 1e6,
+            "both_gbs": (h2d_bytes + d2h_bytes) / both / 1e6}
+
+
 def run_ours(args):
     import torch
     from paper_2606_21101_b200 import binding, build, harness, sharding, workloads as W
@@ -383,6 +422,7 @@ def run_ours(args):
     if dist is not None:
         dist.barrier()
     binding.load_library()
+    device = f"cuda:{local}"
 
     cfg, rows = workload_config(args)
     small = cfg.name in ("c1", "c2", "c3")
@@ -393,21 +433,26 @@ def run_ours(args):
 
     # every rank: all tables + its own shard of each global batch of world*B samples (batch-sharded replicas,
     # no collective on the data path)
-    dt = harness.make_device_tables(cfg, rows, device=f"cuda:{local}")
-    batches = [harness.upload_batch(sharding.make_batch_shard(cfg, rows, cfg.seed + r, rank, world), device=f"cuda:{local}")
+    dt = harness.make_device_tables(cfg, rows, device=device)
+    batches = [harness.upload_batch(sharding.make_batch_shard(cfg, rows, cfg.seed + r, rank, world), device=device)
                for r in range(R)]
     pooling = cfg.pooling_modes()
-    plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg))
+    plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg))   # no bag-length promise: the device picks the a3 variant
     apply_options(plan, args, binding)
-    out = harness.new_output(cfg, device=f"cuda:{local}")
+    if args.fused >= 0:
+        plan.set_option(binding.OPT_FUSED, args.fused)
+    out = harness.new_output(cfg, device=device)
     stream = torch.cuda.Stream()  # a non-default stream: every launch and every event of the timed region is on it
 
-    lookup = plan.lookup if args.kernel == "output_first" else plan.lookup_input_first
+    ablation = args.kernel == "input_first"
 
     def step(i, s):
         b = batches[i % R]
-        plan.build(b.lengths, s)
-        lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=s)
+        if ablation:
+            plan.build(b.lengths, s)
+            plan.lookup_input_first(dt.ptrs, b.indices, out, pooling=pooling, stream=s)
+        else:   # the public one-call path: ONE fused launch (a1+a2+a3) when eligible, else planner + lookup
+            plan.forward(b.lengths, dt.ptrs, b.indices, out, pooling=pooling, stream=s)
 
     def barrier():
         if dist is not None:
@@ -415,12 +460,16 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_ms(ms):
-        return sharding.max_over_ranks(ms, dist, device=f"cuda:{local}")
+        return sharding.max_over_ranks(ms, dist, device=device)
 
     with torch.cuda.stream(stream):
-        for i in range(warmup):
+        n0 = binding.launch_count()
+        step(0, stream)
+        launches_per_step = binding.launch_count() - n0
+        for i in range(1, warmup):
             step(i, stream)
     barrier()
+    fused = (not ablation) and launches_per_step == 1
 
     graph = None
     if use_graph:  # capture the K steps once; the timed region replays them with no host work in between
@@ -450,13 +499,14 @@ def run_ours(args):
         e1.record(stream)
     barrier()
     t1 = time.time()
-    launches = 2 * steps if graph is not None else binding.launch_count() - launches0
+    launches = launches_per_step * steps if graph is not None else binding.launch_count() - launches0
     total_ms = max_ms(e0.elapsed_time(e1))
     clocks = sampler.stop(t0, t1) if rank == 0 else None
 
-    # ---- the dominant kernel alone: per-launch CUDA events around dpi_lookup, same stream, same batches -------
-    # (plain launches here: with programmatic dependent launch the kernel's prologue may start under the planner's tail, and
-    #  an event pair would then time more than the kernel itself; the timed steps above keep the library default)
+    # ---- the dominant kernel alone: per-launch CUDA events, same stream, same batches ---------------------
+    # (plain launches here: with programmatic dependent launch the kernel's prologue may start under the previous kernel's
+    #  tail, and an event pair would then time more than the kernel itself; the timed steps above keep the library default).
+    # Fused path: the ONE kernel of the step (a1+a2+a3). Otherwise: the lookup kernel (a3) behind an untimed planner launch.
     n_k = min(steps, 200)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_k)]
     pdl_was = plan.get_option(binding.OPT_PDL)
@@ -464,14 +514,22 @@ def run_ours(args):
     with torch.cuda.stream(stream):
         for i in range(n_k):
             b = batches[i % R]
-            plan.build(b.lengths, stream)
-            ev[i][0].record(stream)
-            lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
-            ev[i][1].record(stream)
+            if fused:
+                ev[i][0].record(stream)
+                plan.forward(b.lengths, dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
+                ev[i][1].record(stream)
+            else:
+                plan.build(b.lengths, stream)
+                ev[i][0].record(stream)
+                if ablation:
+                    plan.lookup_input_first(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
+                else:
+                    plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
+                ev[i][1].record(stream)
     barrier()
     plan.set_option(binding.OPT_PDL, pdl_was)
-    lookup_ms = [a.elapsed_time(b) for a, b in ev]
-    # and the stream-launched step (plan + lookup, no graph), for the graph-vs-stream comparison
+    kernel_ms = [a.elapsed_time(b) for a, b in ev]
+    # and the stream-launched step (no graph), for the graph-vs-stream comparison
     s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(stream):
         s0.record(stream)
@@ -482,12 +540,13 @@ def run_ours(args):
     stream_step_ms = s0.elapsed_time(s1) / n_k
 
     # plan facts for the byte counts (after timing)
-    Ns, Ss = [], []
+    Ns, Ss, max_lens = [], [], []
     for b in batches:
         plan.build(b.lengths, stream)
         _, _, S, N = plan.export(stream)
         Ns.append(N)
         Ss.append(S)
+        max_lens.append(plan.stats(stream)[1])
     n_mean, s_mean = float(np.mean(Ns)), float(np.mean(Ss))
     bytes_step = W.algorithmic_bytes(cfg, cfg.G, n_mean, s_mean)
 
@@ -516,6 +575,11 @@ def run_ours(args):
                "api": "dpi_forward_host (pinned host lengths/indices in, [B,T*D] block out, tables resident)",
                "d2h": ("staged device block + cudaMemcpyAsync" if args.host_direct_out == 1 else
                        "fused into the lookup's store: the kernel writes the block straight into the pinned host buffer over PCIe")}
+        if rank == 0:   # the host link's own ceiling for exactly these byte counts, measured in this run
+            lf = link_floor(h2d, d2h, device)
+            e2e["link"] = lf
+            e2e["link_floor_ms"] = lf["both_ms"]
+            e2e["frac_of_link"] = lf["both_ms"] / (e2e_ms / n_e2e)
 
     if rank != 0:
         if dist is not None:
@@ -523,16 +587,28 @@ def run_ours(args):
         return
 
     peak, peak_src = measured_peak()
-    lk_ms = statistics.mean(lookup_ms)
-    achieved = bytes_step["lookup"] / (lk_ms * 1e-3) / 1e9
-    short_variant = args.kernel == "output_first" and harness.lookup_variant(cfg, args.mode).startswith("short-bag")
-    roofline = {"bound": "hbm", "kernel": ("direct_kernel (a3 fused gather-and-pool, short-bag variant)" if short_variant else
-                                           "lookup_kernel (a3 fused gather-and-pool)") if args.kernel == "output_first" else "input_first_kernel (ablation)", "achieved": achieved,
+    k_ms = statistics.mean(kernel_ms)
+    if ablation:
+        kname, ncu_name, variant = "input_first_kernel (ablation)", "input_first_kernel", "input-first ablation"
+    elif fused:
+        kname, ncu_name = "fused_forward_kernel (a1 + a2 + a3 in one launch)", "fused_forward_kernel"
+        variant = "fused single launch (dpi_forward): chained scan + lane-group-per-bag pooling"
+    else:
+        short = harness.short_bag_rule(int(max(max_lens)), cfg.G) and args.mode == 0
+        kname = "lookup_kernel (a3 fused gather-and-pool" + (", short-bag body picked on the device from a1's max_len)" if short else ")")
+        ncu_name = "lookup_kernel"
+        variant = "planner + " + ("short-bag body of lookup_kernel (device-picked)" if short else "balanced segments")
+    k_bytes = bytes_step["total"] if fused else bytes_step["lookup"]
+    achieved = k_bytes / (k_ms * 1e-3) / 1e9
+    traffic, traffic_note = ncu_traffic(cfg.name, ncu_name)
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "frac_of_nominal_8000": achieved / 8000.0, "traffic": ncu_traffic(cfg.name),
-                "algorithmic_bytes_per_launch": bytes_step["lookup"], "kernel_ms_avg": lk_ms,
-                "kernel_ms_min": min(lookup_ms), "kernel_ms_median": statistics.median(lookup_ms),
-                "kernel_launches_timed": n_k, "kernel_share_of_step": lk_ms / stream_step_ms}
+                "frac_of_nominal_8000": achieved / 8000.0, "traffic": traffic,
+                "algorithmic_bytes_per_launch": k_bytes, "kernel_ms_avg": k_ms,
+                "kernel_ms_min": min(kernel_ms), "kernel_ms_median": statistics.median(kernel_ms),
+                "kernel_launches_timed": n_k, "kernel_share_of_step": k_ms / stream_step_ms}
+    if traffic_note:
+        roofline["traffic_note"] = traffic_note
     cpu = None
     if not args.no_cpu_baseline:
         r = time_oracle(cfg, rows, args.cpu_seconds)
@@ -544,16 +620,17 @@ def run_ours(args):
         "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_KEY[cfg.dtype], "data": "synthetic",
         "config": describe(cfg, rows, {"parallelism": f"batch-sharded replicas x{world}, no collective",
                                        "launch": "CUDA graph replay of the K steps" if graph is not None else "stream launches",
-                                       "quantum_K": plan.info()["K"],
-                                       "max_bag_hint": harness.max_bag_length(cfg),
-                                       "lookup_variant": ("input-first ablation" if args.kernel == "input_first" else
-                                                          harness.lookup_variant(cfg, args.mode)), "rows_gathered_per_step": n_mean,
+                                       "api": "dpi_forward" if not ablation else "dpi_plan_build + dpi_lookup_input_first",
+                                       "launches_per_step": launches_per_step,
+                                       "quantum_K": plan.info()["K"], "max_bag_hint": 0,
+                                       "max_len_measured_by_a1": int(max(max_lens)),
+                                       "lookup_variant": variant, "rows_gathered_per_step": n_mean,
                                        "segments_per_step": s_mean}, R),
         "row_gathers_per_s": n_mean * steps * world / (total_ms * 1e-3),
         "step_algorithmic_gbs": bytes_step["total"] * world / (total_ms / steps * 1e-3) / 1e9,
         "stream_launched_ms_per_step": stream_step_ms,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "device": torch.cuda.get_device_name(local),
+        "device": torch.cuda.get_device_name(local), "csrc_hash": csrc_hash(),
     }
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -109,11 +109,14 @@ def max_bag_length(cfg: W.Config) -> int:
     return int(cfg.lengths[1]) if kind == "const" else int(cfg.lengths[2])
 
 
+def short_bag_rule(max_len: int, G: int) -> bool:
+    """Reporting mirror of short_bag_rule in csrc/dpi_internal.cuh (the device applies it to a1's max_len)."""
+    return max_len <= 8 if max_len >= 2 else G <= 500000
+
+
 def lookup_variant(cfg: W.Config, mode: int = 0) -> str:
-    """Which a3 body dpi_lookup ends up in for this config (mirrors short_bag_rule in dpi_internal.cuh, which the device
-    applies to a1's max_len; reporting only)."""
-    L = max_bag_length(cfg)
-    short = (2 <= L <= 8) or (L <= 1 and cfg.G <= 500000)
+    """Which a3 body dpi_lookup ends up in for this config (reporting only)."""
+    short = short_bag_rule(max_bag_length(cfg), cfg.G)
     return "short-bag (lane group per bag)" if (mode == 6 or (mode == 0 and short)) else "balanced segments"
 
 
