@@ -60,6 +60,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--fused", type=int, default=-1, help="dpi_forward: -1 library default (auto), 0 auto, 1 fused whenever the layout allows, 2 always planner + lookup")
+    ap.add_argument("--vec-bytes", type=int, default=0, help="DPI_OPT_VEC_BYTES: 0 auto, 16 / 32 bytes of a row per lane and load")
     ap.add_argument("--rows-scale", type=float, default=1.0, help="debug: scale table heights (invalidates the run)")
     return ap.parse_args()
 
@@ -215,6 +216,7 @@ def apply_options(plan, args, binding):
         plan.set_option(binding.OPT_PDL, args.pdl)
     plan.set_option(binding.OPT_HOST_CHUNKS, args.host_chunks)
     plan.set_option(binding.OPT_HOST_DIRECT_OUT, args.host_direct_out)
+    plan.set_option(binding.OPT_VEC_BYTES, args.vec_bytes)
 
 
 def workload_config(args):

@@ -78,7 +78,8 @@ typedef enum { DPI_IDX_I32 = 0, DPI_IDX_I64 = 1 } dpi_index_type_t;
 
 /* Tuning knobs for dpi_plan_set_option (all kernel-internal; none changes a result). */
 typedef enum {
-    DPI_OPT_UNROLL = 0,         /* independent 128-bit row loads in flight per lane: 2, 4, 8 or 16; 0 = auto */
+    DPI_OPT_UNROLL = 0,         /* independent 128-bit row loads in flight per lane: 2, 4, 8 or 16; 0 = auto (a 256-bit load,
+                                   DPI_OPT_VEC_BYTES, counts as two) */
     DPI_OPT_BLOCK_THREADS = 1,  /* lookup CTA size: a multiple of 32 up to 256; 0 = auto */
     DPI_OPT_BLOCKS_PER_SM = 2,  /* persistent grid = SMs * this; 0 = auto (occupancy) */
     DPI_OPT_MODE = 3,           /* 0 auto per task, 1 sub-warp per bag, 2 warp per bag (single-buffered),
@@ -111,6 +112,12 @@ typedef enum {
                                    G <= DPI_OPT_FUSED_MAX_BAGS and the capacity says bags are short on average,
                                    max_indices <= 8*G), 1 = fused whenever the layout allows, 2 = always plan + lookup */
     DPI_OPT_FUSED_MAX_BAGS = 10,/* ceiling of the auto rule above in bags; 0 = library default (2^20) */
+    DPI_OPT_VEC_BYTES = 11,     /* bytes of a row one lane loads at a time in the dense balanced-segment kernel: 0 = auto (32 --
+                                   the sm_100 256-bit load, half the lanes and load instructions per row -- whenever all dims are
+                                   equal and the row size is a multiple of 32 B; else 16), 16 = always 128-bit loads, 32 = require
+                                   256-bit (DPI_ERR_UNSUPPORTED if the rows do not allow it). With 32-byte vectors every table
+                                   base must be 32-byte aligned (any cudaMalloc / framework allocation is); an output block that
+                                   is only 16-byte aligned silently takes the 128-bit kernel. */
     DPI_OPT_COUNT_
 } dpi_option_t;
 
@@ -214,7 +221,8 @@ dpi_status_t dpi_plan_stats(const dpi_plan_t* plan, int32_t* min_len, int32_t* m
 /*
  * dpi_lookup -- step a3, asynchronous on `stream`, ONE kernel launch for all tables and samples.
  *   table_ptrs_dev device array of T device pointers; table t is row-major [table_rows[t], D] of the
- *                  plan's dtype, 16-byte aligned ("Embs", per-table local ids PAPER.md:162)
+ *                  plan's dtype, 16-byte aligned -- 32-byte aligned when the row size is a multiple of 32 B, unless
+ *                  DPI_OPT_VEC_BYTES = 16 ("Embs", per-table local ids PAPER.md:162)
  *   indices_dev    device int32[N], per-table local row ids, bag-contiguous in bag order g
  *   offsets_dev    NULL (use the plan's own offsets) or a device int32[G+1] equal to them
  *   plan           a built plan (same stream, or ordered after dpi_plan_build by an event)
@@ -293,6 +301,25 @@ typedef struct dpi_lookup_args_s {
     int32_t rows_per_peer;
 } dpi_lookup_args_t;
 dpi_status_t dpi_lookup_ex(const dpi_lookup_args_t* args, const dpi_plan_t* plan, void* stream);
+
+/*
+ * Peer-visible output blocks for the fused lookup + all-to-all above (NEXT-3; one process per GPU). CUDA IPC plumbing only.
+ *   dpi_peer_alloc  allocates `bytes` of device memory on the current device as ONE dedicated allocation (an IPC handle
+ *                   names a whole allocation) and writes its DPI_PEER_HANDLE_BYTES-byte handle; the caller ships the handle
+ *                   to the other ranks over its control plane (e.g. torch.distributed all_gather, any backend).
+ *   dpi_peer_open   maps another PROCESS's block into this process (peer access is enabled on demand when the block lives on
+ *                   another GPU); the returned pointer goes into out_peers_dev. Opening a handle in the process that created
+ *                   it is an error of the CUDA runtime (DPI_ERR_CUDA): a rank uses its own dpi_peer_alloc pointer.
+ *   dpi_peer_close  unmaps a pointer returned by dpi_peer_open;  dpi_peer_free releases a dpi_peer_alloc block (after every
+ *                   peer has closed it). NULL is a no-op for both.
+ * Ordering is the caller's: a rank may read its block only after ALL ranks' lookups have completed (stream synchronise +
+ * a barrier of the control plane, or an interprocess event).
+ */
+#define DPI_PEER_HANDLE_BYTES 64
+dpi_status_t dpi_peer_alloc(int64_t bytes, void** dev_ptr, uint8_t* handle);
+dpi_status_t dpi_peer_open(const uint8_t* handle, void** dev_ptr);
+dpi_status_t dpi_peer_close(void* dev_ptr);
+dpi_status_t dpi_peer_free(void* dev_ptr);
 
 /*
  * dpi_lookup_onehot -- Algorithm 1 itself: the one-hot case, where every (sample, table) bag holds

@@ -19,7 +19,7 @@ STATUS_NAMES = {0: "DPI_OK", 1: "DPI_ERR_INVALID_ARG", 2: "DPI_ERR_UNSUPPORTED",
                 4: "DPI_ERR_CUDA", 5: "DPI_ERR_INDEX_RANGE"}
 DPI_F32, DPI_F16, DPI_BF16 = 0, 1, 2
 DPI_POOL_SUM, DPI_POOL_MEAN = 0, 1
-OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL, OPT_HOST_CHUNKS, OPT_HOST_DIRECT_OUT, OPT_MAX_BAG_HINT, OPT_FUSED, OPT_FUSED_MAX_BAGS = range(11)
+OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL, OPT_HOST_CHUNKS, OPT_HOST_DIRECT_OUT, OPT_MAX_BAG_HINT, OPT_FUSED, OPT_FUSED_MAX_BAGS, OPT_VEC_BYTES = range(12)
 BAGS_SAMPLE_MAJOR, BAGS_TABLE_MAJOR = 0, 1
 IDX_I32, IDX_I64 = 0, 1
 LOOKUP_FORCE_GENERAL = 1
@@ -29,7 +29,7 @@ EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "
            "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
            "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export", "dpi_plan_stats",
            "dpi_lookup", "dpi_forward", "dpi_plan_status", "dpi_lookup_onehot", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
-           "dpi_version", "dpi_status_string", "dpi_last_error"]
+           "dpi_version", "dpi_status_string", "dpi_last_error", "dpi_peer_alloc", "dpi_peer_open", "dpi_peer_close", "dpi_peer_free"]
 
 
 class LookupArgs(ctypes.Structure):
@@ -89,6 +89,10 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
         "dpi_forward_host": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_check_indices": (st, [vp, vp, vp, vp]),
         "dpi_plan_destroy": (st, [vp]),
+        "dpi_peer_alloc": (st, [i64, vp, vp]),
+        "dpi_peer_open": (st, [vp, vp]),
+        "dpi_peer_close": (st, [vp]),
+        "dpi_peer_free": (st, [vp]),
         "dpi_launch_count": (i64, []),
         "dpi_version": (i32, []),
         "dpi_status_string": (ctypes.c_char_p, [ctypes.c_int]),
@@ -125,6 +129,33 @@ def _stream_handle(stream) -> int:
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream
+
+
+PEER_HANDLE_BYTES = 64
+
+
+def peer_alloc(nbytes: int):
+    """dpi_peer_alloc: (device pointer, 64-byte IPC handle) of a dedicated allocation on the current device."""
+    ptr = ctypes.c_void_p()
+    handle = (ctypes.c_uint8 * PEER_HANDLE_BYTES)()
+    _check(load_library().dpi_peer_alloc(int(nbytes), ctypes.byref(ptr), handle))
+    return int(ptr.value), bytes(handle)
+
+
+def peer_open(handle: bytes) -> int:
+    """dpi_peer_open: map another process's dpi_peer_alloc block; returns the device pointer in this process."""
+    ptr = ctypes.c_void_p()
+    buf = (ctypes.c_uint8 * PEER_HANDLE_BYTES).from_buffer_copy(handle)
+    _check(load_library().dpi_peer_open(buf, ctypes.byref(ptr)))
+    return int(ptr.value)
+
+
+def peer_close(ptr: int):
+    _check(load_library().dpi_peer_close(ctypes.c_void_p(ptr)))
+
+
+def peer_free(ptr: int):
+    _check(load_library().dpi_peer_free(ctypes.c_void_p(ptr)))
 
 
 def launch_count() -> int:

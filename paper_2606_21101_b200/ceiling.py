@@ -4,7 +4,12 @@ no indices, no pooling and no output -- the number the fused lookup's row stream
     python -m paper_2606_21101_b200.ceiling [--out gpurun_out/ceiling.md]
 
 For row sizes 64 / 128 / 256 / 512 B and spans 1 / 8 / 80 GB: random rows (counter hash) and consecutive rows, reading
-4.3 GB per launch (c5's gathered bytes). Helper kernel in libdpi_synth.so; not part of the method."""
+4.3 GB per launch (c5's gathered bytes). Helper kernel in libdpi_synth.so; not part of the method.
+
+    python -m paper_2606_21101_b200.ceiling --probe pcie [--out gpurun_out/pcie.md]
+
+The host link's ceiling for the end-to-end number (dpi_forward_host): one pinned-memory cudaMemcpyAsync per direction,
+H2D alone, D2H alone and both at once on two streams, 16 ... 256 MB (torch only issues the copies)."""
 from __future__ import annotations
 
 import argparse
@@ -16,12 +21,61 @@ from . import binding, harness
 from .nongemm_bench import peak_gbs
 
 
+def pcie_probe() -> str:
+    sizes = [16, 32, 64, 128, 256]
+    big = max(sizes) << 20
+    hi, ho = torch.empty(big, dtype=torch.uint8).pin_memory(), torch.empty(big, dtype=torch.uint8).pin_memory()
+    di, do = torch.empty(big, dtype=torch.uint8, device="cuda"), torch.empty(big, dtype=torch.uint8, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+
+    def run(n, h2d, d2h):
+        ts = []
+        for it in range(7):
+            torch.cuda.synchronize()
+            a, b, j = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event()
+            a.record(s1)
+            s2.wait_event(a)
+            if h2d:
+                with torch.cuda.stream(s1):
+                    di[:n].copy_(hi[:n], non_blocking=True)
+            if d2h:
+                with torch.cuda.stream(s2):
+                    ho[:n].copy_(do[:n], non_blocking=True)
+            j.record(s2)
+            s1.wait_event(j)
+            b.record(s1)
+            torch.cuda.synchronize()
+            if it >= 2:
+                ts.append(a.elapsed_time(b))
+        return min(ts)
+
+    lines = ["# Host-link ceiling probe (python -m paper_2606_21101_b200.ceiling --probe pcie)", "",
+             f"Device {torch.cuda.get_device_name(0)}; pinned host buffers, ONE cudaMemcpyAsync per direction and measurement, CUDA "
+             "events, best of 5 after 2 warm-ups. 'both' = H2D and D2H of the same size at once on two streams; its GB/s counts "
+             "both directions.", "",
+             "| MB per direction | H2D ms | H2D GB/s | D2H ms | D2H GB/s | both ms | both GB/s (sum) |", "|---|---|---|---|---|---|---|"]
+    for mb in sizes:
+        n = mb << 20
+        h, d, both = run(n, True, False), run(n, False, True), run(n, True, True)
+        lines.append(f"| {mb} | {h:.3f} | {n / h / 1e6:.1f} | {d:.3f} | {n / d / 1e6:.1f} | {both:.3f} | {2 * n / both / 1e6:.1f} |")
+    return "\n".join(lines)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default="")
+    ap.add_argument("--probe", default="rows", choices=["rows", "pcie"])
     args = ap.parse_args()
     harness.require_cuda()
     torch.cuda.set_device(0)
+    if args.probe == "pcie":
+        text = pcie_probe()
+        print(text)
+        if args.out:
+            os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
+            with open(args.out, "w") as f:
+                f.write(text + "\n")
+        return
     peak, src = peak_gbs()
     buf = torch.empty(80 * (1 << 30), dtype=torch.uint8, device="cuda")
     buf.zero_()

@@ -69,14 +69,17 @@ struct dpi_plan_s {
     uint32_t G = 0;
     int64_t max_indices = 0;
     uint32_t nvec = 0;   // 16-byte vectors per row
-    int lanes = 0;       // lanes per row
+    int lanes = 0;       // lanes per row at 16 bytes per lane
+    bool wide = false;   // 256-bit row vectors in the dense balanced-segment kernel (every row a multiple of 32 B)
+    uint32_t nvec_w = 0; // 32-byte vectors per row
+    int lanes_w = 0;     // lanes per row at 32 bytes per lane
     std::vector<int64_t> table_rows;
     // plan parameters
     int32_t K = 0;           // effective quantum
     int32_t K_user = 0;      // 0 = default
     uint32_t seg_cap = 0;    // capacity of seg_bag (elements), sized for K_min
     uint32_t num_tiles = 0, num_chunks = 0, tiles_per_chunk = 0;
-    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 1, 0, 0, 0, 0, 0};  // PDL on: 4-10 % per step on small batches, neutral on large ones
+    int32_t opt[DPI_OPT_COUNT_] = {0, 0, 0, 0, -1, 1, 0, 0, 0, 0, 0, 0};  // PDL on: 4-10 % per step on small batches, neutral on large ones
     // device
     int device = 0, num_sms = 0;
     int32_t* offsets = nullptr;
@@ -98,6 +101,7 @@ struct dpi_plan_s {
     // Launch configurations, computed when the plan is created or re-configured (prepare_launches): occupancy queries
     // and shared-memory attributes happen there, for the plan's device -- a lookup only fills in pointers and launches.
     LookupLaunch launch_dense{}, launch_gen{}, launch_gen_w{};   // balanced-segment kernel: dense / general / general + weights
+    LookupLaunch launch_dense16{};                               // dense with 128-bit row vectors (output not 32-byte aligned)
     int direct_grid_cap = 0;       // short-bag variant as its own launch: SMs x resident CTAs
     uint32_t fused_chunks = 0;     // fused single-launch path: CTAs (0 = no instantiation) and bags per CTA
     uint32_t fused_chunk_bags = 0;
@@ -108,6 +112,7 @@ struct dpi_plan_s {
 // stream c % 3, so the copy engines (both PCIe directions) and the SMs work on different chunks at the same time.
 struct HostPipeline {
     static constexpr int kStreams = 3;
+    int n_requested = 0;                // the chunk count this pipeline was built for
     std::vector<dpi_plan_t*> sub;       // one plan per chunk (B_c samples each)
     std::vector<int32_t> sample_lo;     // first sample of each chunk (+ B at the end)
     cudaStream_t st[kStreams] = {nullptr, nullptr, nullptr};
@@ -116,8 +121,18 @@ struct HostPipeline {
 
 namespace {
 
+// 256-bit row vectors in the dense balanced-segment kernel (DPI_OPT_VEC_BYTES = v). Possible whenever all dims are equal and
+// the row size is a multiple of 32 B; chosen by default only where it measured faster: fp32 rows of
+// >= 256 B (c5: 0.734 -> 0.716 ms). On 16-bit tables the wider accumulator set spills at the 64-register bound and halving
+// the lanes per row doubles the sub-warps whose partial sums meet by shuffle (c4: 0.382 -> 0.515 ms), so they stay at 128 bit.
+bool wide_allowed(const dpi_plan_t* p, int32_t v) {
+    const int64_t row_bytes = static_cast<int64_t>(p->D) * (p->dtype == DPI_F32 ? 4 : 2);
+    if (v == 16 || p->mixed_dims || row_bytes % 32 != 0) return false;
+    return v == 32 || (p->dtype == DPI_F32 && row_bytes >= 256);
+}
+
 int32_t default_quantum(const dpi_plan_t* p) {
-    // Measured on B200 (profiles/sweeps_r01.md): K = 128 is best once there are plenty of tasks per warp (c4/c5:
+    // Measured on B200 (DESIGN.md section 3 and 12 "Balanced quantum"): K = 128 is best once there are plenty of tasks per warp (c4/c5:
     // the per-task pipeline refill is amortised); small batches want more, smaller tasks so that every resident
     // warp has work: aim at >= 4 tasks per warp of a full persistent grid (32 warps per SM), within [16, 128].
     const uint64_t cost_bound = static_cast<uint64_t>(p->max_indices) + p->G;   // >= C[G]
@@ -166,15 +181,20 @@ int prepare(const dpi_plan_t* p, const LookupArgs& a, const LookupLaunch& l) {
     }
 }
 
-LookupLaunch prepare_one_launch(const dpi_plan_t* p, bool general, bool weights) {
+LookupLaunch prepare_one_launch(const dpi_plan_t* p, bool general, bool weights, bool wide = false) {
     LookupArgs a{};   // only T, idx_shift and weights != NULL enter the shared-memory size
     a.T = static_cast<uint32_t>(p->T);
     a.idx_shift = p->index_type == DPI_IDX_I64 ? 1u : 0u;
     a.weights = weights ? reinterpret_cast<const float*>(sizeof(float)) : nullptr;
     LookupLaunch l{};
-    l.lanes = p->lanes;
+    l.lanes = wide ? p->lanes_w : p->lanes;
     l.general = general;
+    l.vec32 = wide;
     l.unroll = (p->opt[DPI_OPT_UNROLL] && !general) ? p->opt[DPI_OPT_UNROLL] : 2;  // x2 by double buffering
+    // DPI_OPT_UNROLL counts 128-bit loads in flight per lane: a 256-bit load is two of them (default: ONE 256-bit load)
+    // (measured on c5: four 256-bit loads per batch and lane, 2 CTAs of 256 threads per SM, beat every
+    // 128-bit configuration and the shallower / deeper 256-bit ones)
+    if (wide) l.unroll = p->opt[DPI_OPT_UNROLL] ? std::min(l.lanes >= 8 ? 8 : 4, std::max(1, l.unroll / 2)) : 4;
     l.block_threads = p->opt[DPI_OPT_BLOCK_THREADS] ? p->opt[DPI_OPT_BLOCK_THREADS] : 256;
     l.out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
     int per_sm = prepare(p, a, l);   // also raises the instantiation's dynamic shared-memory limit when needed
@@ -191,7 +211,8 @@ LookupLaunch prepare_one_launch(const dpi_plan_t* p, bool general, bool weights)
 // Everything a launch needs that costs a CUDA runtime call. Runs in dpi_plan_create and in every setter that changes an
 // input of it (options, quantum, output dtype, layout) -- never in dpi_lookup / dpi_forward.
 void prepare_launches(dpi_plan_t* p) {
-    p->launch_dense = prepare_one_launch(p, false, false);
+    p->launch_dense16 = prepare_one_launch(p, false, false);
+    p->launch_dense = p->wide ? prepare_one_launch(p, false, false, true) : p->launch_dense16;
     p->launch_gen = prepare_one_launch(p, true, false);
     p->launch_gen_w = prepare_one_launch(p, true, true);
     const bool out32 = p->dtype != DPI_F32 && p->out_dtype == DPI_F32;
@@ -208,6 +229,7 @@ void prepare_launches(dpi_plan_t* p) {
         if (chunks < 1) chunks = 1;
         p->fused_chunk_bags = static_cast<uint32_t>((p->G + chunks - 1) / chunks);
         p->fused_chunks = (p->G + p->fused_chunk_bags - 1) / p->fused_chunk_bags;
+        if (p->fused_chunk_bags > static_cast<uint32_t>(kFusedMaxChunkBags)) p->fused_chunks = 0;   // a thread keeps <= 8 bags in registers
     }
 }
 
@@ -303,7 +325,10 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
         if (e != cudaSuccess) return cuda_fail(e, "direct lookup kernel launch");
         return DPI_OK;
     }
-    const LookupLaunch& l = !general ? p->launch_dense : (c.weights ? p->launch_gen_w : p->launch_gen);
+    // 256-bit row vectors store 32 bytes per lane: an output block that is only 16-byte aligned takes the 128-bit kernel
+    const bool out32b = ((reinterpret_cast<uintptr_t>(c.out) | a.out_pitch) & 31u) == 0;
+    const LookupLaunch& l = !general ? (out32b ? p->launch_dense : p->launch_dense16) : (c.weights ? p->launch_gen_w : p->launch_gen);
+    if (l.vec32) a.nvec = p->nvec_w;
     cudaError_t e;
     switch (p->dtype) {
         case DPI_F32: e = launch_lookup_f32(a, l, stream); break;
@@ -366,6 +391,7 @@ dpi_status_t launch_fused_forward(dpi_plan_t* p, const int32_t* lengths_dev, con
     f.plan = plan_args(p, lengths_dev);
     f.plan.num_chunks = p->fused_chunks;
     f.chunk_bags = p->fused_chunk_bags;
+    f.items = (p->fused_chunk_bags + kFusedThreads - 1) / kFusedThreads;
     LookupArgs& a = f.look;
     a.tables = c.tables;
     a.indices = static_cast<const int32_t*>(c.indices);
@@ -382,7 +408,10 @@ dpi_status_t launch_fused_forward(dpi_plan_t* p, const int32_t* lengths_dev, con
     if (c.pooling) {
         for (int t = 0; t < p->T; ++t) {
             if (c.pooling[t] > 1) return fail(DPI_ERR_INVALID_ARG, "pooling[%d] = %d is not a dpi_pool_t", t, c.pooling[t]);
-            if (c.pooling[t] == DPI_POOL_MEAN) a.pool.w[t >> 5] |= 1u << (t & 31);
+            if (c.pooling[t] == DPI_POOL_MEAN) {
+                a.pool.w[t >> 5] |= 1u << (t & 31);
+                f.any_mean = 1;
+            }
         }
     }
     cudaError_t e = launch_fused(f, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->opt[DPI_OPT_PDL] != 0, stream);
@@ -449,9 +478,12 @@ dpi_status_t dpi_plan_create(int32_t T, const int64_t* table_rows, const int32_t
     p->max_indices = max_indices;
     p->nvec = static_cast<uint32_t>(row_bytes / 16);
     p->lanes = pow2ceil(static_cast<int>(p->nvec));
+    p->nvec_w = static_cast<uint32_t>(row_bytes / 32);
+    p->lanes_w = pow2ceil(static_cast<int>(p->nvec_w > 0 ? p->nvec_w : 1));
     p->table_rows.assign(table_rows, table_rows + T);
     p->dims.assign(dims, dims + T);
     p->mixed_dims = mixed;
+    p->wide = wide_allowed(p, 0);
     p->out_width = out_width;
     p->device = dev;
     p->num_sms = prop.multiProcessorCount;
@@ -541,12 +573,20 @@ dpi_status_t dpi_plan_set_option(dpi_plan_t* p, dpi_option_t opt, int32_t v) {
         case DPI_OPT_MAX_BAG_HINT: ok = v >= 0; break;
         case DPI_OPT_FUSED: ok = v >= 0 && v <= 2; break;
         case DPI_OPT_FUSED_MAX_BAGS: ok = v >= 0; break;
+        case DPI_OPT_VEC_BYTES: ok = v == 0 || v == 16 || v == 32; break;
         default: return fail(DPI_ERR_INVALID_ARG, "unknown option %d", (int)opt);
     }
     if (!ok) return fail(DPI_ERR_INVALID_ARG, "value %d not supported for option %d", v, (int)opt);
     if (p->opt[opt] == v) return DPI_OK;
     p->opt[opt] = v;
-    if (opt == DPI_OPT_UNROLL || opt == DPI_OPT_BLOCK_THREADS || opt == DPI_OPT_BLOCKS_PER_SM || opt == DPI_OPT_PDL)
+    if (opt == DPI_OPT_VEC_BYTES) {
+        p->wide = wide_allowed(p, v);
+        if (v == 32 && !p->wide) {
+            p->opt[opt] = 0;
+            return fail(DPI_ERR_UNSUPPORTED, "DPI_OPT_VEC_BYTES = 32 needs equal dims and a row size that is a multiple of 32 B");
+        }
+    }
+    if (opt == DPI_OPT_UNROLL || opt == DPI_OPT_BLOCK_THREADS || opt == DPI_OPT_BLOCKS_PER_SM || opt == DPI_OPT_PDL || opt == DPI_OPT_VEC_BYTES)
         prepare_launches(p);
     return DPI_OK;
 }
@@ -812,6 +852,7 @@ dpi_status_t sync_subplan(const dpi_plan_t* p, dpi_plan_t* q) {
         changed |= q->opt[o] != p->opt[o];
         q->opt[o] = p->opt[o];
     }
+    q->wide = wide_allowed(q, q->opt[DPI_OPT_VEC_BYTES]);
     if (p->custom_columns != q->custom_columns || p->columns != q->columns) {
         dpi_status_t st = dpi_plan_set_columns(q, p->custom_columns ? p->columns.data() : nullptr);
         if (st != DPI_OK) return st;
@@ -822,24 +863,38 @@ dpi_status_t sync_subplan(const dpi_plan_t* p, dpi_plan_t* q) {
 }
 
 dpi_status_t ensure_pipeline(dpi_plan_t* p, int n_chunks) {
-    if (p->pipe && static_cast<int>(p->pipe->sub.size()) == n_chunks) return DPI_OK;
+    if (p->pipe && p->pipe->n_requested == n_chunks) return DPI_OK;
     free_pipeline(p);
     HostPipeline* h = new (std::nothrow) HostPipeline();
     if (!h) return fail(DPI_ERR_ALLOC, "host allocation failed");
     p->pipe = h;
+    h->n_requested = n_chunks;
     for (int i = 0; i < HostPipeline::kStreams; ++i) {
         DPI_CUDA(cudaStreamCreateWithFlags(&h->st[i], cudaStreamNonBlocking));
         DPI_CUDA(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
     }
     DPI_CUDA(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
-    const int32_t per = (p->B + n_chunks - 1) / n_chunks;
-    for (int32_t lo = 0; lo < p->B; lo += per) {
-        const int32_t Bc = std::min(per, p->B - lo);
+    // Chunk sizes: the device -> host stream of the output block is the bottleneck and cannot start before the first chunk
+    // has been copied in and pooled, so the first chunk is a quarter of the others (c5, 8 chunks: the output stream starts
+    // after ~0.07 ms instead of ~0.26 ms); the rest are equal.
+    std::vector<int32_t> sizes;
+    if (n_chunks >= 4 && p->B >= 4 * n_chunks) {
+        const int32_t first = std::max<int32_t>(1, p->B / (4 * n_chunks));
+        const int32_t rest = p->B - first, m = n_chunks - 1;
+        sizes.push_back(first);
+        for (int i = 0; i < m; ++i) sizes.push_back(rest / m + (i < rest % m ? 1 : 0));
+    } else {
+        const int32_t per = (p->B + n_chunks - 1) / n_chunks;
+        for (int32_t lo = 0; lo < p->B; lo += per) sizes.push_back(std::min(per, p->B - lo));
+    }
+    int32_t lo = 0;
+    for (int32_t Bc : sizes) {
         dpi_plan_t* q = nullptr;
         dpi_status_t st = dpi_plan_create(p->T, p->table_rows.data(), p->dims.data(), p->dtype, Bc, p->max_indices, &q);
         if (st != DPI_OK) return st;
         h->sub.push_back(q);
         h->sample_lo.push_back(lo);
+        lo += Bc;
     }
     h->sample_lo.push_back(p->B);
     return DPI_OK;
@@ -906,39 +961,49 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
     HostPipeline* h = p->pipe;
     const size_t n_sub = h->sub.size();
     // Copy sizes only: how many index entries belong to each chunk (the plan itself -- offsets, segments -- is still
-    // computed on the device, per chunk).
-    std::vector<int64_t> entry_lo(n_sub + 1, 0);
-    for (size_t c = 0; c < n_sub; ++c) {
-        const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T, g1 = static_cast<size_t>(h->sample_lo[c + 1]) * p->T;
-        int64_t n = 0;
-        if (sum_lengths(lengths_host, g0, g1, &n)) return fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length");
-        entry_lo[c + 1] = entry_lo[c] + n;
-    }
-    if (entry_lo[n_sub] != n_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)entry_lo[n_sub]);
-
+    // computed on the device, per chunk). The host adds up a chunk's lengths right before it enqueues that chunk, so the
+    // sums of the later chunks run under the transfers of the earlier ones.
     DPI_CUDA(cudaEventRecord(h->ev_in, s));
     for (int i = 0; i < HostPipeline::kStreams; ++i) DPI_CUDA(cudaStreamWaitEvent(h->st[i], h->ev_in, 0));
     const size_t row_bytes = static_cast<size_t>(p->out_width) * oelt;
-    for (size_t c = 0; c < n_sub; ++c) {
+    int64_t e0 = 0;
+    dpi_status_t bad = DPI_OK;
+    for (size_t c = 0; c < n_sub && bad == DPI_OK; ++c) {
         cudaStream_t cs = h->st[c % HostPipeline::kStreams];
         dpi_plan_t* q = h->sub[c];
-        st = sync_subplan(p, q);
-        if (st != DPI_OK) return st;
         const size_t g0 = static_cast<size_t>(h->sample_lo[c]) * p->T;
         const size_t n_g = static_cast<size_t>(q->G);
-        const int64_t e0 = entry_lo[c], n_e = entry_lo[c + 1] - entry_lo[c];
+        int64_t n_e = 0;
+        if (sum_lengths(lengths_host, g0, g0 + n_g, &n_e)) { bad = fail(DPI_ERR_INVALID_ARG, "lengths_host holds a negative length"); break; }
+        if (e0 + n_e > n_indices) { bad = fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to more", (long long)n_indices); break; }
+        bad = sync_subplan(p, q);
+        if (bad != DPI_OK) break;
         char* idx_dev = static_cast<char*>(p->stage_idx) + static_cast<size_t>(e0) * idx_elt;
         char* out_dev = out_base + static_cast<size_t>(h->sample_lo[c]) * row_bytes;
-        DPI_CUDA(cudaMemcpyAsync(p->stage_len + g0, lengths_host + g0, n_g * sizeof(int32_t), cudaMemcpyHostToDevice, cs));
-        if (n_e) DPI_CUDA(cudaMemcpyAsync(idx_dev, static_cast<const char*>(indices_host) + static_cast<size_t>(e0) * idx_elt,
-                                          static_cast<size_t>(n_e) * idx_elt, cudaMemcpyHostToDevice, cs));
+        cudaError_t ce = cudaMemcpyAsync(p->stage_len + g0, lengths_host + g0, n_g * sizeof(int32_t), cudaMemcpyHostToDevice, cs);
+        if (ce == cudaSuccess && n_e)
+            ce = cudaMemcpyAsync(idx_dev, static_cast<const char*>(indices_host) + static_cast<size_t>(e0) * idx_elt,
+                                 static_cast<size_t>(n_e) * idx_elt, cudaMemcpyHostToDevice, cs);
+        if (ce != cudaSuccess) { bad = cuda_fail(ce, "cudaMemcpyAsync (host -> device)"); break; }
         LookupCall lc;
         lc.tables = table_ptrs_dev; lc.indices = idx_dev; lc.pooling = pooling; lc.out = out_dev;
-        st = forward_device(q, p->stage_len + g0, lc, cs);
-        if (st != DPI_OK) return st;
-        if (!out_direct)
-            DPI_CUDA(cudaMemcpyAsync(static_cast<char*>(out_host) + static_cast<size_t>(h->sample_lo[c]) * row_bytes, out_dev,
-                                     static_cast<size_t>(q->B) * row_bytes, cudaMemcpyDeviceToHost, cs));
+        bad = forward_device(q, p->stage_len + g0, lc, cs);
+        if (bad != DPI_OK) break;
+        if (!out_direct) {
+            ce = cudaMemcpyAsync(static_cast<char*>(out_host) + static_cast<size_t>(h->sample_lo[c]) * row_bytes, out_dev,
+                                 static_cast<size_t>(q->B) * row_bytes, cudaMemcpyDeviceToHost, cs);
+            if (ce != cudaSuccess) { bad = cuda_fail(ce, "cudaMemcpyAsync (device -> host)"); break; }
+        }
+        e0 += n_e;
+    }
+    if (bad == DPI_OK && e0 != n_indices) bad = fail(DPI_ERR_INVALID_ARG, "n_indices=%lld but the lengths sum to %lld", (long long)n_indices, (long long)e0);
+    if (bad != DPI_OK) {   // chunks already enqueued run to completion before the error is returned (out_host is then undefined)
+        char keep[sizeof g_err];
+        std::memcpy(keep, g_err, sizeof keep);
+        for (int i = 0; i < HostPipeline::kStreams; ++i) (void)cudaStreamSynchronize(h->st[i]);
+        (void)cudaGetLastError();
+        std::memcpy(g_err, keep, sizeof keep);
+        return bad;
     }
     for (int i = 0; i < HostPipeline::kStreams; ++i) {
         DPI_CUDA(cudaEventRecord(h->ev_done[i], h->st[i]));

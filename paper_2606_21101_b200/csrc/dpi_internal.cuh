@@ -63,9 +63,11 @@ struct PlanArgs {
 cudaError_t launch_plan(const PlanArgs& a, cudaStream_t stream);
 
 // ---- a1 + a2 + a3 in one launch (forward_fused.cu) ----
-constexpr int kFusedThreads = 512;
-constexpr int kFusedMaxChunks = 512;                        // one look-back record per thread of a CTA
-constexpr int kFusedIdxStage = 4096;                        // index entries of a 512-bag tile staged in shared memory
+constexpr int kFusedThreads = 256;
+constexpr int kFusedItems = 8;                              // bags per thread, held in registers across the look-back
+constexpr int kFusedMaxChunkBags = kFusedThreads * kFusedItems;
+constexpr int kFusedMaxChunks = 640;                        // CTAs (one resident wave: 148 SMs x 4)
+constexpr int kFusedIdxStage = 3072;                        // index entries of a chunk staged in shared memory
 constexpr int kStatusRecords = kFusedMaxChunks > kMaxChunks ? kFusedMaxChunks : kMaxChunks;
 
 struct CheckArgs {
@@ -92,7 +94,8 @@ struct LookupArgs {
     void* __restrict__ out;                  // [G * D] in the output dtype (out[b, t*D + c] == out[g*D + c])
     uint32_t G;
     uint32_t T;
-    uint32_t nvec;                           // 16-byte vectors per row = D*sizeof(elt)/16 (the widest table when dims differ)
+    uint32_t nvec;                           // lane vectors per row = D*sizeof(elt)/16 (the widest table when dims differ); the
+                                             // 256-bit instantiations of lookup_kernel take D*sizeof(elt)/32
     int32_t mode;                            // 0 auto, 1 sub-warp per bag, 2 warp per bag
     // ---- general variant only (dpi_lookup_ex; lookup_kernel<..., GEN = true>) ----
     const float* __restrict__ weights;       // NULL or fp32[N]: one weight per index entry
@@ -111,7 +114,9 @@ struct LookupArgs {
 struct FusedArgs {
     PlanArgs plan;
     LookupArgs look;
-    uint32_t chunk_bags;
+    uint32_t chunk_bags;                 // <= kFusedMaxChunkBags
+    uint32_t items;                      // bags per thread = ceil(chunk_bags / kFusedThreads)
+    uint32_t any_mean;                   // some table is mean-pooled (else the pooling mask is never consulted)
 };
 cudaError_t launch_fused(const FusedArgs& a, int dtype, bool out32, int lanes, bool pdl, cudaStream_t stream);
 int fused_occupancy(int dtype, bool out32, int lanes, uint32_t T);   // resident CTAs per SM (0: no instantiation)
@@ -124,6 +129,7 @@ struct LookupLaunch {
     bool pdl;           // programmatic dependent launch
     bool out32;         // 16-bit tables only: emit the output block in fp32
     bool general;       // the GEN instantiation (interface variants)
+    bool vec32;         // 256-bit row vectors (Wide<Traits>): lanes = pow2ceil(row bytes / 32); dense layout only
 };
 
 // Each returns cudaErrorInvalidValue when (lanes, unroll, block_threads) has no instantiation.

@@ -44,6 +44,22 @@ __device__ __forceinline__ uint4 ld_row16(const void* p, bool pred) {
         : "+r"(r.x), "+r"(r.y), "+r"(r.z), "+r"(r.w) : "l"(p), "r"(static_cast<int>(pred)));
     return r;
 }
+// The sm_100 256-bit form of the same load (LDG.E.256): one lane holds 32 bytes of the row, so a row needs half the lanes,
+// a warp holds twice the rows per load instruction and the index reads / address arithmetic per gathered byte halve
+// (DESIGN.md 7.2.2). Needs 32-byte aligned rows: row size a multiple of 32 B and 32-byte aligned table bases.
+struct Row32 {
+    uint4 lo, hi;
+};
+__device__ __forceinline__ Row32 ld_row32(const void* p, bool pred) {
+    Row32 r;
+    r.lo = make_uint4(0u, 0u, 0u, 0u);
+    r.hi = make_uint4(0u, 0u, 0u, 0u);
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %9, 0;\n\t"
+        "@p ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+        : "+r"(r.lo.x), "+r"(r.lo.y), "+r"(r.lo.z), "+r"(r.lo.w), "+r"(r.hi.x), "+r"(r.hi.y), "+r"(r.hi.z), "+r"(r.hi.w)
+        : "l"(p), "r"(static_cast<int>(pred)));
+    return r;
+}
 // streaming stores: the output block is consumed by the next layer, not re-read here
 __device__ __forceinline__ void st_out16(void* p, const uint4& v) {
     asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
@@ -51,6 +67,11 @@ __device__ __forceinline__ void st_out16(void* p, const uint4& v) {
 __device__ __forceinline__ void st_out32(void* p, const float (&f)[8]) {  // sm_100 256-bit store
     asm volatile("st.global.cs.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(f[0]), "f"(f[1]), "f"(f[2]),
                  "f"(f[3]), "f"(f[4]), "f"(f[5]), "f"(f[6]), "f"(f[7]) : "memory");
+}
+__device__ __forceinline__ void st_row(void* p, const uint4& v) { st_out16(p, v); }
+__device__ __forceinline__ void st_row(void* p, const Row32& v) {
+    asm volatile("st.global.cs.v8.u32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(v.lo.x), "r"(v.lo.y), "r"(v.lo.z), "r"(v.lo.w),
+                 "r"(v.hi.x), "r"(v.hi.y), "r"(v.hi.z), "r"(v.hi.w) : "memory");
 }
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 // Plan data (segments, offsets, meta) is written by the planner grid this kernel may have been launched under (PDL), so
@@ -71,6 +92,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 __device__ __forceinline__ void add2(float2& a, float x, float y) { a = __fadd2_rn(a, make_float2(x, y)); }
 
 struct F32Traits {
+    static constexpr int kVecBytes = 16;  // bytes of a row held by one lane
+    using Row = uint4;
+    __device__ static __forceinline__ Row load(const void* p, bool pred) { return ld_row16(p, pred); }
     static constexpr int kAcc = 4;   // fp32 accumulators per lane (one 16-byte vector of the row)
     static constexpr int kEltBytes = 4;
     __device__ static __forceinline__ void add(float2 (&acc)[2], const uint4& v) {
@@ -87,6 +111,9 @@ struct F32Traits {
     }
 };
 struct F16Traits {
+    static constexpr int kVecBytes = 16;  // bytes of a row held by one lane
+    using Row = uint4;
+    __device__ static __forceinline__ Row load(const void* p, bool pred) { return ld_row16(p, pred); }
     static constexpr int kAcc = 8;
     static constexpr int kEltBytes = 2;
     __device__ static __forceinline__ void add(float2 (&acc)[4], const uint4& v) {
@@ -114,6 +141,9 @@ struct F16Traits {
     }
 };
 struct BF16Traits {
+    static constexpr int kVecBytes = 16;  // bytes of a row held by one lane
+    using Row = uint4;
+    __device__ static __forceinline__ Row load(const void* p, bool pred) { return ld_row16(p, pred); }
     static constexpr int kAcc = 8;
     static constexpr int kEltBytes = 2;
     __device__ static __forceinline__ void add(float2 (&acc)[4], const uint4& v) {
@@ -139,6 +169,33 @@ struct BF16Traits {
     }
 };
 
+// 32 bytes of the row per lane (256-bit loads): two halves of the base type side by side, element order preserved.
+template <class Base>
+struct Wide {
+    static constexpr int kAcc = 2 * Base::kAcc;
+    static constexpr int kEltBytes = Base::kEltBytes;
+    static constexpr int kVecBytes = 32;
+    static constexpr int kH = Base::kAcc / 2;   // float2 accumulators per half
+    using Row = Row32;
+    using Half = float2 (&)[kH];
+    using CHalf = const float2 (&)[kH];
+    __device__ static __forceinline__ Row load(const void* p, bool pred) { return ld_row32(p, pred); }
+    __device__ static __forceinline__ void add(float2 (&acc)[2 * kH], const Row32& v) {
+        Base::add(reinterpret_cast<Half>(acc[0]), v.lo);
+        Base::add(reinterpret_cast<Half>(acc[kH]), v.hi);
+    }
+    __device__ static __forceinline__ void fma(float2 (&acc)[2 * kH], const Row32& v, const float2 w) {
+        Base::fma(reinterpret_cast<Half>(acc[0]), v.lo, w);
+        Base::fma(reinterpret_cast<Half>(acc[kH]), v.hi, w);
+    }
+    __device__ static __forceinline__ Row32 pack(const float2 (&acc)[2 * kH]) {
+        Row32 r;
+        r.lo = Base::pack(reinterpret_cast<CHalf>(acc[0]));
+        r.hi = Base::pack(reinterpret_cast<CHalf>(acc[kH]));
+        return r;
+    }
+};
+
 template <int N2>
 __device__ __forceinline__ void zero_acc(float2 (&acc)[N2]) {
 #pragma unroll
@@ -156,16 +213,22 @@ __device__ __forceinline__ void scale_mean(float2 (&acc)[N2], int len) {
     for (int i = 0; i < N2; ++i) acc[i] = __fmul2_rn(acc[i], inv2);
 }
 
-// Store one pooled vector (16 B of table-dtype elements, or 32 B of fp32 for OUT32 with 16-bit tables) at p.
+// Store one pooled vector (kVecBytes of table-dtype elements, or twice that in fp32 for OUT32 with 16-bit tables) at p.
 template <class Tr, bool OUT32>
 __device__ __forceinline__ void store_pooled(char* p, const float2 (&acc)[Tr::kAcc / 2]) {
-    if constexpr (OUT32 && Tr::kAcc == 8) {
-        const float f[8] = {acc[0].x, acc[0].y, acc[1].x, acc[1].y, acc[2].x, acc[2].y, acc[3].x, acc[3].y};
-        st_out32(p, f);
+    if constexpr (OUT32 && Tr::kEltBytes == 2) {
+#pragma unroll
+        for (int i = 0; i < Tr::kAcc / 8; ++i) {
+            const float f[8] = {acc[4 * i].x, acc[4 * i].y, acc[4 * i + 1].x, acc[4 * i + 1].y,
+                                acc[4 * i + 2].x, acc[4 * i + 2].y, acc[4 * i + 3].x, acc[4 * i + 3].y};
+            st_out32(p + 32 * i, f);
+        }
     } else {
-        st_out16(p, Tr::pack(acc));
+        st_row(p, Tr::pack(acc));
     }
 }
+template <class Tr, bool OUT32>
+__host__ __device__ constexpr int out_vec_bytes() { return (OUT32 && Tr::kEltBytes == 2) ? 2 * Tr::kVecBytes : Tr::kVecBytes; }
 
 // ---- short-bag body (a3 variant) -------------------------------------------------------------
 // Algorithm 1's division of labour (every thread fills its own piece of the output matrix, no shared
@@ -180,9 +243,10 @@ template <class Tr, int W, int U, bool OUT32>
 __device__ __forceinline__ void short_bag_body(const LookupArgs& a, const char* const* s_tab, uint32_t q, uint32_t sl,
                                                uint32_t n_groups) {
     constexpr int kAcc2 = Tr::kAcc / 2;
-    constexpr int kOutVec = (OUT32 && Tr::kAcc == 8) ? 32 : 16;
+    constexpr int kVB = Tr::kVecBytes;
+    constexpr int kOutVec = out_vec_bytes<Tr, OUT32>();
     const bool vec_ok = sl < a.nvec;
-    const uint32_t row_bytes = a.nvec * 16;
+    const uint32_t row_bytes = a.nvec * kVB;
     const uint32_t t_step = n_groups % a.T;
     char* const out = static_cast<char*>(a.out);
     uint32_t t = q % a.T;
@@ -205,13 +269,13 @@ __device__ __forceinline__ void short_bag_body(const LookupArgs& a, const char* 
 #pragma unroll
         for (int u = 0; u < U; ++u) zero_acc(acc[u]);
         for (int j = 0; j < max_len; ++j) {
-            uint4 v[U];
+            typename Tr::Row v[U];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const bool ok = vec_ok && j < len[u];
                 // int64 ids are read through their low words (little-endian, rows < 2^31): idx_shift = 1
                 const uint32_t r = ok ? static_cast<uint32_t>(__ldg(a.indices + (static_cast<size_t>(lo[u] + j) << a.idx_shift))) : 0u;
-                v[u] = ld_row16(s_tab[tt[u]] + static_cast<uint64_t>(r) * row_bytes + sl * 16, ok);
+                v[u] = Tr::load(s_tab[tt[u]] + static_cast<uint64_t>(r) * row_bytes + sl * kVB, ok);
             }
 #pragma unroll
             for (int u = 0; u < U; ++u) Tr::add(acc[u], v[u]);
@@ -251,12 +315,24 @@ struct BagRef {
 // GEN = true adds the interface variants of SURVEY.md §8(f) NEXT-2 / NEXT-3 (dpi_lookup_ex): per-table dims,
 // int64 ids (the low word is read: rows < 2^31), per-entry fp32 weights (acc = fma(w, row, acc)), table-major
 // bags (g = t*B + b) and an output row pitch, so a column block can be written into a wider row.
+// Resident CTAs per SM the register allocation is held to: 32 bytes of row per load batch and lane (U = 2 x 128-bit, or
+// U = 1 x 256-bit) fit 64 registers = 4 CTAs; U = 2 x 256-bit gets 80 registers = 3 CTAs; deeper unrolls stay natural.
+template <class Tr, int U, bool GEN>
+__host__ __device__ constexpr int lookup_min_ctas() {
+    if (GEN) return U <= 2 ? 3 : 1;
+    if (Tr::kVecBytes == 32) return U == 1 ? 4 : (U == 2 ? 3 : 1);
+    return U <= 2 ? 4 : 1;
+}
+
 template <class Tr, int W, int U, bool OUT32, bool GEN>
-__global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <= 2 ? 3 : 1)) lookup_kernel(const LookupArgs a) {
+__global__ void __launch_bounds__(kLookupMaxThreads, lookup_min_ctas<Tr, U, GEN>()) lookup_kernel(const LookupArgs a) {
     constexpr int P = 32 / W;
     constexpr int kAcc = Tr::kAcc;
     constexpr int kAcc2 = kAcc / 2;
-    constexpr int kOutVec = (OUT32 && kAcc == 8) ? 32 : 16;  // output bytes per lane
+    constexpr int kVB = Tr::kVecBytes;                       // row bytes per lane
+    constexpr int kOutVec = out_vec_bytes<Tr, OUT32>();      // output bytes per lane
+    static_assert(!GEN || kVB == 16, "the general variant keeps per-table widths in 16-byte vectors");
+    using Row = typename Tr::Row;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int lane = threadIdx.x & 31;
@@ -267,7 +343,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
     const uint32_t n_warps = gridDim.x * warps_per_cta;
     const uint32_t warp_in_cta = threadIdx.x >> 5;
     const uint32_t warp_id = blockIdx.x * warps_per_cta + warp_in_cta;
-    const uint32_t row_bytes_u = a.nvec * 16;  // non-GEN: every table
+    const uint32_t row_bytes_u = a.nvec * kVB;  // non-GEN: every table
     char* const out = static_cast<char*>(a.out);
 
     // smem: [per-table records][per warp: idx stage x2, offsets stage x2, (GEN) weight stage x2]
@@ -321,8 +397,8 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
             if (a.table_major) { r.t = g / a.B; b = g - r.t * a.B; }
             else { b = g / a.T; r.t = g - b * a.T; }
             const TableInfo ti = s_info[r.t];
-            r.tab = ti.base + sl * 16;
-            r.row_bytes = ti.nvec * 16;
+            r.tab = ti.base + sl * kVB;
+            r.row_bytes = ti.nvec * kVB;
             r.ok = static_cast<uint32_t>(sl) < ti.nvec;
             char* row0 = out;
             if (a.peer_out) {  // fused all-to-all: sample b lives on peer b / rows_per_peer (NEXT-3)
@@ -333,7 +409,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
             r.outp = row0 + static_cast<size_t>(b) * a.out_pitch + static_cast<size_t>(ti.col_vec) * kOutVec + sl * kOutVec;
         } else {
             r.t = g % a.T;
-            r.tab = s_tab[r.t] + sl * 16;
+            r.tab = s_tab[r.t] + sl * kVB;
             r.row_bytes = row_bytes_u;
             r.ok = vec_ok;
             r.outp = nullptr;
@@ -353,7 +429,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                 if (t >= a.T) t %= a.T;  // only after a run of >= T empty bags
             }
             r.t = t;
-            r.tab = s_tab[t] + sl * 16;
+            r.tab = s_tab[t] + sl * kVB;
             return r;
         }
     };
@@ -366,7 +442,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
         return static_cast<uint32_t>(GEN ? ip[static_cast<ptrdiff_t>(e) << ish] : ip[e]);  // 64-bit: e may reach 2^30 with int64 ids
     };
     auto wgt_at = [&](const float* wp, int e) -> float { return (GEN && wp) ? wp[e] : 1.f; };
-    auto accum = [&](float2 (&acc)[kAcc2], const uint4& v, float w) {
+    auto accum = [&](float2 (&acc)[kAcc2], const Row& v, float w) {
         if constexpr (GEN) Tr::fma(acc, v, make_float2(w, w));  // fma(x, 1, acc) == x + acc exactly
         else Tr::add(acc, v);
     };
@@ -439,7 +515,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
             if (onehot) {
                 // ---------------- one-hot task: Alg. 1, a pure row copy (bit-exact) ------------------------
                 for (uint32_t i0 = 0; i0 < nb; i0 += P * U) {
-                    uint4 v[U];
+                    Row v[U];
                     BagRef br[GEN ? U : 1];
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
@@ -448,7 +524,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                         BagRef& b = br[GEN ? u : 0];
                         b = bag_ref(g_lo + (ok ? i : 0u));
                         const uint32_t r = idx_at(ip, e_lo + (ok ? i : 0u));
-                        v[u] = ld_row16(b.tab + static_cast<uint64_t>(r) * b.row_bytes, ok && b.ok);
+                        v[u] = Tr::load(b.tab + static_cast<uint64_t>(r) * b.row_bytes, ok && b.ok);
                     }
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
@@ -456,13 +532,13 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                         const BagRef& b = br[GEN ? u : 0];
                         if (i < nb && b.ok) {  // dense layout: b.ok == vec_ok for every bag
                             char* po = out_of(g_lo + i, b);
-                            if constexpr (OUT32 && kAcc == 8) {
+                            if constexpr (OUT32 && Tr::kEltBytes == 2) {
                                 float2 f[kAcc2];
                                 zero_acc(f);
                                 Tr::add(f, v[u]);
                                 store_pooled<Tr, OUT32>(po, f);
                             } else {
-                                st_out16(po, v[u]);
+                                st_row(po, v[u]);
                             }
                         }
                     }
@@ -479,7 +555,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                     float2 acc[kAcc2];
                     zero_acc(acc);
                     for (int j = lo; j < hi; j += U) {
-                        uint4 v[U];
+                        Row v[U];
                         float w[U];
 #pragma unroll
                         for (int u = 0; u < U; ++u) {
@@ -487,7 +563,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                             const int e = ok ? j + u : lo;
                             const uint32_t r = idx_at(ip, e);
                             w[u] = wgt_at(wp, e);
-                            v[u] = ld_row16(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
+                            v[u] = Tr::load(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
                         }
 #pragma unroll
                         for (int u = 0; u < U; ++u) accum(acc, v[u], w[u]);
@@ -505,7 +581,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                     float2 acc[kAcc2];
                     zero_acc(acc);
                     for (int j = lo; j < hi; j += P * U) {
-                        uint4 v[U];
+                        Row v[U];
                         float w[U];
 #pragma unroll
                         for (int u = 0; u < U; ++u) {
@@ -514,7 +590,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                             const int ec = ok ? e : lo;
                             const uint32_t r = idx_at(ip, ec);
                             w[u] = wgt_at(wp, ec);
-                            v[u] = ld_row16(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
+                            v[u] = Tr::load(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
                         }
 #pragma unroll
                         for (int u = 0; u < U; ++u) accum(acc, v[u], w[u]);
@@ -537,7 +613,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                 // are already in smem) are issued before batch k is consumed, so a warp keeps U..2U row
                 // loads per lane in flight across batch and bag boundaries instead of draining at each one.
                 struct Buf {
-                    uint4 v[U];
+                    Row v[U];
                     float w[GEN ? U : 1];
                 };
                 auto store_zero = [&](uint32_t gz) {
@@ -556,7 +632,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, (U <= 2 && !GEN) ? 4 : (U <
                         const int ec = ok ? e : j;
                         const uint32_t r = idx_at(ip, ec);
                         if constexpr (GEN) bf.w[u] = wgt_at(wp, ec);
-                        bf.v[u] = ld_row16(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
+                        bf.v[u] = Tr::load(br.tab + static_cast<uint64_t>(r) * br.row_bytes, ok && br.ok);
                     }
                 };
                 uint32_t g = g_lo;
@@ -681,6 +757,11 @@ int prepare_one(const LookupArgs& a, int block_threads) {
 #define DPI_FOR_EACH_WU(M) \
     DPI_FOR_EACH_U(M, 1) DPI_FOR_EACH_U(M, 2) DPI_FOR_EACH_U(M, 4) DPI_FOR_EACH_U(M, 8) DPI_FOR_EACH_U(M, 16) \
     DPI_FOR_EACH_U(M, 32)
+// 256-bit row vectors (Wide<Traits>): rows of up to 512 B need at most 16 lanes.
+#define DPI_FOR_EACH_U_WIDE(M, W) M(W, 1) M(W, 2) M(W, 4)
+#define DPI_FOR_EACH_WU_WIDE(M) \
+    DPI_FOR_EACH_U_WIDE(M, 1) DPI_FOR_EACH_U_WIDE(M, 2) DPI_FOR_EACH_U_WIDE(M, 4) DPI_FOR_EACH_U_WIDE(M, 8) M(8, 8) \
+    DPI_FOR_EACH_U_WIDE(M, 16) M(16, 8)
 // The general variant (GEN) exists for the default unroll only.
 #define DPI_FOR_EACH_W_GEN(M) M(1, 2) M(2, 2) M(4, 2) M(8, 2) M(16, 2) M(32, 2)
 // Each lookup_<dtype>.cu defines DPI_TRAITS / DPI_SUFFIX (/ DPI_HAS_OUT32) and includes lookup_dispatch.inc.

@@ -121,20 +121,134 @@ def table_shard_batch(batch: W.Batch, T: int, tables) -> W.Batch:
     return W.Batch(sel_ln.astype(np.int32), np.ascontiguousarray(batch.indices[src]))
 
 
+class _DeviceBlock:
+    """A raw device allocation presented to torch through __cuda_array_interface__ (no copy, no ownership)."""
+
+    def __init__(self, ptr: int, shape, typestr: str):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (ptr, False), "version": 2}
+
+
+_TYPESTR = {"torch.float32": "<f4", "torch.float16": "<f2", "torch.bfloat16": "<u2"}
+
+
+class PeerOutput:
+    """This rank's [rows_per_rank, width] batch shard, allocated where the other ranks' lookup kernels can store into it
+    (dpi_peer_alloc: one dedicated allocation + CUDA IPC handle), plus every rank's base pointer as the device array
+    dpi_lookup_ex(out_peers_dev) takes. Works for ranks on different GPUs (stores cross NVLink) and for ranks sharing one
+    device (the one-GPU test of the multi-process glue). world 1 / no process group: a plain local block.
+
+    `local` is a torch view of this rank's block; `ptrs` the int64 device tensor [world]; `barrier()` orders consumers
+    after ALL ranks' kernels (synchronise the current device, then a control-plane barrier); `close()` unmaps and frees."""
+
+    def __init__(self, rows_per_rank: int, width: int, torch_dtype, device, group=None):
+        import torch
+        import torch.distributed as dist
+        from . import binding
+        self._dist = dist if (dist.is_available() and dist.is_initialized()) else None
+        self._group = group
+        self.world = self._dist.get_world_size(group) if self._dist else 1
+        self.rank = self._dist.get_rank(group) if self._dist else 0
+        elt = torch.empty((), dtype=torch_dtype).element_size()
+        nbytes = max(1, rows_per_rank * width * elt)
+        with torch.cuda.device(device):
+            self._own, handle = binding.peer_alloc(nbytes)
+            handles = [handle]
+            if self.world > 1:
+                handles = [None] * self.world
+                self._dist.all_gather_object(handles, handle, group=group)
+            self._opened = []
+            base = []
+            for r, h in enumerate(handles):
+                if r == self.rank:
+                    base.append(self._own)
+                else:
+                    p = binding.peer_open(h)
+                    self._opened.append(p)
+                    base.append(p)
+        block = _DeviceBlock(self._own, (rows_per_rank, width), _TYPESTR[str(torch_dtype)])
+        local = torch.as_tensor(block, device=device)
+        self.local = local.view(torch.bfloat16) if torch_dtype == torch.bfloat16 else local
+        self.ptrs = torch.tensor(base, dtype=torch.int64, device=device)
+        self._device = device
+
+    def barrier(self):
+        import torch
+        torch.cuda.synchronize(self._device)
+        if self._dist and self.world > 1:
+            self._dist.barrier(group=self._group)
+
+    def close(self):
+        from . import binding
+        import torch
+        if self._own is None:
+            return
+        torch.cuda.synchronize(self._device)
+        for p in self._opened:
+            binding.peer_close(p)
+        self._opened = []
+        if self._dist and self.world > 1:
+            self._dist.barrier(group=self._group)   # nobody still maps the block when it is freed
+        binding.peer_free(self._own)
+        self._own = None
+        self.local = None
+
+
 def peer_output_buffers(rows_per_rank: int, width: int, torch_dtype, device, group=None):
-    """Allocate this rank's [rows_per_rank, width] batch shard where the other ranks' kernels can store into it and
-    return (local tensor, int64 device tensor with every rank's base pointer, barrier callable).
-    world 1 (or no process group): an ordinary tensor and its own pointer. world > 1: torch symmetric memory
-    (CUDA IPC / multicast-capable allocations exchanged at rendezvous), pointers from the handle."""
-    import torch
-    import torch.distributed as dist
-    world = dist.get_world_size(group) if (dist.is_available() and dist.is_initialized()) else 1
-    if world == 1:
-        out = torch.empty((rows_per_rank, width), dtype=torch_dtype, device=device)
-        ptrs = torch.tensor([out.data_ptr()], dtype=torch.int64, device=device)
-        return out, ptrs, (lambda: None)
-    import torch.distributed._symmetric_memory as symm_mem
-    out = symm_mem.empty((rows_per_rank, width), dtype=torch_dtype, device=device)
-    hdl = symm_mem.rendezvous(out, group=group if group is not None else dist.group.WORLD)
-    ptrs = torch.tensor([int(p) for p in hdl.buffer_ptrs], dtype=torch.int64, device=device)
-    return out, ptrs, (lambda: hdl.barrier(channel=0))  # device-side barrier on the current stream
+    """(local tensor, device pointer array of every rank's block, barrier callable) -- see PeerOutput."""
+    po = PeerOutput(rows_per_rank, width, torch_dtype, device, group)
+    return po.local, po.ptrs, po.barrier
+
+
+class TableWiseLookup:
+    """Table-wise sharded lookup with the all-to-all fused into the store:
+    the single entry point that wires partition_tables -> table_shard_batch -> PeerOutput -> dpi_lookup_ex(out_peers_dev)
+    -> barrier. Rank r holds `tables_r` (all rows of each) and, per call, receives the bags of its tables for EVERY sample of
+    the global batch; its kernel stores each pooled vector into the batch shard of the rank that owns the sample, at the
+    table's global column. After `forward` returns, `out.local` holds this rank's rows [rank * rows_per_rank, ...) of the
+    global [B, sum dims] block, complete. Comm on the data path: peer stores only, no NCCL."""
+
+    def __init__(self, dims, table_rows, dtype_code: int, torch_dtype, B_global: int, max_indices: int, device, cost=None,
+                 group=None, out_dtype_code=None):
+        import torch.distributed as dist
+        from . import binding
+        on = dist.is_available() and dist.is_initialized()
+        self.world = dist.get_world_size(group) if on else 1
+        self.rank = dist.get_rank(group) if on else 0
+        dims = np.asarray(dims, dtype=np.int64)
+        table_rows = np.asarray(table_rows, dtype=np.int64)
+        self.T = int(dims.shape[0])
+        self.B = int(B_global)
+        self.parts = partition_tables(dims if cost is None else cost, self.world)
+        self.mine = self.parts[self.rank]
+        self.columns = table_columns(dims)
+        self.width = int(dims.sum())
+        self.rows_per_rank = -(-self.B // self.world)
+        self.device = device
+        self.plan = None
+        if self.mine:
+            self.plan = binding.Plan(table_rows[self.mine], np.asarray(dims[self.mine], np.int32), dtype_code, self.B, max_indices)
+            if out_dtype_code is not None:
+                self.plan.set_out_dtype(out_dtype_code)
+            self.plan.set_columns([int(self.columns[t]) for t in self.mine])
+        self.out = PeerOutput(self.rows_per_rank, self.width, torch_dtype, device, group)
+
+    def forward(self, lengths_dev, indices_dev, table_ptrs_dev, pooling=None, stream=None):
+        """lengths / indices: this rank's table shard of the global batch (table_shard_batch), on the device; table_ptrs_dev:
+        device pointer array of this rank's tables (ascending global id). Returns this rank's complete batch shard."""
+        if self.plan is not None:
+            self.plan.build(lengths_dev, stream)
+            self.plan.lookup_ex(table_ptrs_dev, indices_dev, None, pooling=pooling, out_ld=self.width,
+                                out_peers_dev=self.out.ptrs, n_peers=self.world, rows_per_peer=self.rows_per_rank, stream=stream)
+        self.out.barrier()
+        return self.out.local
+
+    def close(self):
+        if self.plan is not None:
+            self.plan.destroy()
+            self.plan = None
+        self.out.close()
+
+
+def table_wise_forward(tw: "TableWiseLookup", lengths_dev, indices_dev, table_ptrs_dev, pooling=None, stream=None):
+    """Functional spelling of TableWiseLookup.forward."""
+    return tw.forward(lengths_dev, indices_dev, table_ptrs_dev, pooling=pooling, stream=stream)

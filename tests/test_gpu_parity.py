@@ -613,3 +613,48 @@ def test_bag_length_hint_selects_the_short_bag_variant_and_a_broken_promise_is_s
         plan.check_indices(db.indices)
     assert e.value.status == 1 and "DPI_OPT_MAX_BAG_HINT" in e.value.detail
     plan.destroy()
+
+
+# --------------------------------------------------------------------------------------------------
+# 256-bit row vectors (DPI_OPT_VEC_BYTES): every Wide<Traits> instantiation against the oracle
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype,D,out", [("f32", 8, None), ("f32", 16, None), ("f32", 24, None), ("f32", 64, None), ("f32", 128, None),
+                                         ("f16", 16, None), ("f16", 48, None), ("f16", 64, "f32"), ("f16", 256, None),
+                                         ("bf16", 16, "f32"), ("bf16", 64, None), ("bf16", 64, "f32"), ("bf16", 256, "f32")])
+@pytest.mark.parametrize("lengths", [("const", 1), ("uniform", 0, 5), ("poisson", 20.0, 100, 0.05)])
+@pytest.mark.parametrize("unroll", [0, 2, 8])
+def test_256bit_row_vectors_match_the_oracle(dtype, D, out, lengths, unroll):
+    """Rows of 32 ... 512 B (1 ... 16 lanes per row, incl. the non-power-of-two 96-byte row), all three task shapes and the
+    device-picked short-bag body, table-dtype and fp32 output, one / two / four 256-bit loads per batch and lane."""
+    cfg = W.Config("w", 5, (1000, 17, 4000, 1, 250), D, dtype, 333, lengths, ("zipf", 1.05), "half", seed=12, out_dtype=out)
+    _full_parity(cfg, opts={binding.OPT_VEC_BYTES: 32, binding.OPT_UNROLL: unroll})
+
+
+def test_256bit_row_vectors_modes_c5_shape_and_fallbacks():
+    cfg = W.Config("w5", 8, (5000,) * 8, 64, "f32", 300, ("uniform", 1, 64), ("uniform",), "sum", seed=2)
+    for mode in (0, 1, 2, 3):   # auto rule: fp32 rows of 256 B take the 256-bit kernel without being asked
+        _full_parity(cfg, opts={binding.OPT_MODE: mode})
+    _full_parity(cfg, opts={binding.OPT_VEC_BYTES: 16})
+    _full_parity(cfg, K=7, opts={binding.OPT_VEC_BYTES: 32, binding.OPT_UNROLL: 16, binding.OPT_BLOCK_THREADS: 128})
+    # rows that are not a multiple of 32 B cannot take 256-bit vectors; asking for them is refused, auto stays at 128 bit
+    plan = binding.Plan([10, 10], np.asarray([12, 12], np.int32), 0, 4, 8)
+    with pytest.raises(binding.DpiError) as e:
+        plan.set_option(binding.OPT_VEC_BYTES, 32)
+    assert e.value.status == 2
+    plan.destroy()
+    # an output block that is only 16-byte aligned silently runs the 128-bit kernel (same results)
+    rows = cfg.table_rows()
+    host_tables = [W.full_table_storage(cfg, t, int(rows[t])) for t in range(cfg.T)]
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, rows, None)
+    db = harness.upload_batch(batch)
+    plan = harness.make_plan(cfg, rows, batch.N)
+    plan.build(db.lengths)
+    flat = torch.full((cfg.B * cfg.T * cfg.D + 4,), float("nan"), dtype=torch.float32, device="cuda")
+    out = flat[4:].view(cfg.B, cfg.T * cfg.D)          # 16 bytes past a 512-byte aligned allocation
+    assert out.data_ptr() % 32 == 16
+    plan.lookup(dt.ptrs, db.indices, out, pooling=cfg.pooling_modes())
+    torch.cuda.synchronize()
+    ref = oracle_reference(host_tables, cfg.dtype, cfg.B, batch.lengths, batch.indices, cfg.pooling_modes())
+    assert_outputs_match(harness.out_to_f64(out), ref, batch.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out)
+    plan.destroy()
