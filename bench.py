@@ -61,6 +61,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--fused", type=int, default=-1, help="dpi_forward: -1 library default (auto), 0 auto, 1 fused whenever the layout allows, 2 always planner + lookup")
     ap.add_argument("--vec-bytes", type=int, default=0, help="DPI_OPT_VEC_BYTES: 0 auto, 16 / 32 bytes of a row per lane and load")
+    ap.add_argument("--shard", default="batch", choices=["batch", "tables"],
+                    help="multi-GPU layout: batch-sharded replicas (default, DESIGN.md 9) or table-wise sharding with the all-to-all "
+                         "fused into the lookup's store (NEXT-3, DESIGN.md 11.3)")
     ap.add_argument("--rows-scale", type=float, default=1.0, help="debug: scale table heights (invalidates the run)")
     return ap.parse_args()
 
@@ -639,10 +642,112 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_table_sharded(args):
+    """NEXT-3: every rank holds a SUBSET of the tables and the bags of those tables for the
+    whole global batch of cfg.B samples; its fused lookup stores each pooled vector straight into the batch shard of the rank
+    that owns the sample (dpi_lookup_ex out_peers_dev over CUDA IPC / NVLink). Strong scaling: the global batch is fixed.
+    A step = planner + lookup on every rank + the barrier that makes all shards complete. Ranks may share a device (the
+    control plane is then gloo): that exercises the glue, not NVLink."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_21101_b200 import binding, build, harness, sharding, workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    n_dev = torch.cuda.device_count()
+    if n_dev == 0:
+        raise SystemExit("bench.py: no CUDA device; the DPI lookup has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", "0")) % n_dev
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+    shared_device = world > n_dev
+    if world > 1:
+        if shared_device:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    binding.load_library()
+    cfg, rows = workload_config(args)
+    warmup = max(args.warmup if args.warmup is not None else 5, 3)
+    steps = max(args.steps if args.steps is not None else 50, 1)
+    R = max(1, min(args.rotating_batches, 4))
+    dims = [cfg.D] * cfg.T
+    mean_len = {"const": lambda l: l[1], "uniform": lambda l: (l[1] + l[2]) / 2, "poisson": lambda l: l[1]}[cfg.lengths[0]](cfg.lengths)
+    tw = sharding.TableWiseLookup(dims, rows, W.DTYPE_CODE[cfg.dtype], harness.TORCH_DTYPE[cfg.out], cfg.B,
+                                  harness.max_indices_bound(cfg), device, cost=[mean_len * cfg.row_bytes] * cfg.T,
+                                  out_dtype_code=W.DTYPE_CODE[cfg.out] if cfg.out != cfg.dtype else None)
+    mine = tw.mine
+    tables = []
+    for t in mine:   # this rank's tables only, filled in place with the seeded recipe
+        buf = torch.empty((int(rows[t]), cfg.D), dtype=harness.TORCH_DTYPE[cfg.dtype], device=device)
+        binding.synth_fill_table(buf, buf.numel(), W.DTYPE_CODE[cfg.dtype], W.value_key(cfg.seed, t))
+        tables.append(buf)
+    ptrs = torch.tensor([t.data_ptr() for t in tables] or [0], dtype=torch.int64, device=device)
+    pooling = cfg.pooling_modes()[mine] if mine else None
+    batches = []
+    for r in range(R):
+        local_b = sharding.table_shard_batch(W.make_batch(cfg, rows, cfg.seed + r), cfg.T, mine)
+        batches.append(harness.upload_batch(local_b, device=device))
+    stream = torch.cuda.Stream()
+
+    def step(i):
+        b = batches[i % R]
+        with torch.cuda.stream(stream):
+            tw.forward(b.lengths, b.indices, ptrs, pooling=pooling, stream=stream)
+
+    for i in range(warmup):
+        step(i)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.05)
+    tw.out.barrier()
+    launches0 = binding.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record(stream)
+    for i in range(steps):
+        step(i)
+    e1.record(stream)
+    tw.out.barrier()
+    t1 = time.time()
+    launches = binding.launch_count() - launches0
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        allms = [None] * world
+        dist.all_gather_object(allms, ms)
+        ms = max(allms)
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    n_local = float(np.mean([b.N for b in batches]))
+    if rank == 0:
+        line = {"metric": METRIC, "value": cfg.G * steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+                "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": DTYPE_KEY[cfg.dtype], "data": "synthetic",
+                "config": describe(cfg, rows, {"parallelism": f"table-wise sharding x{world}: rank r pools its tables for the whole batch and "
+                                               "stores into the batch shard of the sample's owner",
+                                               "comm": "peer stores (CUDA IPC mapped blocks), no NCCL on the data path; one control-plane "
+                                                       "barrier per step",
+                                               "ranks_share_a_device": shared_device, "tables_of_rank0": mine,
+                                               "rows_gathered_per_step_rank0": n_local, "launch": "stream launches"}, R),
+                "gpu_launches": int(launches), "clocks": clocks, "device": torch.cuda.get_device_name(local),
+                "roofline": None, "cpu_baseline": None, "e2e": None,
+                "note": "NEXT-3 demonstration mode; the headline bench is the default --shard batch"}
+        print(json.dumps(line), flush=True)
+    tw.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard == "tables":
+        run_table_sharded(args)
     else:
         run_ours(args)
 

@@ -157,6 +157,27 @@ dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* plan, dpi_dtype_t out_dtype);
 dpi_status_t dpi_plan_set_layout(dpi_plan_t* plan, dpi_bag_order_t order, dpi_index_type_t index_type);
 
 /*
+ * dpi_plan_set_offset_type -- 64-bit offsets (SURVEY.md 8(f) NEXT-2 "int64 indices/offsets"; ids and their positions reach a
+ * serving stack as 64-bit integers). DPI_OFF_I32 (default): offsets, seg_off and N are int32, N < 2^31.
+ * DPI_OFF_I64: the same plan definition with int64 offsets[G+1], seg_off[S+1] and N, so one batch may hold N >= 2^31 index
+ * entries (G = B*T < 2^31 still; every single bag shorter than 2^31). max_indices: the new capacity (0 = keep), < 2^31 for
+ * DPI_OFF_I32, < 2^40 for DPI_OFF_I64. Invalidates the current build. With 64-bit offsets:
+ *   - dpi_plan_build runs the 64-bit planner (two stream-ordered launches instead of one);
+ *   - dpi_lookup / dpi_lookup_ex / dpi_forward run the general kernel (one launch); a caller-provided offsets_dev must be a
+ *     device int64[G+1] passed through the int32 pointer; dpi_plan_device_views returns offsets_dev as such a pointer and
+ *     meta words 8 / 9 hold the high halves of N / C[G];
+ *   - dpi_plan_export64 replaces dpi_plan_export; dpi_check_indices works unchanged;
+ *   - dpi_forward_host, dpi_lookup_input_first and the short-bag / fused single-launch variants are not available
+ *     (DPI_ERR_UNSUPPORTED, or silently not chosen).
+ */
+typedef enum { DPI_OFF_I32 = 0, DPI_OFF_I64 = 1 } dpi_offset_type_t;
+dpi_status_t dpi_plan_set_offset_type(dpi_plan_t* plan, dpi_offset_type_t type, int64_t max_indices);
+/* dpi_plan_export for a plan with 64-bit offsets: offsets_host int64[G+1], seg_bag_host int32[seg_cap], seg_off_host
+ * int64[seg_cap] (S+1 entries each; any may be NULL), S, N. Synchronises `stream`. */
+dpi_status_t dpi_plan_export64(const dpi_plan_t* plan, int64_t* offsets_host, int32_t* seg_bag_host, int64_t* seg_off_host,
+                               int64_t seg_cap, int64_t* S, int64_t* N, void* stream);
+
+/*
  * dpi_plan_set_columns -- place table t's block at column columns[t] (in elements) of the output row instead of the
  * running prefix of dims. columns: host int64[T], each columns[t]*sizeof(dtype) a multiple of 16 B; blocks must not
  * overlap (not checked); NULL restores the default. The row width becomes max_t(columns[t] + dims[t]). This is what a
@@ -196,8 +217,9 @@ dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims,
 
 /* Borrowed device pointers into the plan, valid until the next build/destroy. Any out-pointer may be NULL.
  *   offsets_dev int32[G+1]; seg_dev int32[2*seg_capacity], interleaved pairs {seg_bag[s], seg_off[s]};
- *   meta_dev int32[8] = {S, N, C[G] low 32 bits, overflow flag, K, G, min_len, max_len} (min / max bag length of the
- *   batch: a1's summary of the workload; min_len == max_len is the uniform-length flag). */
+ *   meta_dev int32[12] = {S, N (low 32 bits), C[G] (low 32 bits), overflow flag, K, G, min_len, max_len, N (high 32 bits),
+ *   C[G] (high 32 bits), -, -} (min / max bag length of the batch: a1's summary of the workload;
+ *   min_len == max_len is the uniform-length flag; the high words are zero unless the plan holds 64-bit offsets). */
 dpi_status_t dpi_plan_device_views(const dpi_plan_t* plan, const int32_t** offsets_dev,
                                    const int32_t** seg_dev, const int32_t** meta_dev);
 

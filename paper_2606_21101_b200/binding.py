@@ -22,6 +22,7 @@ DPI_POOL_SUM, DPI_POOL_MEAN = 0, 1
 OPT_UNROLL, OPT_BLOCK_THREADS, OPT_BLOCKS_PER_SM, OPT_MODE, OPT_ROW_L1_NO_ALLOC, OPT_PDL, OPT_HOST_CHUNKS, OPT_HOST_DIRECT_OUT, OPT_MAX_BAG_HINT, OPT_FUSED, OPT_FUSED_MAX_BAGS, OPT_VEC_BYTES = range(12)
 BAGS_SAMPLE_MAJOR, BAGS_TABLE_MAJOR = 0, 1
 IDX_I32, IDX_I64 = 0, 1
+OFF_I32, OFF_I64 = 0, 1
 LOOKUP_FORCE_GENERAL = 1
 
 # every symbol include/dpi.h declares (tests check the .so exports each one)
@@ -29,7 +30,8 @@ EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "
            "dpi_plan_set_quantum", "dpi_plan_set_option", "dpi_plan_get_option",
            "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export", "dpi_plan_stats",
            "dpi_lookup", "dpi_forward", "dpi_plan_status", "dpi_lookup_onehot", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
-           "dpi_version", "dpi_status_string", "dpi_last_error", "dpi_peer_alloc", "dpi_peer_open", "dpi_peer_close", "dpi_peer_free"]
+           "dpi_version", "dpi_status_string", "dpi_last_error", "dpi_peer_alloc", "dpi_peer_open", "dpi_peer_close", "dpi_peer_free",
+           "dpi_plan_set_offset_type", "dpi_plan_export64"]
 
 
 class LookupArgs(ctypes.Structure):
@@ -81,6 +83,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
         "dpi_plan_info": (st, [vp, vp, vp, vp, vp, vp, vp, vp]),
         "dpi_plan_export": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_plan_stats": (st, [vp, vp, vp, vp]),
+        "dpi_plan_set_offset_type": (st, [vp, ctypes.c_int, i64]),
+        "dpi_plan_export64": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_lookup": (st, [vp, vp, vp, vp, vp, vp, vp]),
         "dpi_lookup_input_first": (st, [vp, vp, vp, vp, vp, vp, vp]),
         "dpi_forward": (st, [vp, vp, vp, vp, vp, vp, vp]),
@@ -274,6 +278,21 @@ class Plan:
                                          ctypes.byref(S), ctypes.byref(N), _stream_handle(stream)))
         res = (offsets, seg[: S.value + 1].copy(), int(S.value), int(N.value))
         return res + (seg_off[: S.value + 1].copy(),) if with_seg_off else res
+
+    # -- dpi_plan_set_offset_type / dpi_plan_export64 (NEXT-2: 64-bit offsets) ------------------------------
+    def set_offset_type(self, offset_type: int, max_indices: int = 0):
+        _check(self._lib.dpi_plan_set_offset_type(self._h, int(offset_type), int(max_indices)))
+
+    def export64(self, stream=None):
+        """Plan with 64-bit offsets -> (offsets int64[G+1], seg_bag int32[S+1], S, N, seg_off int64[S+1]) (synchronises)."""
+        cap = self.info()["seg_capacity"]
+        offsets = np.empty(self.G + 1, dtype=np.int64)
+        seg = np.empty(cap, dtype=np.int32)
+        seg_off = np.empty(cap, dtype=np.int64)
+        S, N = ctypes.c_int64(), ctypes.c_int64()
+        _check(self._lib.dpi_plan_export64(self._h, offsets.ctypes.data, seg.ctypes.data, seg_off.ctypes.data, cap,
+                                           ctypes.byref(S), ctypes.byref(N), _stream_handle(stream)))
+        return offsets, seg[: S.value + 1].copy(), int(S.value), int(N.value), seg_off[: S.value + 1].copy()
 
     # -- dpi_plan_stats -------------------------------------------------------------------------------------
     def stats(self, stream=None):

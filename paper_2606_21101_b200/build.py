@@ -24,7 +24,7 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 LIBS = {
-    "libdpi.so": ["dpi_api.cu", "plan_kernels.cu", "lookup_f32.cu", "lookup_f16.cu", "lookup_bf16.cu",
+    "libdpi.so": ["dpi_api.cu", "plan_kernels.cu", "plan64_kernels.cu", "lookup_f32.cu", "lookup_f16.cu", "lookup_bf16.cu",
                   "ablation_input_first.cu", "lookup_onehot.cu", "lookup_direct.cu", "forward_fused.cu", "nongemm_kernels.cu", "nongemm_api.cu", "peer_api.cu"],
     "libdpi_synth.so": ["synth_fill.cu"],
 }

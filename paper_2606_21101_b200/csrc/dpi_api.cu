@@ -91,6 +91,11 @@ struct dpi_plan_s {
     uint32_t* tab_nvec_dev = nullptr;   // [T] 16-byte vectors per row of each table
     uint32_t* tab_col_dev = nullptr;    // [T] first output vector of each table's column block
     unsigned long long* n_bad_dev = nullptr;
+    // 64-bit offsets (dpi_plan_set_offset_type; NEXT-2): the plan then lives in these instead of `offsets`
+    bool off64 = false;
+    long long* offsets64 = nullptr;   // [G+1]
+    long long* seg_off64 = nullptr;   // [seg_cap]
+    void* agg64 = nullptr;            // [num_chunks] chunk aggregates of the two-launch 64-bit planner
     // staging for dpi_forward_host
     int32_t* stage_len = nullptr;
     void* stage_idx = nullptr;
@@ -150,13 +155,23 @@ uint32_t seg_capacity_for(const dpi_plan_t* p, int32_t K) {
 }
 
 dpi_status_t ensure_seg_capacity(dpi_plan_t* p, int32_t K) {
+    const uint64_t c_max = static_cast<uint64_t>(p->max_indices) + p->G;
+    if ((c_max + K - 1) / K + 2 >= (1ull << 31)) return fail(DPI_ERR_INVALID_ARG, "quantum K=%d gives more than 2^31 segments for max_indices=%lld", K, (long long)p->max_indices);
     const uint32_t need = seg_capacity_for(p, K);
-    if (need <= p->seg_cap && p->seg) return DPI_OK;
+    if (need <= p->seg_cap && p->seg && (!p->off64 || p->seg_off64)) return DPI_OK;
     int2* fresh = nullptr;
-    DPI_CUDA(cudaMalloc(&fresh, static_cast<size_t>(need) * sizeof(int2)));   // on failure the old buffer stays in place
+    long long* fresh64 = nullptr;
+    const uint32_t cap = std::max(need, p->seg_cap);
+    DPI_CUDA(cudaMalloc(&fresh, static_cast<size_t>(cap) * sizeof(int2)));   // on failure the old buffers stay in place
+    if (p->off64) {
+        cudaError_t e = cudaMalloc(&fresh64, static_cast<size_t>(cap) * sizeof(long long));
+        if (e != cudaSuccess) { (void)cudaFree(fresh); return cuda_fail(e, "cudaMalloc(seg_off64)"); }
+    }
     if (p->seg) (void)cudaFree(p->seg);
+    if (p->seg_off64) (void)cudaFree(p->seg_off64);
     p->seg = fresh;
-    p->seg_cap = need;
+    p->seg_off64 = fresh64;
+    p->seg_cap = cap;
     return DPI_OK;
 }
 
@@ -168,6 +183,7 @@ void free_plan(dpi_plan_t* p) {
     cudaFree(p->offsets); cudaFree(p->seg); cudaFree(p->meta); cudaFree(p->status);
     cudaFree(p->state); cudaFree(p->table_rows_dev); cudaFree(p->n_bad_dev);
     cudaFree(p->tab_nvec_dev); cudaFree(p->tab_col_dev);
+    cudaFree(p->offsets64); cudaFree(p->seg_off64); cudaFree(p->agg64);
     cudaFree(p->stage_len); cudaFree(p->stage_idx); cudaFree(p->stage_out);
     (void)cudaGetLastError();
     delete p;
@@ -267,7 +283,9 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
     LookupArgs a{};
     a.tables = c.tables;
     a.indices = static_cast<const int32_t*>(c.indices);
-    a.offsets = c.offsets ? c.offsets : p->offsets;
+    a.offsets = c.offsets ? c.offsets : (p->off64 ? reinterpret_cast<const int32_t*>(p->offsets64) : p->offsets);
+    a.off_shift = p->off64 ? 1u : 0u;
+    a.seg_off64 = p->seg_off64;
     a.seg = p->seg;
     a.meta = p->meta;
     a.out = c.out;
@@ -303,7 +321,7 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
         a.rows_per_peer = static_cast<uint32_t>(c.rows_per_peer);
     }
     const bool general = c.force_general || p->mixed_dims || p->custom_columns || a.idx_shift || a.table_major || c.weights ||
-                         c.peers || ld != p->out_width;
+                         c.peers || ld != p->out_width || p->off64;
     if (input_first) {
         if (general) return fail(DPI_ERR_UNSUPPORTED, "the input-first ablation kernel only takes the dense int32 sample-major layout");
         cudaError_t e = launch_input_first(a, static_cast<uint32_t>(p->B), p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, stream);
@@ -318,7 +336,7 @@ dpi_status_t do_lookup(const dpi_plan_t* p, const LookupCall& c, cudaStream_t st
     const bool short_bags = hint >= 1 && short_bag_rule(static_cast<uint32_t>(hint), p->G);
     // the short-bag variant also takes int64 ids (the one interface variant every framework feeds)
     const bool general_but_ids = c.force_general || p->mixed_dims || p->custom_columns || a.table_major || c.weights || c.peers ||
-                                 ld != p->out_width;
+                                 ld != p->out_width || p->off64;
     if (!general_but_ids && (p->opt[DPI_OPT_MODE] == 6 || (p->opt[DPI_OPT_MODE] == 0 && short_bags))) {
         cudaError_t e = launch_direct(a, p->dtype, p->dtype != DPI_F32 && p->out_dtype == DPI_F32, p->lanes, p->direct_grid_cap,
                                       p->opt[DPI_OPT_PDL] != 0, stream);
@@ -377,7 +395,7 @@ constexpr uint64_t kFusedDefaultMaxBags = 1u << 20;
 // capacity says bags are short on average (max_indices <= 8 * G) -- the fused kernel is correct for any bag length but
 // does not balance load across CTAs, so long-bag batches keep the planner + balanced-segment lookup.
 bool fused_eligible(const dpi_plan_t* p, const LookupCall& c) {
-    if (p->fused_chunks == 0 || p->opt[DPI_OPT_FUSED] == 2 || p->opt[DPI_OPT_MODE] != 0) return false;
+    if (p->fused_chunks == 0 || p->opt[DPI_OPT_FUSED] == 2 || p->opt[DPI_OPT_MODE] != 0 || p->off64) return false;
     if (c.force_general || p->mixed_dims || p->custom_columns || p->bag_order != DPI_BAGS_SAMPLE_MAJOR || c.weights || c.peers ||
         c.offsets || (c.out_ld && c.out_ld != p->out_width))
         return false;
@@ -392,6 +410,8 @@ dpi_status_t launch_fused_forward(dpi_plan_t* p, const int32_t* lengths_dev, con
     f.plan.num_chunks = p->fused_chunks;
     f.chunk_bags = p->fused_chunk_bags;
     f.items = (p->fused_chunk_bags + kFusedThreads - 1) / kFusedThreads;
+    f.k_shift = 32;
+    for (uint32_t b = 0; b < 31; ++b) if (static_cast<uint32_t>(p->K) == (1u << b)) f.k_shift = b;
     LookupArgs& a = f.look;
     a.tables = c.tables;
     a.indices = static_cast<const int32_t*>(c.indices);
@@ -601,6 +621,17 @@ dpi_status_t dpi_plan_build(dpi_plan_t* p, const int32_t* lengths_dev, void* str
     if (!p || !lengths_dev) return fail(DPI_ERR_INVALID_ARG, "plan/lengths_dev is NULL");
     if (reinterpret_cast<uintptr_t>(lengths_dev) & 3u) return fail(DPI_ERR_INVALID_ARG, "lengths_dev is not 4-byte aligned");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (p->off64) {
+        Plan64Args b{};
+        b.len = lengths_dev; b.offsets = p->offsets64; b.seg = p->seg; b.seg_off = p->seg_off64; b.meta = p->meta;
+        b.agg = p->agg64; b.state = p->state; b.G = p->G; b.K = static_cast<unsigned long long>(p->K); b.seg_cap = p->seg_cap;
+        b.num_tiles = p->num_tiles; b.num_chunks = p->num_chunks; b.tiles_per_chunk = p->tiles_per_chunk;
+        b.max_indices = static_cast<unsigned long long>(p->max_indices);
+        cudaError_t e64 = launch_plan64(b, s);
+        if (e64 != cudaSuccess) return cuda_fail(e64, "64-bit plan kernel launch");
+        p->built = true;
+        return DPI_OK;
+    }
     const PlanArgs a = plan_args(p, lengths_dev);
     cudaError_t e = launch_plan(a, s);
     if (e != cudaSuccess) return cuda_fail(e, "plan kernel launch");
@@ -623,7 +654,7 @@ dpi_status_t dpi_plan(const int64_t* table_rows, int32_t T, const int32_t* dims,
 dpi_status_t dpi_plan_device_views(const dpi_plan_t* p, const int32_t** offsets_dev, const int32_t** seg_dev,
                                    const int32_t** meta_dev) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
-    if (offsets_dev) *offsets_dev = p->offsets;
+    if (offsets_dev) *offsets_dev = p->off64 ? reinterpret_cast<const int32_t*>(p->offsets64) : p->offsets;
     if (seg_dev) *seg_dev = reinterpret_cast<const int32_t*>(p->seg);
     if (meta_dev) *meta_dev = p->meta;
     return DPI_OK;
@@ -646,6 +677,7 @@ dpi_status_t dpi_plan_export(const dpi_plan_t* p, int32_t* offsets_host, int32_t
                              int64_t seg_cap, int32_t* S, int64_t* N, void* stream) {
     if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
     if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
+    if (p->off64) return fail(DPI_ERR_INVALID_ARG, "the plan holds 64-bit offsets: use dpi_plan_export64");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int32_t meta[kMetaWords];
     DPI_CUDA(cudaMemcpyAsync(meta, p->meta, sizeof meta, cudaMemcpyDeviceToHost, s));
@@ -665,6 +697,71 @@ dpi_status_t dpi_plan_export(const dpi_plan_t* p, int32_t* offsets_host, int32_t
             if (seg_off_host) seg_off_host[i] = rec[i].y;
         }
     }
+    DPI_CUDA(cudaStreamSynchronize(s));
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_set_offset_type(dpi_plan_t* p, dpi_offset_type_t type, int64_t max_indices) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (type != DPI_OFF_I32 && type != DPI_OFF_I64) return fail(DPI_ERR_INVALID_ARG, "unknown offset type %d", (int)type);
+    if (max_indices == 0) max_indices = p->max_indices;
+    const int64_t limit = type == DPI_OFF_I64 ? (1ll << 40) : (1ll << 31);
+    if (max_indices < 0 || max_indices >= limit) return fail(DPI_ERR_INVALID_ARG, "max_indices=%lld outside [0, 2^%d)", (long long)max_indices, type == DPI_OFF_I64 ? 40 : 31);
+    if (type == DPI_OFF_I32 && static_cast<int64_t>(p->G) + max_indices >= (1ll << 32) - 16) return fail(DPI_ERR_INVALID_ARG, "B*T + max_indices too large for 32-bit offsets");
+    p->built = false;
+    const bool was64 = p->off64;
+    const int64_t was_max = p->max_indices;
+    p->off64 = type == DPI_OFF_I64;
+    p->max_indices = max_indices;
+    dpi_status_t st = DPI_OK;
+    if (p->off64) {
+        if (!p->offsets64) {
+            cudaError_t e = cudaMalloc(&p->offsets64, (static_cast<size_t>(p->G) + 1) * sizeof(long long));
+            if (e != cudaSuccess) st = cuda_fail(e, "cudaMalloc(offsets64)");
+        }
+        if (st == DPI_OK && !p->agg64) {
+            cudaError_t e = cudaMalloc(&p->agg64, static_cast<size_t>(kMaxChunks) * 32);
+            if (e != cudaSuccess) st = cuda_fail(e, "cudaMalloc(agg64)");
+        }
+    }
+    if (st == DPI_OK) {
+        if (!p->K_user) p->K = default_quantum(p);
+        st = ensure_seg_capacity(p, p->K);
+    }
+    if (st != DPI_OK) {   // the plan keeps its previous offset type and capacity
+        p->off64 = was64;
+        p->max_indices = was_max;
+        return st;
+    }
+    if (p->stage_idx) { (void)cudaFree(p->stage_idx); p->stage_idx = nullptr; p->stage_idx_bytes = 0; }
+    free_pipeline(p);
+    prepare_launches(p);
+    return DPI_OK;
+}
+
+dpi_status_t dpi_plan_export64(const dpi_plan_t* p, int64_t* offsets_host, int32_t* seg_bag_host, int64_t* seg_off_host,
+                               int64_t seg_cap, int64_t* S, int64_t* N, void* stream) {
+    if (!p) return fail(DPI_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->built) return fail(DPI_ERR_INVALID_ARG, "plan has not been built");
+    if (!p->off64) return fail(DPI_ERR_INVALID_ARG, "the plan holds 32-bit offsets: use dpi_plan_export");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int32_t meta[kMetaWords];
+    DPI_CUDA(cudaMemcpyAsync(meta, p->meta, sizeof meta, cudaMemcpyDeviceToHost, s));
+    DPI_CUDA(cudaStreamSynchronize(s));
+    const int64_t n_total = (static_cast<int64_t>(meta[META_N_HI]) << 32) | static_cast<uint32_t>(meta[META_N]);
+    if (meta[META_OVERFLOW]) return fail(DPI_ERR_INVALID_ARG, "batch has N=%lld > max_indices=%lld (plan capacity exceeded)", (long long)n_total, (long long)p->max_indices);
+    if (S) *S = meta[META_S];
+    if (N) *N = n_total;
+    if (offsets_host) DPI_CUDA(cudaMemcpyAsync(offsets_host, p->offsets64, (static_cast<size_t>(p->G) + 1) * sizeof(long long), cudaMemcpyDeviceToHost, s));
+    const size_t n = static_cast<size_t>(meta[META_S]) + 1;
+    if ((seg_bag_host || seg_off_host) && seg_cap < static_cast<int64_t>(n)) return fail(DPI_ERR_INVALID_ARG, "seg_cap=%lld < S+1=%zu", (long long)seg_cap, n);
+    if (seg_bag_host) {
+        std::vector<int2> rec(n);
+        DPI_CUDA(cudaMemcpyAsync(rec.data(), p->seg, n * sizeof(int2), cudaMemcpyDeviceToHost, s));
+        DPI_CUDA(cudaStreamSynchronize(s));
+        for (size_t i = 0; i < n; ++i) seg_bag_host[i] = rec[i].x;
+    }
+    if (seg_off_host) DPI_CUDA(cudaMemcpyAsync(seg_off_host, p->seg_off64, n * sizeof(long long), cudaMemcpyDeviceToHost, s));
     DPI_CUDA(cudaStreamSynchronize(s));
     return DPI_OK;
 }
@@ -906,6 +1003,7 @@ dpi_status_t dpi_forward_host(dpi_plan_t* p, const void* const* table_ptrs_dev, 
                               const void* indices_host, int64_t n_indices, const uint8_t* pooling, void* out_host,
                               void* stream) {
     if (!p || !table_ptrs_dev || !lengths_host || !out_host) return fail(DPI_ERR_INVALID_ARG, "NULL argument");
+    if (p->off64) return fail(DPI_ERR_UNSUPPORTED, "dpi_forward_host covers 32-bit offsets only (N < 2^31 per call)");
     if (n_indices < 0 || n_indices > p->max_indices) return fail(DPI_ERR_INVALID_ARG, "n_indices=%lld outside [0, max_indices=%lld]", (long long)n_indices, (long long)p->max_indices);
     if (n_indices > 0 && !indices_host) return fail(DPI_ERR_INVALID_ARG, "indices_host is NULL");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -1020,7 +1118,8 @@ dpi_status_t dpi_check_indices(const dpi_plan_t* p, const void* indices_dev, int
     DPI_CUDA(cudaMemsetAsync(p->n_bad_dev, 0, 2 * sizeof(unsigned long long), s));
     CheckArgs a{};
     a.indices = indices_dev;
-    a.offsets = p->offsets;
+    a.offsets = p->off64 ? reinterpret_cast<const int32_t*>(p->offsets64) : p->offsets;
+    a.off64 = p->off64;
     a.table_rows = p->table_rows_dev;
     a.n_bad = p->n_bad_dev;
     a.max_bag = p->opt[DPI_OPT_MAX_BAG_HINT];

@@ -14,8 +14,10 @@
 
 namespace dpi {
 
-constexpr int kMetaWords = 8;  // meta_dev layout: {S, N, C[G] (low 32), overflow, K, G, min_len, max_len}
-enum MetaSlot { META_S = 0, META_N = 1, META_C = 2, META_OVERFLOW = 3, META_K = 4, META_G = 5, META_MINLEN = 6, META_MAXLEN = 7 };
+constexpr int kMetaWords = 12;  // meta_dev layout: {S, N (low 32), C[G] (low 32), overflow, K, G, min_len, max_len, N (high 32),
+                                // C[G] (high 32), -, -}; the high words are written by the 64-bit planner only (else 0)
+enum MetaSlot { META_S = 0, META_N = 1, META_C = 2, META_OVERFLOW = 3, META_K = 4, META_G = 5, META_MINLEN = 6, META_MAXLEN = 7,
+                META_N_HI = 8, META_C_HI = 9 };
 // The device picks the a3 variant from a1's max_len: bags of 2..kShortBagMax entries run the short-bag
 // body (one lane group per bag); exactly one entry per bag runs it up to kShortOnehotMaxBags bags, beyond that the
 // balanced-segment kernel's row-copy path with its index prefetch pipeline is faster (measured).
@@ -62,6 +64,23 @@ struct PlanArgs {
 
 cudaError_t launch_plan(const PlanArgs& a, cudaStream_t stream);
 
+// 64-bit offsets (plan64_kernels.cu; NEXT-2): two stream-ordered launches, no status records
+struct Plan64Args {
+    const int32_t* __restrict__ len;   // [G]
+    long long* __restrict__ offsets;   // [G+1] int64
+    int2* __restrict__ seg;            // [seg_cap] {seg_bag[s], low 32 bits of seg_off[s]}
+    long long* __restrict__ seg_off;   // [seg_cap] int64
+    int32_t* __restrict__ meta;        // [kMetaWords]
+    void* agg;                         // [num_chunks] 32-byte chunk aggregates
+    unsigned int* state;               // planner state of the plan (sticky overflow counter)
+    uint32_t G;
+    unsigned long long K;
+    unsigned long long seg_cap;
+    uint32_t num_tiles, num_chunks, tiles_per_chunk;
+    unsigned long long max_indices;
+};
+cudaError_t launch_plan64(const Plan64Args& a, cudaStream_t stream);
+
 // ---- a1 + a2 + a3 in one launch (forward_fused.cu) ----
 constexpr int kFusedThreads = 256;
 constexpr int kFusedItems = 8;                              // bags per thread, held in registers across the look-back
@@ -72,7 +91,7 @@ constexpr int kStatusRecords = kFusedMaxChunks > kMaxChunks ? kFusedMaxChunks : 
 
 struct CheckArgs {
     const void* __restrict__ indices;        // int32 or int64 (idx64)
-    const int32_t* __restrict__ offsets;
+    const int32_t* __restrict__ offsets;     // int32[G+1], or int64[G+1] when off64
     const int64_t* __restrict__ table_rows;  // device [T]
     unsigned long long* n_bad;               // [0] indices out of range, [1] bags longer than max_bag (when max_bag > 0)
     int32_t max_bag;                         // DPI_OPT_MAX_BAG_HINT, 0 = no promise to check
@@ -81,6 +100,7 @@ struct CheckArgs {
     uint32_t B;
     bool idx64;
     bool table_major;
+    bool off64;
 };
 cudaError_t launch_check_indices(const CheckArgs& a, cudaStream_t stream);
 
@@ -107,6 +127,8 @@ struct LookupArgs {
     uint32_t B;
     uint32_t idx_shift;                      // 0: int32 ids, 1: int64 ids (indices then points at the low words)
     uint32_t table_major;                    // 0: g = b*T + t, 1: g = t*B + b
+    uint32_t off_shift;                      // 0: int32 offsets; 1: int64 offsets (offsets then points at the low words; GEN only)
+    const long long* __restrict__ seg_off64; // off_shift = 1: 64-bit first entry of every task (seg[s].y holds its low word)
     PoolMask pool;
 };
 
@@ -117,6 +139,7 @@ struct FusedArgs {
     uint32_t chunk_bags;                 // <= kFusedMaxChunkBags
     uint32_t items;                      // bags per thread = ceil(chunk_bags / kFusedThreads)
     uint32_t any_mean;                   // some table is mean-pooled (else the pooling mask is never consulted)
+    uint32_t k_shift;                    // log2(K) when the quantum is a power of two, else 32 (divide)
 };
 cudaError_t launch_fused(const FusedArgs& a, int dtype, bool out32, int lanes, bool pdl, cudaStream_t stream);
 int fused_occupancy(int dtype, bool out32, int lanes, uint32_t T);   // resident CTAs per SM (0: no instantiation)

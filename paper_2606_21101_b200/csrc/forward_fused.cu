@@ -111,7 +111,10 @@ __device__ __forceinline__ void pool_lane_groups(const LookupArgs& la, const cha
     }
 }
 
-template <class Tr, int W, bool OUT32>
+// ITEMS = bags per thread the scan phases are compiled for (1, 2, 4 or 8 >= the run-time count): with one launch covering
+// 64 ... 2048 bags per CTA, code unrolled for 8 bags per thread cost a c2-sized batch (1 bag per thread) 700 instructions per
+// warp before the first row was loaded.
+template <class Tr, int W, bool OUT32, int ITEMS>
 __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fused_forward_kernel(const FusedArgs a) {
     constexpr int P = 32 / W;
     constexpr int NW = kFusedThreads / 32;         // warps per CTA
@@ -128,7 +131,7 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
     const PlanArgs& pa = a.plan;
     const LookupArgs& la = a.look;
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t I = a.items;                    // bags per thread, <= kFusedItems
+    const uint32_t I = ITEMS == 1 ? 1u : a.items;  // bags per thread, <= ITEMS
 
     griddep_wait();  // PDL: nothing is read before the preceding grid (e.g. the previous step) has completed
     if (tid == 0) {
@@ -136,13 +139,13 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
         s_bcast[1] = *reinterpret_cast<volatile unsigned int*>(pa.state + kStateEpoch);
     }
     // ---- A: the lengths of this thread's I consecutive bags, issued before the ticket is back ----
-    uint32_t v[kFusedItems];
+    uint32_t v[ITEMS];
     uint32_t chunk = blockIdx.x;
     auto load_lengths = [&](uint32_t c) {
         const uint32_t c_lo = c * a.chunk_bags;
         const uint32_t c_n = min(pa.G - c_lo, a.chunk_bags);
 #pragma unroll
-        for (int i = 0; i < kFusedItems; ++i) {
+        for (int i = 0; i < ITEMS; ++i) {
             const uint32_t local = tid * I + i;
             v[i] = (static_cast<uint32_t>(i) < I && local < c_n) ? static_cast<uint32_t>(__ldg(pa.len + c_lo + local)) : 0u;
         }
@@ -161,7 +164,7 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
     // ---- B: thread sums, warp scan, CTA totals; publish ----
     uint32_t t_len = 0, t_cost = 0, t_lo = 0xffffffffu, t_hi = 0u;
 #pragma unroll
-    for (int i = 0; i < kFusedItems; ++i) {
+    for (int i = 0; i < ITEMS; ++i) {
         const bool ok = static_cast<uint32_t>(i) < I && tid * I + i < nb;
         t_len += v[i];
         t_cost += ok ? max(v[i], 1u) : 0u;
@@ -223,7 +226,7 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
         uint32_t off = pre_len + w_len + i_len - t_len;       // offsets[first bag of this thread]
         uint32_t c = pre_cost + w_cost + i_cost - t_cost;     // C[first bag of this thread]
 #pragma unroll
-        for (int i = 0; i < kFusedItems; ++i) {
+        for (int i = 0; i < ITEMS; ++i) {
             const uint32_t local = tid * I + i;
             if (static_cast<uint32_t>(i) < I && local < nb) {
                 const uint32_t g = g_lo + local, l = v[i], cost = max(l, 1u);
@@ -232,7 +235,7 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
                 s_off[local] = static_cast<int>(off);
                 if (g == 0) pa.seg[0] = make_int2(0, 0);
                 const uint32_t c1 = c + cost;
-                uint32_t s = c / pa.K;
+                uint32_t s = a.k_shift < 32u ? c >> a.k_shift : c / pa.K;   // the default quanta are powers of two
                 unsigned long long next_boundary = static_cast<unsigned long long>(s + 1) * pa.K;
                 while (c1 >= next_boundary) {
                     ++s;
@@ -330,31 +333,38 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
     }
 }
 
-template <class Tr, bool OUT32, class F>
+template <class Tr, bool OUT32, int ITEMS, class F>
 auto for_lanes(int lanes, F&& f) {
     switch (lanes) {
-        case 1: return f(fused_forward_kernel<Tr, 1, OUT32>);
-        case 2: return f(fused_forward_kernel<Tr, 2, OUT32>);
-        case 4: return f(fused_forward_kernel<Tr, 4, OUT32>);
-        case 8: return f(fused_forward_kernel<Tr, 8, OUT32>);
-        case 16: return f(fused_forward_kernel<Tr, 16, OUT32>);
-        case 32: return f(fused_forward_kernel<Tr, 32, OUT32>);
+        case 1: return f(fused_forward_kernel<Tr, 1, OUT32, ITEMS>);
+        case 2: return f(fused_forward_kernel<Tr, 2, OUT32, ITEMS>);
+        case 4: return f(fused_forward_kernel<Tr, 4, OUT32, ITEMS>);
+        case 8: return f(fused_forward_kernel<Tr, 8, OUT32, ITEMS>);
+        case 16: return f(fused_forward_kernel<Tr, 16, OUT32, ITEMS>);
+        case 32: return f(fused_forward_kernel<Tr, 32, OUT32, ITEMS>);
         default: return f(static_cast<void (*)(const FusedArgs)>(nullptr));
     }
 }
+template <class Tr, bool OUT32, class F>
+auto for_items(uint32_t items, int lanes, F&& f) {
+    if (items <= 1) return for_lanes<Tr, OUT32, 1>(lanes, f);
+    if (items <= 2) return for_lanes<Tr, OUT32, 2>(lanes, f);
+    if (items <= 4) return for_lanes<Tr, OUT32, 4>(lanes, f);
+    return for_lanes<Tr, OUT32, kFusedItems>(lanes, f);
+}
 template <class F>
-auto for_kernel(int dtype, bool out32, int lanes, F&& f) {
+auto for_kernel(int dtype, bool out32, int lanes, uint32_t items, F&& f) {
     switch (dtype) {
-        case DPI_F32: return for_lanes<F32Traits, false>(lanes, f);
-        case DPI_F16: return out32 ? for_lanes<F16Traits, true>(lanes, f) : for_lanes<F16Traits, false>(lanes, f);
-        default: return out32 ? for_lanes<BF16Traits, true>(lanes, f) : for_lanes<BF16Traits, false>(lanes, f);
+        case DPI_F32: return for_items<F32Traits, false>(items, lanes, f);
+        case DPI_F16: return out32 ? for_items<F16Traits, true>(items, lanes, f) : for_items<F16Traits, false>(items, lanes, f);
+        default: return out32 ? for_items<BF16Traits, true>(items, lanes, f) : for_items<BF16Traits, false>(items, lanes, f);
     }
 }
 
 }  // namespace
 
 int fused_occupancy(int dtype, bool out32, int lanes, uint32_t T) {
-    return for_kernel(dtype, out32, lanes, [&](void (*k)(const FusedArgs)) -> int {
+    return for_kernel(dtype, out32, lanes, kFusedItems, [&](void (*k)(const FusedArgs)) -> int {
         int occ = 0;
         if (!k || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kFusedThreads, static_cast<size_t>(T) * sizeof(const char*)) != cudaSuccess) {
             (void)cudaGetLastError();
@@ -365,7 +375,7 @@ int fused_occupancy(int dtype, bool out32, int lanes, uint32_t T) {
 }
 
 cudaError_t launch_fused(const FusedArgs& a, int dtype, bool out32, int lanes, bool pdl, cudaStream_t stream) {
-    return for_kernel(dtype, out32, lanes, [&](void (*k)(const FusedArgs)) -> cudaError_t {
+    return for_kernel(dtype, out32, lanes, a.items, [&](void (*k)(const FusedArgs)) -> cudaError_t {
         if (!k) return cudaErrorInvalidValue;
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(a.plan.num_chunks);

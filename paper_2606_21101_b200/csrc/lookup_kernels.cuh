@@ -291,6 +291,21 @@ __device__ __forceinline__ void short_bag_body(const LookupArgs& a, const char* 
     }
 }
 
+// The offsets of a task as the kernel reads them. Plain layout: an int array indexed by bag id, values = absolute entry
+// positions. General variant with int64 offsets (NEXT-2, DESIGN.md 11.2 V6): only the LOW words are read (stride 2) and every
+// value is rebased to the task's first entry -- inside a task all positions are < 2^32 apart, so the difference of the low
+// words is exact -- and the 64-bit part enters once per task, in the base pointer of its index run (seg_off64).
+template <bool GEN>
+struct OffView {
+    const int* p;
+    int sh;            // GEN: 1 when p walks the low words of int64 offsets
+    uint32_t rebase;   // GEN: low word of the task's first entry when positions are task-relative, else 0
+    __device__ __forceinline__ int operator[](ptrdiff_t g) const {
+        if constexpr (GEN) return static_cast<int>(static_cast<uint32_t>(p[g << sh]) - rebase);
+        else return p[g];
+    }
+};
+
 // Per-table record of the general (GEN) variant, staged in shared memory.
 struct TableInfo {
     const char* base;
@@ -449,19 +464,26 @@ __global__ void __launch_bounds__(kLookupMaxThreads, lookup_min_ctas<Tr, U, GEN>
     auto is_mean = [&](uint32_t t) -> bool { return (a.pool.w[t >> 5] >> (t & 31)) & 1u; };
 
     // Stage offsets[g_lo..g_hi] and indices[e_lo..e_hi) (and weights) of one task into buffer `b` (if they fit).
-    auto stage = [&](const int2 r_lo, const int2 r_hi, int b) {
-        const int nb1 = r_hi.x - r_lo.x + 1, ne = r_hi.y - r_lo.y;
-        if (r_hi.x > r_lo.x && nb1 <= kStageOff && ne <= kStageIdx) {
+    const int osh = GEN ? static_cast<int>(a.off_shift) : 0;   // 1: int64 offsets, the low words are read
+    // first entry of task s as a 64-bit position: seg[s].y, or seg_off64[s] when the offsets are 64-bit
+    auto task_base = [&](uint32_t s_, const int2 r_lo) -> long long {
+        if constexpr (GEN) { if (osh) return a.seg_off64[s_]; }
+        return static_cast<long long>(r_lo.y);
+    };
+    auto stage = [&](const int2 r_lo, const int2 r_hi, long long e_base, int b) {
+        const int nb1 = r_hi.x - r_lo.x + 1;
+        const uint32_t ne = static_cast<uint32_t>(r_hi.y) - static_cast<uint32_t>(r_lo.y);   // low words: exact inside a task
+        if (r_hi.x > r_lo.x && nb1 <= kStageOff && ne <= static_cast<uint32_t>(kStageIdx)) {
             int* ib = s_warp + b * stage_idx;
             int* ob = s_off + b * kStageOff;
-            const int nw = ne << ish;
-            const int* src = a.indices + (static_cast<size_t>(r_lo.y) << ish);
+            const int nw = static_cast<int>(ne) << ish;
+            const int* src = a.indices + (static_cast<size_t>(e_base) << ish);
             for (int i = lane; i < nw; i += 32) cp_async4(ib + i, src + i);
-            for (int i = lane; i < nb1; i += 32) cp_async4(ob + i, a.offsets + r_lo.x + i);
+            for (int i = lane; i < nb1; i += 32) cp_async4(ob + i, a.offsets + (static_cast<size_t>(r_lo.x + i) << osh));
             if constexpr (GEN) {
                 if (a.weights) {
                     float* wb = s_wgt + b * kStageIdx;
-                    for (int i = lane; i < ne; i += 32) cp_async4(wb + i, a.weights + r_lo.y + i);
+                    for (int i = lane; i < static_cast<int>(ne); i += 32) cp_async4(wb + i, a.weights + e_base + i);
                 }
             }
         }
@@ -474,7 +496,8 @@ __global__ void __launch_bounds__(kLookupMaxThreads, lookup_min_ctas<Tr, U, GEN>
     int2 nxt_lo = cur_lo, nxt_hi = cur_hi;
     bool have_next = s + n_warps < S;
     if (have_next) { nxt_lo = ld_plan(a.seg + s + n_warps); nxt_hi = ld_plan(a.seg + s + n_warps + 1); }
-    stage(cur_lo, cur_hi, 0);
+    long long cur_base = task_base(s, cur_lo);
+    stage(cur_lo, cur_hi, cur_base, 0);
     int buf = 0;
 
     for (;;) {
@@ -483,8 +506,10 @@ __global__ void __launch_bounds__(kLookupMaxThreads, lookup_min_ctas<Tr, U, GEN>
         const bool have_next2 = s2 < S;
         int2 n2_lo = nxt_lo, n2_hi = nxt_hi;
         if (have_next2) { n2_lo = ld_plan(a.seg + s2); n2_hi = ld_plan(a.seg + s2 + 1); }
+        long long nxt_base = 0;
         if (have_next) {
-            stage(nxt_lo, nxt_hi, buf ^ 1);
+            nxt_base = task_base(s + n_warps, nxt_lo);
+            stage(nxt_lo, nxt_hi, nxt_base, buf ^ 1);
             cp_async_wait<1>();
         } else {
             cp_async_wait<0>();
@@ -494,15 +519,20 @@ __global__ void __launch_bounds__(kLookupMaxThreads, lookup_min_ctas<Tr, U, GEN>
         const uint32_t g_lo = cur_lo.x, g_hi = cur_hi.x;
         if (g_lo < g_hi) {  // a long bag spanning several quanta leaves empty tasks behind it
             const uint32_t nb = g_hi - g_lo;
-            const int e_lo = cur_lo.y, e_hi = cur_hi.y;
-            const uint32_t ne = static_cast<uint32_t>(e_hi - e_lo);
+            const uint32_t ne = static_cast<uint32_t>(cur_hi.y) - static_cast<uint32_t>(cur_lo.y);
             const bool staged = (nb + 1 <= static_cast<uint32_t>(kStageOff)) && (ne <= static_cast<uint32_t>(kStageIdx));
-            // generic pointers indexed by ABSOLUTE entry / bag id: staged smem or the global arrays
-            const int* ip = staged ? (s_warp + buf * stage_idx - (static_cast<ptrdiff_t>(e_lo) << ish)) : a.indices;
-            const int* op = staged ? (s_off + buf * kStageOff - static_cast<int>(g_lo)) : a.offsets;
+            // entry positions are absolute (int32 offsets) or relative to the task's first entry (int64 offsets: osh = 1)
+            const int e_lo = osh ? 0 : cur_lo.y;
+            // generic pointers indexed by entry position / ABSOLUTE bag id: staged smem or the global arrays
+            const int* ip = staged ? (s_warp + buf * stage_idx - (static_cast<ptrdiff_t>(e_lo) << ish))
+                                   : (osh ? a.indices + (static_cast<size_t>(cur_base) << ish) : a.indices);
+            OffView<GEN> op;
+            op.p = staged ? (s_off + buf * kStageOff - static_cast<int>(g_lo)) : a.offsets;
+            op.sh = staged ? 0 : osh;
+            op.rebase = osh ? static_cast<uint32_t>(cur_lo.y) : 0u;
             const float* wp = nullptr;
             if constexpr (GEN) {
-                if (a.weights) wp = staged ? (s_wgt + buf * kStageIdx - e_lo) : a.weights;
+                if (a.weights) wp = staged ? (s_wgt + buf * kStageIdx - e_lo) : (osh ? a.weights + cur_base : a.weights);
             }
 
             bool onehot = false;
@@ -702,6 +732,7 @@ __global__ void __launch_bounds__(kLookupMaxThreads, lookup_min_ctas<Tr, U, GEN>
         __syncwarp();  // every lane is done with buffer `buf` before the next iteration refills it
         s += n_warps;
         cur_lo = nxt_lo; cur_hi = nxt_hi;
+        cur_base = nxt_base;
         nxt_lo = n2_lo; nxt_hi = n2_hi;
         have_next = have_next2;
         buf ^= 1;

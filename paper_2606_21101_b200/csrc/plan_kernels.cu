@@ -299,9 +299,10 @@ __global__ void __launch_bounds__(256) check_indices_kernel(const CheckArgs a) {
     unsigned long long bad = 0, too_long = 0;
     for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < a.G; g += gridDim.x * blockDim.x) {
         const long long rows = a.table_rows[a.table_major ? g / a.B : g % a.T];
-        const int lo = a.offsets[g], hi = a.offsets[g + 1];
+        const long long lo = a.off64 ? reinterpret_cast<const long long*>(a.offsets)[g] : a.offsets[g];
+        const long long hi = a.off64 ? reinterpret_cast<const long long*>(a.offsets)[g + 1] : a.offsets[g + 1];
         too_long += (a.max_bag > 0 && hi - lo > a.max_bag) ? 1ull : 0ull;
-        for (int j = lo; j < hi; ++j) {
+        for (long long j = lo; j < hi; ++j) {
             const long long r = a.idx64 ? static_cast<const long long*>(a.indices)[j]
                                         : static_cast<long long>(static_cast<const int*>(a.indices)[j]);
             bad += (r < 0 || r >= rows) ? 1ull : 0ull;

@@ -31,7 +31,7 @@ def _problem(seed, dims, rows, B, lengths_spec, index_dist=("uniform",)):
 
 
 def _run(dims, rows, B, dtype, lengths_spec, *, seed=3, out_dtype=None, table_major=False, idx64=False, weighted=False,
-         pooling=None, out_ld=0, K=0, force_general=False, mode=0):
+         pooling=None, out_ld=0, K=0, force_general=False, mode=0, off64=False, explicit_offsets=False):
     T = len(dims)
     out_dtype = out_dtype or dtype
     lengths, indices = _problem(seed, dims, rows, B, lengths_spec)
@@ -55,6 +55,8 @@ def _run(dims, rows, B, dtype, lengths_spec, *, seed=3, out_dtype=None, table_ma
         plan.set_out_dtype(W.DTYPE_CODE[out_dtype])
     plan.set_layout(binding.BAGS_TABLE_MAJOR if table_major else binding.BAGS_SAMPLE_MAJOR,
                     binding.IDX_I64 if idx64 else binding.IDX_I32)
+    if off64:
+        plan.set_offset_type(binding.OFF_I64)
     if K:
         plan.set_quantum(K)
     plan.set_option(binding.OPT_MODE, mode)
@@ -66,11 +68,22 @@ def _run(dims, rows, B, dtype, lengths_spec, *, seed=3, out_dtype=None, table_ma
     wgt_dev = torch.from_numpy(wgt).cuda() if weighted and wgt.size else (torch.zeros(1, device="cuda") if weighted else None)
     plan.build(ln_dev)
     assert plan.check_indices(idx_dev) == 0
+    off_dev = None
+    if off64:   # the plan itself: bit-exact against the 64-bit oracle plan
+        off, seg, S, N, seg_off = plan.export64()
+        o_off, o_seg, o_S, o_seg_off = oracle.plan64(ln, plan.info()["K"])
+        assert N == int(np.asarray(ln, np.int64).sum()) and S == o_S
+        assert np.array_equal(off, o_off) and np.array_equal(seg, o_seg) and np.array_equal(seg_off, o_seg_off)
+        assert plan.stats() == oracle.plan_stats(ln)
+        with pytest.raises(binding.DpiError):
+            plan.export()
+        if explicit_offsets:
+            off_dev = torch.from_numpy(o_off).cuda()
     width = int(np.sum(dims))
     assert plan.plan_out_width() == width
     ld = out_ld or width
     out = torch.full((B, ld), float("nan"), dtype=TORCH_OUT[out_dtype], device="cuda")
-    plan.lookup_ex(ptrs, idx_dev, out, pooling=pooling, weights_dev=wgt_dev, out_ld=out_ld,
+    plan.lookup_ex(ptrs, idx_dev, out, pooling=pooling, weights_dev=wgt_dev, out_ld=out_ld, offsets_dev=off_dev,
                    flags=binding.LOOKUP_FORCE_GENERAL if force_general else 0)
     torch.cuda.synchronize()
     got_full = harness.out_to_f64(out)
@@ -261,3 +274,93 @@ def test_int64_ids_through_the_short_bag_variant(dtype, out, lengths):
     D = 16 if dtype == "f32" else 32
     _run([D] * 7, [1000, 50, 7, 3000, 1, 640, 99], 333, dtype, lengths, out_dtype=out, idx64=True, mode=6,
          pooling=[0, 1, 0, 1, 1, 0, 1])
+
+
+# --------------------------------------------------------------------------------------------------
+# NEXT-2 completion: 64-bit offsets (dpi_plan_set_offset_type; DESIGN.md 11.2 V6)
+# --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lengths", LENGTHS + [("uniform", 0, 300)])
+@pytest.mark.parametrize("dtype,out", [("f32", None), ("f16", None), ("bf16", "f32")])
+@pytest.mark.parametrize("K", [0, 7, 1000])
+def test_64bit_offsets_plan_and_lookup_match_the_oracle(dtype, out, lengths, K):
+    """Same inputs as the 32-bit tests, the plan kept in int64: offsets / seg_off / S bit-exact against oracle.plan64, the block
+    against the oracle; staged tasks, tasks too large for the staging buffers (U{0..300} bags at K = 1000) and K = 7."""
+    D = 16 if dtype == "f32" else 32
+    _run([D] * 5, [1000, 17, 4000, 1, 250], 333, dtype, lengths, out_dtype=out, off64=True, K=K, pooling=[0, 1, 0, 1, 1])
+
+
+def test_64bit_offsets_with_every_other_variant_and_through_dpi_forward():
+    dims, rows = [16, 8, 32, 8, 24], [50, 7, 400, 90, 3]
+    _run(dims, rows, 257, "f32", ("uniform", 0, 9), off64=True, idx64=True, weighted=True, explicit_offsets=True)
+    _run(dims, rows, 129, "bf16", ("poisson", 20.0, 100, 0.05), out_dtype="f32", off64=True, table_major=True, out_ld=128,
+         pooling=[1, 0, 1, 0, 1])
+    _run([32] * 4, rows[:4], 64, "f16", ("const", 0), off64=True)          # all bags empty
+    _run([16], [9], 1, "f32", ("const", 5000), off64=True, K=32)            # one long bag across many quanta
+    # dpi_forward on a 64-bit plan = 64-bit planner (two launches) + general lookup; dpi_forward_host refuses
+    cfg = W.Config("f64", 3, (100, 20, 7), 16, "f32", 50, ("uniform", 0, 6), ("uniform",), "half", 5)
+    rows3 = cfg.table_rows()
+    host_tables = [W.full_table_storage(cfg, t, int(rows3[t])) for t in range(cfg.T)]
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, rows3, None)
+    db = harness.upload_batch(batch)
+    plan = harness.make_plan(cfg, rows3, max(batch.N, 1))
+    plan.set_offset_type(binding.OFF_I64, 1 << 33)
+    out = harness.new_output(cfg, fill_nan=True)
+    before = binding.launch_count()
+    plan.forward(db.lengths, dt.ptrs, db.indices, out, pooling=cfg.pooling_modes())
+    assert binding.launch_count() - before == 3
+    torch.cuda.synchronize()
+    ref = oracle.lookup_general(host_tables, oracle.F32, cfg.B, batch.indices, host_offsets(batch.lengths).astype(np.int64),
+                                cfg.pooling_modes())
+    assert_outputs_match_general(harness.out_to_f64(out), ref, batch.lengths.reshape(cfg.B, cfg.T), [cfg.D] * cfg.T, "f32", "f32")
+    with pytest.raises(binding.DpiError) as e:
+        plan.forward_host(dt.ptrs, torch.from_numpy(batch.lengths), torch.from_numpy(batch.indices),
+                          torch.empty((cfg.B, cfg.T * cfg.D)))
+    assert e.value.status == 2
+    plan.set_offset_type(binding.OFF_I32, max(batch.N, 1))   # and back: the 32-bit single-launch planner again
+    plan.build(db.lengths)
+    assert plan.export()[3] == batch.N
+    plan.destroy()
+
+
+def test_64bit_offsets_with_more_than_2_pow_31_index_entries():
+    """N = 2^31 + 2^18 entries in one batch (int32 ids: 8.6 GB on the device): 8192 bags of 262 176 entries over two tiny
+    tables of 16-byte rows. Offsets beyond 2^31 must be exact (plan vs closed form and vs oracle.plan64) and the pooled
+    block must match the oracle, which walks all 2.1e9 entries once."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 24 << 30:
+        pytest.skip("needs 24 GB of free device memory")
+    B, T, L = 4096, 2, 262176
+    G = B * T
+    N = G * L
+    assert N > (1 << 31)
+    rows = [1000, 37]
+    rng = np.random.default_rng(7)
+    lengths = np.full(G, L, np.int32)
+    lengths[5] -= 3; lengths[6] += 3; lengths[G - 1] -= 1; lengths[0] += 1           # not all equal
+    block = rng.integers(0, 37, size=1 << 20).astype(np.int32)                        # valid for either table
+    idx = np.tile(block, N // block.size + 1)[:N]
+    tables = [(rng.integers(-8, 9, size=(r, 4)) / 64.0).astype(np.float32) for r in rows]   # sums stay exact in fp32
+    off = np.concatenate(([0], np.cumsum(lengths.astype(np.int64))))
+    plan = binding.Plan(rows, np.asarray([4, 4], np.int32), 0, B, 1)
+    plan.set_offset_type(binding.OFF_I64, N)
+    dev_tables, ptrs = harness.tables_from_host_mixed(tables, "f32")
+    ln_dev = torch.from_numpy(lengths).cuda()
+    idx_dev = torch.from_numpy(idx).cuda()
+    plan.build(ln_dev)
+    g_off, g_seg, S, g_N, g_seg_off = plan.export64()
+    assert g_N == N and np.array_equal(g_off, off)
+    o_off, o_seg, o_S, o_seg_off = oracle.plan64(lengths, plan.info()["K"])
+    assert S == o_S and np.array_equal(g_seg, o_seg) and np.array_equal(g_seg_off, o_seg_off)
+    assert plan.check_indices(idx_dev) == 0
+    out = torch.full((B, 8), float("nan"), dtype=torch.float32, device="cuda")
+    pooling = np.array([0, 1], np.uint8)
+    plan.lookup_ex(ptrs, idx_dev, out, pooling=pooling)
+    torch.cuda.synchronize()
+    got = harness.out_to_f64(out)
+    del idx_dev
+    ref = oracle.lookup_general(tables, oracle.F32, B, idx, off, pooling)
+    # multiples of 1/64 with |sum| < 2^18 * 1/8: every partial sum is exactly representable in fp32 -> sum pooling exact
+    assert np.array_equal(got[:, :4], ref[:, :4])
+    assert np.allclose(got[:, 4:], ref[:, 4:], rtol=1e-6, atol=1e-7)
+    plan.destroy()
