@@ -47,6 +47,22 @@ dpi_status_t dpi_fm_interaction(const void* x_dev, dpi_dtype_t dtype, int32_t B,
                                 float* y_dev, float* v_dev, void* stream);
 
 /*
+ * dpi_forward_fm -- the lookup and its first non-GEMM consumer as one operator ("we combine all neighbouring
+ * non-GEMM operators into a single operator"; the embedding lookup is itself non-GEMM and DeepFM's FM reads what it writes,
+ * PAPER.md:186): a1 + a2 + a3 exactly as dpi_forward (out_dev receives the [B, T*D] block, the plan is left built) PLUS the
+ * FM second-order term of every sample, y_dev fp32[B] and / or v_dev fp32[B, D] as in dpi_fm_interaction.
+ * For small / short-bag batches (the dpi_forward rule, DPI_OPT_FUSED) with table-dtype output this is ONE launch: chunks of
+ * the fused forward kernel are whole samples, and the CTA that pooled a sample's T bags forms its FM term from the vectors
+ * it has just stored (read back through L2 after a CTA barrier) -- no second launch, no second pass over X_embed in HBM.
+ * Otherwise it is dpi_forward followed by the FM kernel on the same stream. Either way y / v are bit-identical to
+ * dpi_fm_interaction applied to the block this call wrote (the same per-sample code runs in both). One common dim, default columns and
+ * sample-major bags only (DPI_ERR_UNSUPPORTED otherwise); y_dev 4-byte, v_dev 16-byte aligned. Asynchronous on `stream`.
+ */
+dpi_status_t dpi_forward_fm(dpi_plan_t* plan, const int32_t* lengths_dev, const void* const* table_ptrs_dev,
+                            const void* indices_dev, const uint8_t* pooling, void* out_dev, float* y_dev, float* v_dev,
+                            void* stream);
+
+/*
  * dpi_cross_combine -- the non-GEMM part of one DCNv2 cross layer, x_{l+1} = x_0 * (W x_l + b) + x_l, given
  * u = W x_l from the caller's GEMM: out[b,f] = x0[b,f] * (u[b,f] + bias[f]) + xl[b,f]  (element-wise add, multiply,
  * add fused into one pass).

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "dpi_internal.cuh"
+#include "../../include/dpi_nongemm.h"
 
 namespace dpi {
 namespace {
@@ -110,6 +111,8 @@ struct dpi_plan_s {
     int direct_grid_cap = 0;       // short-bag variant as its own launch: SMs x resident CTAs
     uint32_t fused_chunks = 0;     // fused single-launch path: CTAs (0 = no instantiation) and bags per CTA
     uint32_t fused_chunk_bags = 0;
+    uint32_t fused_fm_chunks = 0;  // the same with chunks of whole samples (dpi_forward_fm); 0 = not possible
+    uint32_t fused_fm_chunk_bags = 0;
     std::vector<int64_t> columns;  // dpi_plan_set_columns, kept for the sub-plans of dpi_forward_host
 };
 
@@ -246,6 +249,14 @@ void prepare_launches(dpi_plan_t* p) {
         p->fused_chunk_bags = static_cast<uint32_t>((p->G + chunks - 1) / chunks);
         p->fused_chunks = (p->G + p->fused_chunk_bags - 1) / p->fused_chunk_bags;
         if (p->fused_chunk_bags > static_cast<uint32_t>(kFusedMaxChunkBags)) p->fused_chunks = 0;   // a thread keeps <= 8 bags in registers
+        // chunks of whole samples for the FM epilogue: the bag count of a chunk rounded up to a multiple of T
+        const uint64_t T = static_cast<uint64_t>(p->T);
+        const uint64_t fm_bags = (p->fused_chunk_bags + T - 1) / T * T;
+        p->fused_fm_chunks = 0;
+        if (p->fused_chunks && fm_bags <= static_cast<uint64_t>(kFusedMaxChunkBags)) {
+            p->fused_fm_chunk_bags = static_cast<uint32_t>(fm_bags);
+            p->fused_fm_chunks = static_cast<uint32_t>((p->G + fm_bags - 1) / fm_bags);
+        }
     }
 }
 
@@ -404,12 +415,16 @@ bool fused_eligible(const dpi_plan_t* p, const LookupCall& c) {
     return p->G <= max_bags && static_cast<uint64_t>(p->max_indices) <= 8ull * p->G;
 }
 
-dpi_status_t launch_fused_forward(dpi_plan_t* p, const int32_t* lengths_dev, const LookupCall& c, cudaStream_t stream) {
+dpi_status_t launch_fused_forward(dpi_plan_t* p, const int32_t* lengths_dev, const LookupCall& c, cudaStream_t stream,
+                                  float* fm_y = nullptr, float* fm_v = nullptr) {
     FusedArgs f{};
     f.plan = plan_args(p, lengths_dev);
-    f.plan.num_chunks = p->fused_chunks;
-    f.chunk_bags = p->fused_chunk_bags;
-    f.items = (p->fused_chunk_bags + kFusedThreads - 1) / kFusedThreads;
+    const bool fm = fm_y || fm_v;
+    f.plan.num_chunks = fm ? p->fused_fm_chunks : p->fused_chunks;
+    f.chunk_bags = fm ? p->fused_fm_chunk_bags : p->fused_chunk_bags;
+    f.fm_y = fm_y;
+    f.fm_v = fm_v;
+    f.items = (f.chunk_bags + kFusedThreads - 1) / kFusedThreads;
     f.k_shift = 32;
     for (uint32_t b = 0; b < 31; ++b) if (static_cast<uint32_t>(p->K) == (1u << b)) f.k_shift = b;
     LookupArgs& a = f.look;
@@ -825,6 +840,34 @@ dpi_status_t dpi_forward(dpi_plan_t* p, const int32_t* lengths_dev, const void* 
     LookupCall c;
     c.tables = table_ptrs_dev; c.indices = indices_dev; c.pooling = pooling; c.out = out_dev;
     return forward_device(p, lengths_dev, c, static_cast<cudaStream_t>(stream));
+}
+
+dpi_status_t dpi_forward_fm(dpi_plan_t* p, const int32_t* lengths_dev, const void* const* table_ptrs_dev, const void* indices_dev,
+                            const uint8_t* pooling, void* out_dev, float* y_dev, float* v_dev, void* stream) {
+    if (!p || !lengths_dev) return fail(DPI_ERR_INVALID_ARG, "plan/lengths_dev is NULL");
+    if (!y_dev && !v_dev) return fail(DPI_ERR_INVALID_ARG, "dpi_forward_fm: neither y_dev nor v_dev given");
+    if ((reinterpret_cast<uintptr_t>(lengths_dev) & 3u) || (reinterpret_cast<uintptr_t>(y_dev) & 3u) || (reinterpret_cast<uintptr_t>(v_dev) & 15u))
+        return fail(DPI_ERR_INVALID_ARG, "dpi_forward_fm: misaligned pointer");
+    if (p->mixed_dims || p->custom_columns || p->bag_order != DPI_BAGS_SAMPLE_MAJOR)
+        return fail(DPI_ERR_UNSUPPORTED, "dpi_forward_fm needs one common dim, default columns and sample-major bags");
+    const bool was_built = p->built;
+    p->built = true;
+    dpi_status_t st = check_lookup_pointers(p, table_ptrs_dev, indices_dev, out_dev);
+    p->built = was_built;
+    if (st != DPI_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    LookupCall c;
+    c.tables = table_ptrs_dev; c.indices = indices_dev; c.pooling = pooling; c.out = out_dev;
+    // one launch: the fused forward kernel with chunks of whole samples and the FM epilogue
+    if (fused_eligible(p, c) && p->fused_fm_chunks != 0 && p->out_dtype == p->dtype)
+        return launch_fused_forward(p, lengths_dev, c, s, y_dev, v_dev);
+    // otherwise the chain: dpi_forward, then fm_kernel on the block it wrote (same per-sample arithmetic)
+    st = forward_device(p, lengths_dev, c, s);
+    if (st != DPI_OK) return st;
+    cudaError_t e = launch_fm(out_dev, p->out_dtype, static_cast<uint32_t>(p->B), static_cast<uint32_t>(p->T), static_cast<uint32_t>(p->D),
+                              static_cast<uint64_t>(p->out_width) * out_elt_bytes(p), y_dev, v_dev, s);
+    if (e != cudaSuccess) return cuda_fail(e, "fm_kernel launch");
+    return DPI_OK;
 }
 
 dpi_status_t dpi_plan_status(const dpi_plan_t* p, int32_t* overflowed_builds, void* stream) {

@@ -140,6 +140,8 @@ struct FusedArgs {
     uint32_t items;                      // bags per thread = ceil(chunk_bags / kFusedThreads)
     uint32_t any_mean;                   // some table is mean-pooled (else the pooling mask is never consulted)
     uint32_t k_shift;                    // log2(K) when the quantum is a power of two, else 32 (divide)
+    float* fm_y;                         // dpi_forward_fm: fp32[B] FM second-order term (chunk_bags is then a multiple of T), or NULL
+    float* fm_v;                         // dpi_forward_fm: fp32[B, D] or NULL
 };
 cudaError_t launch_fused(const FusedArgs& a, int dtype, bool out32, int lanes, bool pdl, cudaStream_t stream);
 int fused_occupancy(int dtype, bool out32, int lanes, uint32_t T);   // resident CTAs per SM (0: no instantiation)

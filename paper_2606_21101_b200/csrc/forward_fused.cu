@@ -27,6 +27,7 @@
 // lookup. Same arithmetic as lookup_kernel: fp32 accumulation in entry order, one RNE cast at the store, mean by
 // reciprocal, bags of length <= 1 bit-exact, empty bags +0.0.
 #include "lookup_kernels.cuh"
+#include "nongemm_device.cuh"
 
 namespace dpi {
 namespace {
@@ -309,6 +310,24 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
                 if (((la.pool.w[t >> 5] >> (t & 31)) & 1u) && hi - lo > 1) scale_mean(acc, hi - lo);
                 store_pooled<Tr, OUT32>(out + (static_cast<size_t>(g_lo + i) * la.nvec + sl) * kOutVec, acc);
             }
+        }
+    }
+
+    // ---- FM epilogue (dpi_forward_fm; "combine all neighbouring non-GEMM operators into a single operator"):
+    // chunks hold whole samples, so the FM second-order term of a sample is formed by this CTA from the T pooled vectors it
+    // has just stored -- read back through L2 (coherent loads, after a CTA barrier), not from HBM by a second kernel.
+    // Same per-sample code as fm_kernel: bit-identical to dpi_fm_interaction run on the block this launch wrote. ----
+    if constexpr (!(OUT32 && Tr::kEltBytes == 2)) {
+        if (a.fm_y != nullptr || a.fm_v != nullptr) {
+            __syncthreads();
+            FmArgs fa;
+            fa.x = static_cast<const char*>(la.out);
+            fa.y = a.fm_y; fa.v = a.fm_v;
+            fa.x_pitch = static_cast<uint64_t>(la.T) * la.nvec * 16;
+            fa.B = la.B; fa.T = la.T; fa.nvec = la.nvec;
+            fa.D = la.nvec * (16 / Tr::kEltBytes);
+            const uint32_t b0 = g_lo / la.T, ns = nb / la.T;
+            for (uint32_t b = warp; b < ns; b += NW) fm_one_sample<Tr::kDtype, W, 4>(fa, b0 + b, static_cast<int>(lane));
         }
     }
 

@@ -92,6 +92,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 __device__ __forceinline__ void add2(float2& a, float x, float y) { a = __fadd2_rn(a, make_float2(x, y)); }
 
 struct F32Traits {
+    static constexpr int kDtype = DPI_F32;
     static constexpr int kVecBytes = 16;  // bytes of a row held by one lane
     using Row = uint4;
     __device__ static __forceinline__ Row load(const void* p, bool pred) { return ld_row16(p, pred); }
@@ -111,6 +112,7 @@ struct F32Traits {
     }
 };
 struct F16Traits {
+    static constexpr int kDtype = DPI_F16;
     static constexpr int kVecBytes = 16;  // bytes of a row held by one lane
     using Row = uint4;
     __device__ static __forceinline__ Row load(const void* p, bool pred) { return ld_row16(p, pred); }
@@ -141,6 +143,7 @@ struct F16Traits {
     }
 };
 struct BF16Traits {
+    static constexpr int kDtype = DPI_BF16;
     static constexpr int kVecBytes = 16;  // bytes of a row held by one lane
     using Row = uint4;
     __device__ static __forceinline__ Row load(const void* p, bool pred) { return ld_row16(p, pred); }
@@ -172,6 +175,7 @@ struct BF16Traits {
 // 32 bytes of the row per lane (256-bit loads): two halves of the base type side by side, element order preserved.
 template <class Base>
 struct Wide {
+    static constexpr int kDtype = Base::kDtype;
     static constexpr int kAcc = 2 * Base::kAcc;
     static constexpr int kEltBytes = Base::kEltBytes;
     static constexpr int kVecBytes = 32;

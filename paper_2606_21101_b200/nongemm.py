@@ -13,7 +13,7 @@ import numpy as np
 from . import binding
 from .binding import _check, _ptr, _stream_handle
 
-EXPORTS = ["dpi_fm_interaction", "dpi_lr_first_order", "dpi_cross_combine", "dpi_bias_act", "dpi_bfs_schedule", "dpi_launcher_create",
+EXPORTS = ["dpi_forward_fm", "dpi_fm_interaction", "dpi_lr_first_order", "dpi_cross_combine", "dpi_bias_act", "dpi_bfs_schedule", "dpi_launcher_create",
            "dpi_launcher_destroy", "dpi_launcher_run"]
 
 ACT_IDENTITY, ACT_RELU, ACT_SIGMOID = 0, 1, 2
@@ -37,6 +37,7 @@ def _lib() -> ctypes.CDLL:
         vp, i32, i64, st = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int
         sig = {
             "dpi_fm_interaction": (st, [vp, ctypes.c_int, i32, i32, i32, i64, vp, vp, vp]),
+            "dpi_forward_fm": (st, [vp, vp, vp, vp, vp, vp, vp, vp, vp]),
             "dpi_cross_combine": (st, [vp, vp, vp, vp, vp, ctypes.c_int, i32, i32, vp]),
             "dpi_lr_first_order": (st, [vp, vp, vp, i32, i32, ctypes.c_float, vp, i32, vp]),
             "dpi_bias_act": (st, [vp, vp, vp, ctypes.c_int, i32, i32, ctypes.c_int, vp]),
@@ -57,6 +58,15 @@ def fm_interaction(x, dtype: int, B: int, T: int, D: int, y=None, v=None, x_ld: 
     """dpi_fm_interaction: x [B, x_ld] device tensor of `dtype`; y fp32[B] and / or v fp32[B, D] device tensors."""
     _check(_lib().dpi_fm_interaction(_ptr(x), int(dtype), int(B), int(T), int(D), int(x_ld), _ptr(y), _ptr(v),
                                      _stream_handle(stream)))
+
+
+def forward_fm(plan, lengths_dev, table_ptrs_dev, indices_dev, out_dev, y=None, v=None, pooling=None, stream=None) -> None:
+    """dpi_forward_fm: dpi_forward (plan + fused lookup into out_dev) plus the FM second-order term y fp32[B] / v fp32[B, D] of
+    every sample -- one launch on small / short-bag batches. `plan` is a binding.Plan."""
+    import numpy as np
+    pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
+    _check(_lib().dpi_forward_fm(plan._h, _ptr(lengths_dev), _ptr(table_ptrs_dev), _ptr(indices_dev), _ptr(pool), _ptr(out_dev),
+                                 _ptr(y), _ptr(v), _stream_handle(stream)))
 
 
 def lr_first_order(w_ptrs, indices, offsets, B: int, T: int, bias: float, y, accumulate: bool = False, stream=None) -> None:

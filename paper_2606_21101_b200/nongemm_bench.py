@@ -206,6 +206,47 @@ def bench_launcher(lines):
     lines.append("")
 
 
+def bench_forward_fm(lines):
+    """dpi_forward_fm (lookup + FM term, ONE launch on the small configs) against the chain dpi_forward -> dpi_fm_interaction
+    (two launches) and planner + lookup + FM (three): GPU time per step from graph replays over rotating batches."""
+    from . import binding
+    lines += ["## dpi_forward_fm: the lookup and its first non-GEMM consumer as one operator (PAPER.md:188)", "",
+              "GPU time per step (us), CUDA-graph replays of 24 steps over 8 rotating batches, median (min).", "",
+              "| workload | forward_fm (1 launch) | forward + fm (2 launches) | plan + lookup + fm (3 launches) |", "|---|---|---|---|"]
+    for name in ("c1", "c2", "c3"):
+        cfg = W.CONFIGS[name]
+        rows = cfg.table_rows()
+        dt = harness.make_device_tables(cfg, rows)
+        batches = [harness.upload_batch(W.make_batch(cfg, rows, cfg.seed + r)) for r in range(8)]
+        pooling = cfg.pooling_modes()
+        plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg))
+        out = harness.new_output(cfg)
+        y = torch.zeros(cfg.B, device="cuda")
+        code = W.DTYPE_CODE[cfg.out]
+
+        def one(i, s):
+            b = batches[i]
+            nongemm.forward_fm(plan, b.lengths, dt.ptrs, b.indices, out, y=y, pooling=pooling, stream=s)
+
+        def two(i, s):
+            b = batches[i]
+            plan.forward(b.lengths, dt.ptrs, b.indices, out, pooling=pooling, stream=s)
+            nongemm.fm_interaction(out, code, cfg.B, cfg.T, cfg.D, y=y, stream=s)
+
+        def three(i, s):
+            b = batches[i]
+            plan.build(b.lengths, s)
+            plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=s)
+            nongemm.fm_interaction(out, code, cfg.B, cfg.T, cfg.D, y=y, stream=s)
+
+        res = [time_rotating(f, 8) for f in (one, two, three)]
+        lines.append(f"| {name} | " + " | ".join(f"{m:.2f} ({lo:.2f})" for m, lo in res) + " |")
+        plan.destroy()
+        del dt, batches
+        torch.cuda.empty_cache()
+    lines.append("")
+
+
 def profile_pass():
     """Three plain launches of each operator at a 65 536-row shape (no graphs, no timing): the target of an
     `ncu --set full -k regex:"fm_kernel|cross_combine|bias_act"` capture."""
@@ -232,6 +273,7 @@ def main():
     ap.add_argument("--out", default="")
     ap.add_argument("--skip-launcher", action="store_true")
     ap.add_argument("--profile", action="store_true", help="only launch each operator three times (for ncu)")
+    ap.add_argument("--forward-fm", action="store_true", help="only the dpi_forward_fm comparison")
     args = ap.parse_args()
     harness.require_cuda()
     torch.cuda.set_device(0)
@@ -239,9 +281,13 @@ def main():
         return profile_pass()
     lines = ["# NEXT-4 measurements (python -m paper_2606_21101_b200.nongemm_bench)", "",
              f"Device: {torch.cuda.get_device_name(0)}. CUDA events on the launching stream, after warm-up. Synthetic seeded inputs.", ""]
-    bench_operators(lines)
-    if not args.skip_launcher:
-        bench_launcher(lines)
+    if args.forward_fm:
+        bench_forward_fm(lines)
+    else:
+        bench_operators(lines)
+        bench_forward_fm(lines)
+        if not args.skip_launcher:
+            bench_launcher(lines)
     text = "\n".join(lines)
     print(text)
     if args.out:

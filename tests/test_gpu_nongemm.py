@@ -12,7 +12,7 @@ import pytest
 import torch
 
 import oracle
-from paper_2606_21101_b200 import harness, nongemm
+from paper_2606_21101_b200 import binding, harness, nongemm
 from paper_2606_21101_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
@@ -373,3 +373,92 @@ def test_lr_all_empty_and_validation():
         nongemm.lr_first_order(None, idx, off, B, T, 0.0, y)
     with pytest.raises(binding.DpiError):
         nongemm.lr_first_order(ptrs, idx, off, B, 0, 0.0, y)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# dpi_forward_fm: the lookup and its first non-GEMM consumer as one operator
+# ---------------------------------------------------------------------------------------------------------------
+def _lookup_tol(ref, lengths, T, D, dtype):
+    """Per-element tolerance of the pooled block (tests/parity.py) as an array [B, T*D]."""
+    L = np.repeat(np.maximum(lengths.reshape(-1, T), 1), D, axis=1).astype(np.float64)
+    if dtype == "f32":
+        return 1e-5 * L
+    return np.maximum(2e-3 * np.abs(ref), 1e-6 * L)
+
+
+def _forward_fm_case(cfg, batch_seed=None, fused=0, expect_launches=None):
+    from tests.parity import assert_outputs_match, oracle_reference
+    rows = cfg.table_rows()
+    host_tables = [W.full_table_storage(cfg, t, int(rows[t])) for t in range(cfg.T)]
+    dt = harness.tables_from_host(cfg, host_tables)
+    batch = W.make_batch(cfg, rows, batch_seed)
+    db = harness.upload_batch(batch)
+    pooling = cfg.pooling_modes()
+    plan = harness.make_plan(cfg, rows, max(batch.N, 1))
+    plan.set_option(binding.OPT_FUSED, fused)
+    B, T, D = cfg.B, cfg.T, cfg.D
+    out = harness.new_output(cfg, fill_nan=True)
+    y = torch.full((B,), float("nan"), device="cuda")
+    v = torch.full((B, D), float("nan"), device="cuda")
+    before = binding.launch_count()
+    nongemm.forward_fm(plan, db.lengths, dt.ptrs, db.indices, out, y=y, v=v, pooling=pooling)
+    launches = binding.launch_count() - before
+    torch.cuda.synchronize()
+    if expect_launches is not None:
+        assert launches == expect_launches
+    # the block and the plan are exactly what dpi_forward leaves behind
+    ref = oracle_reference(host_tables, cfg.dtype, B, batch.lengths, batch.indices, pooling)
+    assert_outputs_match(harness.out_to_f64(out), ref, batch.lengths, T, D, cfg.dtype, cfg.out)
+    off, seg, S, N = plan.export()
+    o_off, o_seg, o_S = oracle.plan(batch.lengths, plan.info()["K"])
+    assert N == batch.N and S == o_S and np.array_equal(off, o_off) and np.array_equal(seg, o_seg)
+    # FM by its definition on the ORACLE's block; tolerance = the FM operator's own bound + the pooled block's tolerance
+    # carried through v_c = sum_{t<u} x_t x_u:  |dv_c| <= A_c E_c + E_c^2,  A_c = sum_t |x_tc|,  E_c = sum_t tol_tc
+    ref_y, ref_v = oracle.fm_pairwise(ref, T, D)
+    A = np.abs(ref).reshape(B, T, D).sum(axis=1)
+    E = _lookup_tol(ref, batch.lengths, T, D, cfg.dtype).reshape(B, T, D).sum(axis=1)
+    tol_v = 2 * (T + 2) * U32 * (A + E) ** 2 + A * E + E * E
+    got_v, got_y = f64(v), f64(y)
+    assert not np.isnan(got_v).any() and not np.isnan(got_y).any()
+    assert (np.abs(got_v - ref_v) <= tol_v).all(), f"v: max err {np.abs(got_v - ref_v).max():.3e}"
+    tol_y = tol_v.sum(axis=1) + 8 * U32 * np.abs(ref_v).sum(axis=1)
+    assert (np.abs(got_y - ref_y) <= tol_y).all(), f"y: max err {np.abs(got_y - ref_y).max():.3e}"
+    # and y / v are bit-identical to dpi_fm_interaction applied to the block this very call wrote (the same per-sample code
+    # runs in the epilogue and in fm_kernel; the block itself may differ from plan + lookup in summation order only)
+    y2 = torch.full((B,), float("nan"), device="cuda")
+    v2 = torch.full((B, D), float("nan"), device="cuda")
+    nongemm.fm_interaction(out, W.DTYPE_CODE[cfg.out], B, T, D, y=y2, v=v2)
+    torch.cuda.synchronize()
+    assert torch.equal(y, y2) and torch.equal(v, v2)
+    plan.destroy()
+    return launches
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3"])
+def test_forward_fm_is_one_launch_on_the_small_configs_full_size(name):
+    assert _forward_fm_case(W.CONFIGS[name], expect_launches=1) == 1
+
+
+@pytest.mark.parametrize("dtype,D,lengths,pool", [("f32", 16, ("uniform", 0, 4), "half"), ("f16", 32, ("uniform", 1, 3), "mean"),
+                                                   ("bf16", 64, ("const", 1), "sum"), ("f32", 64, ("poisson", 20.0, 100, 0.05), "half"),
+                                                   ("f16", 8, ("uniform", 0, 40), "sum")])
+@pytest.mark.parametrize("B,T", [(1, 1), (37, 3), (300, 22), (2049, 7), (129, 100)])
+def test_forward_fm_shapes_whole_sample_chunks_and_long_bags(dtype, D, lengths, pool, B, T):
+    """T that does not divide the natural chunk size (chunks are rounded up to whole samples), one sample, more tables than
+    lane groups, bags long enough for the warp-per-bag chunk path; fused forced on so every shape takes the single launch."""
+    cfg = W.Config("ffm", T, tuple(int(7 + 13 * t) for t in range(T)), D, dtype, B, lengths, ("zipf", 1.1), pool, seed=5)
+    assert _forward_fm_case(cfg, fused=1, expect_launches=1) == 1
+
+
+def test_forward_fm_falls_back_to_the_chain_and_validates():
+    # fp32 output of bf16 tables and batches beyond the fused rule: planner + lookup + FM kernel, same results
+    cfg = W.Config("ffm2", 5, (100, 20, 7, 300, 50), 32, "bf16", 200, ("uniform", 0, 5), ("uniform",), "half", seed=3, out_dtype="f32")
+    assert _forward_fm_case(cfg, expect_launches=None) >= 2
+    cfg = W.Config("ffm3", 4, (100, 20, 7, 300), 16, "f32", 64, ("poisson", 20.0, 100, 0.0), ("uniform",), "sum", seed=3)
+    assert _forward_fm_case(cfg, fused=2, expect_launches=3) == 3
+    plan = binding.Plan([10, 10], np.asarray([16, 8], np.int32), 0, 4, 8)     # mixed dims: no FM
+    z = torch.zeros(64, device="cuda")
+    with pytest.raises(binding.DpiError) as e:
+        nongemm.forward_fm(plan, z.view(torch.int32), z, z.view(torch.int32), z, y=z)
+    assert e.value.status == 2
+    plan.destroy()
