@@ -60,6 +60,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--fused", type=int, default=-1, help="dpi_forward: -1 library default (auto), 0 auto, 1 fused whenever the layout allows, 2 always planner + lookup")
+    ap.add_argument("--bag-hint", type=int, default=0, help="1: pass the recipe's longest bag as the OPTIONAL promise DPI_OPT_MAX_BAG_HINT "
+                    "(the short-bag variant then runs as its own launch, chosen on the host); default 0 = no promise, the device picks")
     ap.add_argument("--vec-bytes", type=int, default=0, help="DPI_OPT_VEC_BYTES: 0 auto, 16 / 32 bytes of a row per lane and load")
     ap.add_argument("--shard", default="batch", choices=["batch", "tables"],
                     help="multi-GPU layout: batch-sharded replicas (default, DESIGN.md 9) or table-wise sharding with the all-to-all "
@@ -442,7 +444,7 @@ def run_ours(args):
     batches = [harness.upload_batch(sharding.make_batch_shard(cfg, rows, cfg.seed + r, rank, world), device=device)
                for r in range(R)]
     pooling = cfg.pooling_modes()
-    plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg))   # no bag-length promise: the device picks the a3 variant
+    plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg), bag_hint=bool(args.bag_hint))   # default: no promise, the device picks
     apply_options(plan, args, binding)
     if args.fused >= 0:
         plan.set_option(binding.OPT_FUSED, args.fused)
@@ -603,6 +605,9 @@ def run_ours(args):
         kname = "lookup_kernel (a3 fused gather-and-pool" + (", short-bag body picked on the device from a1's max_len)" if short else ")")
         ncu_name = "lookup_kernel"
         variant = "planner + " + ("short-bag body of lookup_kernel (device-picked)" if short else "balanced segments")
+        if args.bag_hint and harness.lookup_variant(cfg, args.mode).startswith("short-bag"):
+            kname, ncu_name = "direct_kernel (a3, short-bag variant as its own launch, chosen on the host from the promise)", "direct_kernel"
+            variant = "planner + direct_kernel (DPI_OPT_MAX_BAG_HINT promise)"
     k_bytes = bytes_step["total"] if fused else bytes_step["lookup"]
     achieved = k_bytes / (k_ms * 1e-3) / 1e9
     traffic, traffic_note = ncu_traffic(cfg.name, ncu_name)
@@ -627,7 +632,7 @@ def run_ours(args):
                                        "launch": "CUDA graph replay of the K steps" if graph is not None else "stream launches",
                                        "api": "dpi_forward" if not ablation else "dpi_plan_build + dpi_lookup_input_first",
                                        "launches_per_step": launches_per_step,
-                                       "quantum_K": plan.info()["K"], "max_bag_hint": 0,
+                                       "quantum_K": plan.info()["K"], "max_bag_hint": harness.max_bag_length(cfg) if args.bag_hint else 0,
                                        "max_len_measured_by_a1": int(max(max_lens)),
                                        "lookup_variant": variant, "rows_gathered_per_step": n_mean,
                                        "segments_per_step": s_mean}, R),
