@@ -110,7 +110,9 @@ typedef enum {
                                    only without load balancing; dpi_check_indices verifies the promise off the hot path. */
     DPI_OPT_FUSED = 9,          /* dpi_forward / dpi_forward_host: 0 = auto (one fused launch when the layout is the dense one,
                                    G <= DPI_OPT_FUSED_MAX_BAGS and the capacity says bags are short on average,
-                                   max_indices <= 8*G), 1 = fused whenever the layout allows, 2 = always plan + lookup */
+                                   max_indices <= 8*G; not when DPI_OPT_MAX_BAG_HINT = 1 promises one id per bag and G < 4e5:
+                                   planner + the short-bag launch measured 11-24 % faster there), 1 = fused whenever the layout
+                                   allows, 2 = always plan + lookup */
     DPI_OPT_FUSED_MAX_BAGS = 10,/* ceiling of the auto rule above in bags; 0 = library default (2^20) */
     DPI_OPT_VEC_BYTES = 11,     /* bytes of a row one lane loads at a time in the dense balanced-segment kernel: 0 = auto (32 --
                                    the sm_100 256-bit load, half the lanes and load instructions per row -- whenever all dims are

@@ -398,8 +398,10 @@ PlanArgs plan_args(const dpi_plan_t* p, const int32_t* lengths_dev) {
     return a;
 }
 
-// Default ceiling of the fused single-launch path (bags). Measured on B200: below it one launch beats
-// plan + lookup on every short-bag shape tried; above it the statically chunked CTAs lose to the persistent kernels.
+// Default ceiling of the fused single-launch path (bags). Measured on B200 (profiles/r02_forward_crossover.md):
+// against planner + lookup WITHOUT a bag-length promise the single launch is within 3 % at worst (one id per bag, < 2e5 bags) and
+// 6-22 % faster elsewhere, up to the size where a chunk no longer fits the kernel's 2048 bags (~1.2e6 bags at one wave). Against
+// the PROMISED two-launch path it loses 11-24 % on one-hot batches below ~2e5 bags: see fused_eligible().
 constexpr uint64_t kFusedDefaultMaxBags = 1u << 20;
 
 // May this call run as ONE launch (forward_fused.cu)? Host-known facts only: the layout is the dense one, and the plan's
@@ -411,6 +413,10 @@ bool fused_eligible(const dpi_plan_t* p, const LookupCall& c) {
         c.offsets || (c.out_ld && c.out_ld != p->out_width))
         return false;
     if (p->opt[DPI_OPT_FUSED] == 1) return true;
+    // A caller who promised at most ONE id per bag gets planner + the lean short-bag launch below 4e5 bags: 7.5 / 8.1 / 9.3 / 11.3 us
+    // against 8.3 / 10.0 / 10.6 / 13.2 us fused at 1.3e4 / 5.3e4 / 1.1e5 / 2.1e5 bags (the fused launch has nothing to amortise its
+    // look-back over); from 4.3e5 bags on the single launch wins again (16.9 vs 18.6 us).
+    if (p->opt[DPI_OPT_MAX_BAG_HINT] == 1 && p->G < 400000u) return false;
     const uint64_t max_bags = p->opt[DPI_OPT_FUSED_MAX_BAGS] > 0 ? static_cast<uint64_t>(p->opt[DPI_OPT_FUSED_MAX_BAGS]) : kFusedDefaultMaxBags;
     return p->G <= max_bags && static_cast<uint64_t>(p->max_indices) <= 8ull * p->G;
 }

@@ -681,9 +681,10 @@ __global__ void __launch_bounds__(kLookupMaxThreads, lookup_min_ctas<Tr, U, GEN>
                     if constexpr (!GEN && Tr::kEltBytes == 4) {
                         // whole batch inside the bag (warp-uniform): no bounds compare, no clamped index, no predicate and
                         // no zeroed destination registers per load; only a bag's ragged last batch takes the predicated
-                        // form below. fp32 tables only (measured): c5 0.720 -> 0.703 ms, but on bf16 c4
-                        // the extra compare + branch and the second copy of the load code cost more than they save
-                        // (0.381 -> 0.396 ms) -- its loop is dominated by the bf16 -> fp32 conversions and already issue-bound
+                        // form below. An instruction diet, not a speed-up: on c5 it removes 15 % of the
+                        // issued instructions and, in a same-box A/B, no time (the kernel is HBM-bound). fp32 tables only:
+                        // on bf16 c4, which IS issue-bound, the extra compare + branch and the second copy of the load code
+                        // cost more than they save (0.396 ms, against 0.381-0.384 ms on every other call)
                         if (lanes_full && j + P * U <= hi) {
 #pragma unroll
                             for (int u = 0; u < U; ++u) {

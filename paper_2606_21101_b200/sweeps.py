@@ -1,6 +1,7 @@
 """Scenario sweeps of the paper's Fig. 10 / Fig. 11 on synthetic Criteo-shaped one-hot input.
 
     python -m paper_2606_21101_b200.sweeps [--only fig10_batch,fig11_dim] [--out gpurun_out/sweeps.md]
+    python -m paper_2606_21101_b200.sweeps --only forward_crossover [--out ...]   # one launch vs two, over batch size
 
 The paper varies four things around the embedding stage (§V-F): batch size (D = 32),
 embedding dimension (B = 2048), number of feature fields (B = 2048, D = 32, 5e5 features per field) and
@@ -138,6 +139,59 @@ def run_point(cfg, n_iter: int = 200, rotating: int = 4, with_torch: bool = True
     return res
 
 
+def run_forward_crossover(n_iter: int = 200, rotating: int = 8) -> str:
+    """Where does ONE launch (dpi_forward's fused kernel) stop paying off? Graph-replayed us per step over batch size for a
+    one-hot shape (c2's recipe, D = 16) and a 1-3-entries shape (c3's recipe, fp16 D = 32, mean): fused forced on
+    (DPI_OPT_FUSED = 1; '-' where a chunk would exceed the kernel's 2048 bags), two launches without a promise (device-picked
+    variant), two launches with the bag-length promise. The auto rule's ceiling (DPI_OPT_FUSED_MAX_BAGS) is read off this table."""
+    import torch
+    from . import binding, harness, workloads as W
+    lines = ["## forward_crossover", "",
+             "Graph-replayed us per step (plan + lookup work of one batch), 8 rotating batches. fused = `dpi_forward` with `DPI_OPT_FUSED = 1`; two launches ="
+             " `DPI_OPT_FUSED = 2`, without / with `DPI_OPT_MAX_BAG_HINT`.", "",
+             "| shape | B | bags G | fused (1 launch) | two launches, no promise | two launches, promise | fused / no promise | fused / promise |",
+             "|---|---|---|---|---|---|---|---|"]
+    shapes = [("one id per bag (c2 recipe)", W.C2, (512, 2048, 4096, 8192, 16384, 32768, 65536)),
+              ("1-3 ids per bag (c3 recipe)", W.C3, (512, 2048, 8192, 16384, 32768, 65536, 98304))]
+    for label, base, sizes in shapes:
+        for B in sizes:
+            cfg = base.scaled(name=f"{base.name}-B{B}", B=B)
+            rows = cfg.table_rows()
+            dt = harness.make_device_tables(cfg, rows)
+            batches = [harness.upload_batch(W.make_batch(cfg, rows, cfg.seed + r)) for r in range(rotating)]
+            out = harness.new_output(cfg)
+            pooling = cfg.pooling_modes()
+            stream = torch.cuda.Stream()
+            res = []
+            for fused, hint in ((1, False), (2, False), (2, True)):
+                plan = harness.make_plan(cfg, rows, harness.max_indices_bound(cfg), bag_hint=hint)
+                plan.set_option(binding.OPT_FUSED, fused)
+
+                def step(i, st, plan=plan):
+                    b = batches[i % rotating]
+                    plan.forward(b.lengths, dt.ptrs, b.indices, out, pooling=pooling, stream=st)
+
+                with torch.cuda.stream(stream):
+                    n0 = binding.launch_count()
+                    step(0, stream)
+                    launches = binding.launch_count() - n0
+                    for i in range(1, 4):
+                        step(i, stream)
+                torch.cuda.synchronize()
+                us = _time_graph(step, stream, n_iter)
+                res.append(None if (fused == 1 and launches != 1) else us)
+                plan.destroy()
+            f, n, h = res
+            fmt = lambda x: "-" if x is None else f"{x:.2f}"
+            lines.append(f"| {label} | {B} | {cfg.G} | {fmt(f)} | {fmt(n)} | {fmt(h)} | " +
+                         ("-" if f is None else f"{f / n:.2f}") + " | " + ("-" if f is None else f"{f / h:.2f}") + " |")
+            print(lines[-1], flush=True)
+            del dt, batches, out
+            torch.cuda.empty_cache()
+    lines.append("")
+    return "\n".join(lines)
+
+
 def sweep_points() -> Dict[str, List]:
     from . import workloads as W
     base = W.C2  # 26 one-hot fields, heights log-uniform [10, 1e6], Zipf 1.05, fp32, sum
@@ -188,6 +242,13 @@ def main():
     binding.load_library()
     sweeps = sweep_points()
     only = [s for s in args.only.split(",") if s]
+    if only == ["forward_crossover"]:
+        text = run_forward_crossover(n_iter=args.iters)
+        os.makedirs(os.path.dirname(os.path.abspath(args.out)) or ".", exist_ok=True)
+        with open(args.out, "w") as f:
+            f.write(text)
+        print("wrote", args.out)
+        return
     results = {}
     for name, pts in sweeps.items():
         if only and name not in only:

@@ -141,6 +141,26 @@ def test_forward_falls_back_to_two_launches_for_long_bag_capacities_and_variants
     assert launches == 2
 
 
+def test_forward_honours_a_one_id_per_bag_promise_below_4e5_bags():
+    """DPI_OPT_MAX_BAG_HINT = 1 on a small batch: dpi_forward takes planner + the short-bag launch (measured faster there,
+    profiles/r02_forward_crossover.md), two launches, same block; without the promise the same call is one launch."""
+    cfg = W.C2.scaled(name="c2-small", B=256)
+    rows, host_tables, dt = _tables(cfg)
+    batch = W.make_batch(cfg, rows, None)
+    db = harness.upload_batch(batch)
+    ref = oracle_reference(host_tables, cfg.dtype, cfg.B, batch.lengths, batch.indices, cfg.pooling_modes())
+    for hint, want in ((True, 2), (False, 1)):
+        plan = harness.make_plan(cfg, rows, batch.N, bag_hint=hint)
+        out = harness.new_output(cfg, fill_nan=True)
+        before = binding.launch_count()
+        plan.forward(db.lengths, dt.ptrs, db.indices, out, pooling=cfg.pooling_modes())
+        assert binding.launch_count() - before == want
+        torch.cuda.synchronize()
+        assert_outputs_match(harness.out_to_f64(out), ref, batch.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out)
+        _check_plan(plan, batch.lengths)
+        plan.destroy()
+
+
 def test_forward_overflow_is_counted():
     cfg = W.C1
     rows, host_tables, dt = _tables(cfg)
