@@ -276,6 +276,39 @@ dpi_status_t dpi_forward(dpi_plan_t* plan, const int32_t* lengths_dev, const voi
                          const void* indices_dev, const uint8_t* pooling, void* out_dev, void* stream);
 
 /*
+ * dpi_forward_noalloc -- dpi_forward for callers that cannot allocate device memory. It takes no dpi_plan_t (creating one
+ * costs nine cudaMalloc calls) and itself calls no cudaMalloc, cudaFree or any other allocating routine: the working memory
+ * of the one-launch path (forward_fused.cu: the offsets it scans, its look-back records and counters) is a fixed array of
+ * about 2 MB built into the library image. Meant for
+ *   - operators inside a serving runtime whose own arena holds all of the GPU's memory (tables + framework pool), where a
+ *     cudaMalloc from the operator fails or takes memory somebody else has budgeted;
+ *   - request threads with a latency bound, which cannot afford the driver locks and the device-wide synchronisation that
+ *     cudaMalloc / cudaFree may bring;
+ *   - stateless callbacks that are handed pointers and a stream and have nowhere to keep a plan handle between calls.
+ * The price: the array occupies its ~2 MB on EVERY GPU on which this library's code gets loaded, until the process exits; the
+ * batch is limited to DPI_NOALLOC_MAX_BAGS bags; and all calls on one GPU share the array, so calls whose kernels may overlap
+ * in time (different streams or host threads, same GPU) race on it and give wrong results -- keep them on one stream, or
+ * order them with events. Each call first resets the shared words (a one-CTA kernel), so nothing carries over from the call
+ * before, whatever its shape was; then runs the fused forward kernel: two launches, asynchronous on `stream`.
+ * The FIRST call on each device (with that device current) also looks up the array's device address and the SM count and
+ * caches them; make that first call outside any stream capture. Later calls do no set-up.
+ *   T, D, dtype     tables, their common embedding dim and storage type; D*sizeof(dtype) a multiple of 16 B, <= 512 B
+ *   B               samples; G = B*T must be <= DPI_NOALLOC_MAX_BAGS, else DPI_ERR_INVALID_ARG with a message naming the limit
+ *   lengths_dev     device int32[G], g = b*T + t (sample-major), as in dpi_plan_build; N = sum of lengths must be < 2^30
+ *                   (precondition; the host never sees N)
+ *   table_ptrs_dev, indices_dev (int32[N]), pooling (host uint8[T] or NULL), out_dev ([B, T*D] in the table dtype, 16-byte
+ *                   aligned)   as in dpi_lookup
+ * Result: the block dpi_forward writes on its fused path, bit for bit (same kernel). Like that path the chunks are not
+ * load-balanced across CTAs: right for the short-bag batches of CTR serving, correct but slower for long bags.
+ * Equal dims, int32 ids, sample-major bags, dense output in the table dtype only; everything else needs a dpi_plan_t.
+ * No plan is left behind for the caller: the array's contents after a call are unspecified.
+ */
+#define DPI_NOALLOC_MAX_BAGS 524288   /* 2^19 bags: 4 B of scratch per bag + 11 KB fixed */
+dpi_status_t dpi_forward_noalloc(int32_t T, int32_t D, dpi_dtype_t dtype, int32_t B, const int32_t* lengths_dev,
+                                 const void* const* table_ptrs_dev, const int32_t* indices_dev, const uint8_t* pooling,
+                                 void* out_dev, void* stream);
+
+/*
  * dpi_plan_status -- did any build of this plan since the last call exceed its capacity (N > max_indices)? Such a build
  * leaves S = 0 behind, so the balanced-segment lookup that follows writes nothing; the planner also bumps a sticky device
  * counter, which this call reads (synchronises `stream`) and clears. DPI_OK and *overflowed_builds = 0 when all builds

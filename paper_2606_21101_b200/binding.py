@@ -31,7 +31,7 @@ EXPORTS = ["dpi_plan_create", "dpi_plan_set_out_dtype", "dpi_plan_set_layout", "
            "dpi_plan_build", "dpi_plan", "dpi_plan_device_views", "dpi_plan_info", "dpi_plan_export", "dpi_plan_stats",
            "dpi_lookup", "dpi_forward", "dpi_plan_status", "dpi_lookup_onehot", "dpi_lookup_input_first", "dpi_forward_host", "dpi_check_indices", "dpi_plan_destroy", "dpi_launch_count",
            "dpi_version", "dpi_status_string", "dpi_last_error", "dpi_peer_alloc", "dpi_peer_open", "dpi_peer_close", "dpi_peer_free",
-           "dpi_plan_set_offset_type", "dpi_plan_export64"]
+           "dpi_plan_set_offset_type", "dpi_plan_export64", "dpi_forward_noalloc"]
 
 
 class LookupArgs(ctypes.Structure):
@@ -89,6 +89,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
         "dpi_lookup_input_first": (st, [vp, vp, vp, vp, vp, vp, vp]),
         "dpi_forward": (st, [vp, vp, vp, vp, vp, vp, vp]),
         "dpi_plan_status": (st, [vp, vp, vp]),
+        "dpi_forward_noalloc": (st, [i32, i32, ctypes.c_int, i32, vp, vp, vp, vp, vp, vp]),
         "dpi_lookup_onehot": (st, [vp, vp, vp, vp, vp]),
         "dpi_forward_host": (st, [vp, vp, vp, vp, i64, vp, vp, vp]),
         "dpi_check_indices": (st, [vp, vp, vp, vp]),
@@ -160,6 +161,18 @@ def peer_close(ptr: int):
 
 def peer_free(ptr: int):
     _check(load_library().dpi_peer_free(ctypes.c_void_p(ptr)))
+
+
+NOALLOC_MAX_BAGS = 524288
+
+
+def forward_noalloc(T: int, D: int, dtype: int, B: int, lengths_dev, table_ptrs_dev, indices_dev, out_dev, pooling=None, stream=None):
+    """dpi_forward_noalloc: the one-launch forward path on the library's built-in scratch array -- no plan object and no
+    device allocation, for callers that cannot call cudaMalloc (include/dpi.h). At most NOALLOC_MAX_BAGS bags; calls that
+    may overlap on one GPU race on the shared array."""
+    pool = None if pooling is None else np.ascontiguousarray(pooling, dtype=np.uint8)
+    _check(load_library().dpi_forward_noalloc(int(T), int(D), int(dtype), int(B), _ptr(lengths_dev), _ptr(table_ptrs_dev),
+                                              _ptr(indices_dev), _ptr(pool), _ptr(out_dev), _stream_handle(stream)))
 
 
 def launch_count() -> int:

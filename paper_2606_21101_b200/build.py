@@ -25,7 +25,7 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas"
 
 LIBS = {
     "libdpi.so": ["dpi_api.cu", "plan_kernels.cu", "plan64_kernels.cu", "lookup_f32.cu", "lookup_f16.cu", "lookup_bf16.cu",
-                  "ablation_input_first.cu", "lookup_onehot.cu", "lookup_direct.cu", "forward_fused.cu", "nongemm_kernels.cu", "nongemm_api.cu", "peer_api.cu"],
+                  "ablation_input_first.cu", "lookup_onehot.cu", "lookup_direct.cu", "forward_fused.cu", "forward_noalloc.cu", "nongemm_kernels.cu", "nongemm_api.cu", "peer_api.cu"],
     "libdpi_synth.so": ["synth_fill.cu"],
 }
 HEADERS = ["dpi_internal.cuh", "lookup_kernels.cuh", "lookup_dispatch.inc", os.path.join(INCLUDE, "dpi.h"),
