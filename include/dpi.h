@@ -114,12 +114,18 @@ typedef enum {
                                    planner + the short-bag launch measured 11-24 % faster there), 1 = fused whenever the layout
                                    allows, 2 = always plan + lookup */
     DPI_OPT_FUSED_MAX_BAGS = 10,/* ceiling of the auto rule above in bags; 0 = library default (2^20) */
-    DPI_OPT_VEC_BYTES = 11,     /* bytes of a row one lane loads at a time in the dense balanced-segment kernel: 0 = auto (32 --
-                                   the sm_100 256-bit load, half the lanes and load instructions per row -- whenever all dims are
-                                   equal and the row size is a multiple of 32 B; else 16), 16 = always 128-bit loads, 32 = require
-                                   256-bit (DPI_ERR_UNSUPPORTED if the rows do not allow it). With 32-byte vectors every table
-                                   base must be 32-byte aligned (any cudaMalloc / framework allocation is); an output block that
-                                   is only 16-byte aligned silently takes the 128-bit kernel. */
+    DPI_OPT_VEC_BYTES = 11,     /* bytes of a row one lane loads at a time in the dense balanced-segment kernel: 0 = auto: 32 (the
+                                   sm_100 256-bit load, half the lanes and load instructions per row) for fp32 tables with equal
+                                   dims and rows of >= 256 B that are a multiple of 32 B -- the one case where it measured faster
+                                    -- and 16 for everything else (16-bit tables, narrower rows, mixed dims);
+                                   16 = always 128-bit loads; 32 = require 256-bit for any dtype (DPI_ERR_UNSUPPORTED unless all
+                                   dims are equal and the row size is a multiple of 32 B). Whenever 32-byte vectors are in use
+                                   (auto on fp32 rows >= 256 B, or forced) every table BASE must be 32-byte aligned -- tighter than
+                                   the 16 bytes dpi_lookup otherwise asks for; any cudaMalloc / framework allocation is, a table
+                                   sliced at an odd 16-byte offset is not and faults with a misaligned address. The library
+                                   cannot check this (the pointers live on the device, and dpi_check_indices does not take
+                                   them): set 16 to keep such tables. An output block that is only 16-byte aligned
+                                   silently takes the 128-bit kernel. */
     DPI_OPT_COUNT_
 } dpi_option_t;
 
@@ -154,7 +160,8 @@ dpi_status_t dpi_plan_set_out_dtype(dpi_plan_t* plan, dpi_dtype_t out_dtype);
  *               length sequence only, so its definition does not change; the output stays [B, sum dims] with table
  *               t in its own column block.
  *   index_type  DPI_IDX_I32 (default) or DPI_IDX_I64: element type of `indices` (values must still lie in
- *               [0, table_rows[t]), table_rows[t] < 2^31). Offsets stay int32 inside the plan (N < 2^31).
+ *               [0, table_rows[t]), table_rows[t] < 2^31). The element type of the offsets is a separate setting:
+ *               dpi_plan_set_offset_type below (int32 by default, N < 2^31).
  */
 dpi_status_t dpi_plan_set_layout(dpi_plan_t* plan, dpi_bag_order_t order, dpi_index_type_t index_type);
 
@@ -245,8 +252,9 @@ dpi_status_t dpi_plan_stats(const dpi_plan_t* plan, int32_t* min_len, int32_t* m
 /*
  * dpi_lookup -- step a3, asynchronous on `stream`, ONE kernel launch for all tables and samples.
  *   table_ptrs_dev device array of T device pointers; table t is row-major [table_rows[t], D] of the
- *                  plan's dtype, 16-byte aligned -- 32-byte aligned when the row size is a multiple of 32 B, unless
- *                  DPI_OPT_VEC_BYTES = 16 ("Embs", per-table local ids PAPER.md:162)
+ *                  plan's dtype, 16-byte aligned -- 32-byte aligned when 256-bit row loads are in use (DPI_OPT_VEC_BYTES:
+ *                  by default fp32 tables with equal dims and rows >= 256 B) ("Embs", per-table local ids
+ *                  PAPER.md:162)
  *   indices_dev    device int32[N], per-table local row ids, bag-contiguous in bag order g
  *   offsets_dev    NULL (use the plan's own offsets) or a device int32[G+1] equal to them
  *   plan           a built plan (same stream, or ordered after dpi_plan_build by an event)
@@ -310,7 +318,11 @@ dpi_status_t dpi_forward_noalloc(int32_t T, int32_t D, dpi_dtype_t dtype, int32_
 
 /*
  * dpi_plan_status -- did any build of this plan since the last call exceed its capacity (N > max_indices)? Such a build
- * leaves S = 0 behind, so the balanced-segment lookup that follows writes nothing; the planner also bumps a sticky device
+ * leaves S = 0 behind (a fitting batch always has S >= 1), and every a3 kernel launched through dpi_lookup / dpi_lookup_ex /
+ * the two-launch dpi_forward returns at once on S = 0: nothing is read through the oversized offsets and the output block
+ * is left untouched. The ONE exception is dpi_forward's fused single launch: its CTAs pool their chunk before the batch
+ * total N exists anywhere, so an over-capacity batch is pooled and stored like any other (it reads indices[0, N), which the
+ * caller must own anyway); only the plan it leaves behind is marked S = 0. The planner also bumps a sticky device
  * counter, which this call reads (synchronises `stream`) and clears. DPI_OK and *overflowed_builds = 0 when all builds
  * fitted, DPI_ERR_INVALID_ARG and the count otherwise. overflowed_builds may be NULL. Off the hot path: call it once per
  * served batch group, not per lookup.
@@ -416,6 +428,9 @@ dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int
  *   lengths_host int32[G]; indices_host int32 / int64 [n_indices] per the plan's index type
  *   (n_indices <= max_indices); out_host [B, sum dims].
  *   Pinned (page-locked) host buffers make the copies asynchronous and faster but are not required.
+ *   With dpi_plan_set_columns (a row wider than the tables' blocks) the two output paths differ outside the blocks: the direct
+ *   path stores pooled vectors only and leaves every other column of out_host untouched; the staged path copies whole rows
+ *   of its device block back, so columns that belong to no table are overwritten with unspecified values.
  */
 dpi_status_t dpi_forward_host(dpi_plan_t* plan, const void* const* table_ptrs_dev,
                               const int32_t* lengths_host, const void* indices_host, int64_t n_indices,

@@ -732,6 +732,7 @@ dpi_status_t dpi_plan_set_offset_type(dpi_plan_t* p, dpi_offset_type_t type, int
     p->built = false;
     const bool was64 = p->off64;
     const int64_t was_max = p->max_indices;
+    const int32_t was_K = p->K;
     p->off64 = type == DPI_OFF_I64;
     p->max_indices = max_indices;
     dpi_status_t st = DPI_OK;
@@ -749,10 +750,15 @@ dpi_status_t dpi_plan_set_offset_type(dpi_plan_t* p, dpi_offset_type_t type, int
         if (!p->K_user) p->K = default_quantum(p);
         st = ensure_seg_capacity(p, p->K);
     }
-    if (st != DPI_OK) {   // the plan keeps its previous offset type and capacity
+    if (st != DPI_OK) {   // the plan keeps its previous offset type, capacity and quantum (the segment buffer is still sized for them)
         p->off64 = was64;
         p->max_indices = was_max;
+        p->K = was_K;
         return st;
+    }
+    if (!p->off64 && was64) {   // dpi.h: the high words of N / C[G] are zero unless the plan holds 64-bit offsets
+        cudaError_t e = cudaMemset(p->meta + META_N_HI, 0, 2 * sizeof(int32_t));
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMemset(meta high words)");
     }
     if (p->stage_idx) { (void)cudaFree(p->stage_idx); p->stage_idx = nullptr; p->stage_idx_bytes = 0; }
     free_pipeline(p);
@@ -886,7 +892,8 @@ dpi_status_t dpi_plan_status(const dpi_plan_t* p, int32_t* overflowed_builds, vo
     if (n == 0) return DPI_OK;
     DPI_CUDA(cudaMemsetAsync(p->state + kStateOverflows, 0, sizeof n, s));   // reported once
     return fail(DPI_ERR_INVALID_ARG, "%u build(s) since the last dpi_plan_status exceeded the plan's capacity (N > max_indices=%lld): "
-                "their lookups wrote nothing", n, (long long)p->max_indices);
+                "their plans were left with S = 0 and the lookups launched on them wrote nothing (only dpi_forward's fused single launch "
+                "pools such a batch anyway)", n, (long long)p->max_indices);
 }
 
 dpi_status_t dpi_lookup_input_first(const void* const* table_ptrs_dev, const int32_t* indices_dev, const int32_t* offsets_dev,

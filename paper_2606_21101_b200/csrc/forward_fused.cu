@@ -248,10 +248,11 @@ __global__ void __launch_bounds__(kFusedThreads, Tr::kEltBytes == 2 ? 3 : 4) fus
                     pa.offsets[pa.G] = static_cast<int32_t>(n_total);
                     const uint32_t S = c1 / pa.K + ((c1 % pa.K) ? 1u : 0u);
                     if ((c1 % pa.K) != 0 && S < pa.seg_cap) pa.seg[S] = make_int2(static_cast<int>(pa.G), static_cast<int>(n_total));
-                    pa.meta[META_S] = (S < pa.seg_cap) ? S : 0;
+                    const bool overflow = n_total > pa.max_indices || S >= pa.seg_cap;
+                    pa.meta[META_S] = overflow ? 0 : S;   // the plan left behind must not drive a later dpi_lookup (this launch's own
+                                                          // pooling cannot be held back: chunks pool before N is known, dpi.h)
                     pa.meta[META_N] = n_total;
                     pa.meta[META_C] = c1;
-                    const bool overflow = n_total > pa.max_indices || S >= pa.seg_cap;
                     pa.meta[META_OVERFLOW] = overflow ? 1 : 0;
                     if (overflow) atomicAdd(pa.state + kStateOverflows, 1u);
                     pa.meta[META_K] = pa.K;

@@ -17,8 +17,10 @@ template <class Tr, int W, bool OUT32>
 __global__ void __launch_bounds__(256) direct_kernel(const LookupArgs a) {
     extern __shared__ const char* s_tab_direct[];
     griddep_wait();  // PDL: nothing (table pointers included) is read before the preceding grid has completed
+    const int S = ld_plan(a.meta + META_S);   // S == 0 marks an overflowed plan (N > max_indices): its offsets may point past indices
     for (uint32_t t = threadIdx.x; t < a.T; t += blockDim.x) s_tab_direct[t] = static_cast<const char*>(a.tables[t]);
     __syncthreads();
+    if (S == 0) return;
     const uint32_t lane_id = blockIdx.x * blockDim.x + threadIdx.x;
     short_bag_body<Tr, W, kDirectU, OUT32>(a, s_tab_direct, lane_id / W, lane_id % W, (gridDim.x * blockDim.x) / W);
 }

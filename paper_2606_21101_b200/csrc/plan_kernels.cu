@@ -258,10 +258,11 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
                 a.offsets[a.G] = n_total;
                 const uint32_t S = c / a.K + ((c % a.K) ? 1u : 0u);   // ceil(C[G]/K)
                 if ((c % a.K) != 0 && S < a.seg_cap) a.seg[S] = make_int2(a.G, n_total);  // C[G] < S*K: clamped to G
-                a.meta[META_S] = (S < a.seg_cap) ? S : 0;             // an overflowed plan must not drive a lookup
+                const bool overflow = n_total > a.max_indices || S >= a.seg_cap;
+                a.meta[META_S] = overflow ? 0 : S;                    // an overflowed plan must not drive a lookup (S = 0 is the mark:
+                                                                      // a fitting batch has S >= 1), as in plan64_kernels.cu
                 a.meta[META_N] = n_total;
                 a.meta[META_C] = c;
-                const bool overflow = n_total > a.max_indices || S >= a.seg_cap;
                 a.meta[META_OVERFLOW] = overflow ? 1 : 0;
                 if (overflow) atomicAdd(a.state + kStateOverflows, 1u);   // sticky until dpi_plan_status reads it
                 a.meta[META_K] = a.K;
@@ -288,7 +289,8 @@ __global__ void __launch_bounds__(kScanThreads) plan_scan_partition_kernel(const
         a.state[kStateMaxLen] = 0u;
         uint32_t next = epoch + 1;
         if (next >= kEpochLimit) {  // 30-bit tag about to wrap: clear the records once and restart at 1
-            for (uint32_t i = 0; i < a.num_chunks; ++i) a.status[i] = make_ulonglong2(0ull, 0ull);
+            // all kStatusRecords of them: the buffer is shared with fused_forward_kernel, which tags up to 640 records
+            for (uint32_t i = 0; i < static_cast<uint32_t>(kStatusRecords); ++i) a.status[i] = make_ulonglong2(0ull, 0ull);
             next = 1;
         }
         a.state[kStateEpoch] = next;

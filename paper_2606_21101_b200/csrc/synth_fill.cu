@@ -3,7 +3,7 @@
 // NOT part of the method: this is the input generator of workloads.py restated for the device, so that an
 // 82 GB table set can be created in place (the host cannot mirror it). Same counter-based recipe:
 //   h = fmix64(key + i*GAMMA),  i = r*D + c,   x = float(h >> 40) * 2^-24,   v = (x - 0.5f) * 0.1f
-// then one RNE cast to the table dtype. tests/test_gpu_synth.py checks host/device equality bit for bit.
+// then one RNE cast to the table dtype. tests/test_gpu_parity.py::test_synth_fill_matches_host_generator checks host/device equality bit for bit.
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
 #include <cuda_bf16.h>

@@ -205,7 +205,14 @@ class TableWiseLookup:
     -> barrier. Rank r holds `tables_r` (all rows of each) and, per call, receives the bags of its tables for EVERY sample of
     the global batch; its kernel stores each pooled vector into the batch shard of the rank that owns the sample, at the
     table's global column. After `forward` returns, `out.local` holds this rank's rows [rank * rows_per_rank, ...) of the
-    global [B, sum dims] block, complete. Comm on the data path: peer stores only, no NCCL."""
+    global [B, sum dims] block, complete. Comm on the data path: peer stores only, no NCCL.
+
+    The output shard is DOUBLE-BUFFERED: step k stores into block k % 2 of every rank. There is one barrier per step, after
+    the stores; a rank that leaves it may start step k+1 at once, and its kernel then stores into the OTHER block of its
+    peers, which may still be reading step k's result. Block k % 2 is written again only in step k+2, which a peer reaches
+    after the barrier of step k+1 -- and every rank enters that barrier through a device synchronise, i.e. after whatever it
+    had enqueued on step k's result. Hence the contract: the tensor `forward` returns stays valid until the second-next
+    `forward` call on this object; enqueue its consumers before calling `forward` again (any stream of this device)."""
 
     def __init__(self, dims, table_rows, dtype_code: int, torch_dtype, B_global: int, max_indices: int, device, cost=None,
                  group=None, out_dtype_code=None):
@@ -230,23 +237,38 @@ class TableWiseLookup:
             if out_dtype_code is not None:
                 self.plan.set_out_dtype(out_dtype_code)
             self.plan.set_columns([int(self.columns[t]) for t in self.mine])
-        self.out = PeerOutput(self.rows_per_rank, self.width, torch_dtype, device, group)
+        self.outs = [PeerOutput(self.rows_per_rank, self.width, torch_dtype, device, group) for _ in range(2)]
+        self._step = 0
+
+    @property
+    def out(self) -> "PeerOutput":
+        """The block the most recent `forward` filled (block 0 before the first call)."""
+        return self.outs[(self._step - 1) % 2] if self._step else self.outs[0]
+
+    def fill(self, value: float):
+        """Fill both local blocks (tests: NaN sentinel) and wait until every rank has done so."""
+        for o in self.outs:
+            o.local.fill_(value)
+        self.outs[0].barrier()
 
     def forward(self, lengths_dev, indices_dev, table_ptrs_dev, pooling=None, stream=None):
         """lengths / indices: this rank's table shard of the global batch (table_shard_batch), on the device; table_ptrs_dev:
         device pointer array of this rank's tables (ascending global id). Returns this rank's complete batch shard."""
+        buf = self.outs[self._step % 2]
         if self.plan is not None:
             self.plan.build(lengths_dev, stream)
             self.plan.lookup_ex(table_ptrs_dev, indices_dev, None, pooling=pooling, out_ld=self.width,
-                                out_peers_dev=self.out.ptrs, n_peers=self.world, rows_per_peer=self.rows_per_rank, stream=stream)
-        self.out.barrier()
-        return self.out.local
+                                out_peers_dev=buf.ptrs, n_peers=self.world, rows_per_peer=self.rows_per_rank, stream=stream)
+        buf.barrier()
+        self._step += 1
+        return buf.local
 
     def close(self):
         if self.plan is not None:
             self.plan.destroy()
             self.plan = None
-        self.out.close()
+        for o in self.outs:
+            o.close()
 
 
 def table_wise_forward(tw: "TableWiseLookup", lengths_dev, indices_dev, table_ptrs_dev, pooling=None, stream=None):

@@ -172,6 +172,23 @@ def test_forward_overflow_is_counted():
     assert plan.status() == 1 and plan.status() == 0
     with pytest.raises(binding.DpiError):
         plan.export()
+    # The plan it left behind carries S = 0 (N = max_indices + 1 still fits the segment buffer: the case ADVICE r2 found), so
+    # no later lookup on it reads or writes anything: balanced segments, the device-picked and the host-picked short-bag body
+    for mode, hint in ((0, 0), (3, 0), (6, 0), (0, 4)):
+        plan.set_option(binding.OPT_MODE, mode)
+        plan.set_option(binding.OPT_MAX_BAG_HINT, hint)
+        out2 = harness.new_output(cfg, fill_nan=True)
+        plan.lookup(dt.ptrs, db.indices, out2, pooling=cfg.pooling_modes())
+        torch.cuda.synchronize()
+        assert bool(torch.isnan(out2).all()), (mode, hint)
+    # ... and the two-launch dpi_forward (planner + lookup) leaves the block untouched as a whole
+    plan.set_option(binding.OPT_MODE, 0)
+    plan.set_option(binding.OPT_MAX_BAG_HINT, 0)
+    plan.set_option(binding.OPT_FUSED, 2)
+    out3 = harness.new_output(cfg, fill_nan=True)
+    plan.forward(db.lengths, dt.ptrs, db.indices, out3, pooling=cfg.pooling_modes())
+    torch.cuda.synchronize()
+    assert bool(torch.isnan(out3).all()) and plan.status() == 1
     plan.destroy()
 
 

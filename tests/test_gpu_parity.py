@@ -99,6 +99,16 @@ def test_plan_overflow_is_reported_not_out_of_bounds():
     plan.build(torch.from_numpy(ln).cuda())
     assert plan.status() == 2
     assert plan.status() == 0
+    # N = max_indices + 1: the segment buffer (sized for max_indices + G) still has room, the plan is marked S = 0 all the same
+    one_over = np.full(100, 5, np.int32)
+    one_over[17] = 6
+    plan.build(torch.from_numpy(one_over).cuda())
+    _, _, meta_ptr = plan.device_views()
+    meta = torch.zeros(12, dtype=torch.int32, device="cuda")
+    binding.copy_device_words(meta, meta_ptr, 12)
+    meta = meta.cpu().numpy()
+    assert meta[0] == 0 and meta[1] == 501 and meta[3] == 1      # S, N, overflow flag
+    assert plan.status() == 1
     ok = np.full(100, 5, np.int32)
     plan.build(torch.from_numpy(ok).cuda())
     assert plan.status() == 0 and plan.export()[3] == 500
@@ -300,6 +310,8 @@ def test_forward_host_equals_device_path():
     out = torch.empty((cfg.B, cfg.T * cfg.D), dtype=torch.bfloat16).pin_memory()
     plan.forward_host(dt.ptrs, ln, idx, out, pooling=pooling)
     assert np.array_equal(out.double().numpy(), dev)
+    ref = oracle_reference(host_tables, cfg.dtype, cfg.B, batch.lengths, batch.indices, pooling)
+    assert_outputs_match(out.double().numpy(), ref, batch.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out)   # and against the oracle
     # the pipelined variant (chunks of whole samples over three streams) gives the same block, ragged last chunk included
     for chunks in (2, 3, 7, 64):
         plan.set_option(binding.OPT_HOST_CHUNKS, chunks)
@@ -391,20 +403,56 @@ def test_c5_full_size_sampled():
     _sampled_full_size(W.C5, 4096)
 
 
+def _via_forward(cfg, dt, batch, pooling):
+    """dpi_forward (what bench.py times for `value`): planner + lookup, or one fused launch, library defaults."""
+    db = harness.upload_batch(batch)
+    plan = harness.make_plan(cfg, dt.rows, max(batch.N, 1))
+    out = harness.new_output(cfg, fill_nan=True)
+    plan.forward(db.lengths, dt.ptrs, db.indices, out, pooling=pooling)
+    torch.cuda.synchronize()
+    res = harness.out_to_f64(out)
+    plan.destroy()
+    return res
+
+
+def _via_forward_host(cfg, dt, batch, pooling, direct_out):
+    """dpi_forward_host (the call behind bench.py's `e2e`): pinned host buffers, library-default chunking (c5: 8 sample chunks
+    on three streams, first chunk a quarter of the rest), NaN-filled host block. direct_out: 0 = auto (the lookup stores
+    straight into the pinned block over PCIe), 1 = staged block + D2H copy."""
+    plan = harness.make_plan(cfg, dt.rows, max(batch.N, 1))
+    plan.set_option(binding.OPT_HOST_DIRECT_OUT, direct_out)
+    ln = torch.from_numpy(np.ascontiguousarray(batch.lengths)).pin_memory()
+    idx = torch.from_numpy(np.ascontiguousarray(batch.indices)).pin_memory()
+    out = torch.full((cfg.B, cfg.T * cfg.D), float("nan"), dtype=harness.TORCH_DTYPE[cfg.out]).pin_memory()
+    plan.forward_host(dt.ptrs, ln, idx, out, pooling=pooling)
+    res = out.to(torch.float64).numpy()
+    plan.destroy()
+    return res
+
+
 def _every_sample_full_size(cfg, samples_per_pass):
-    """Every output element of one full-size batch against the oracle. The tables do not fit on the host (c5) or are slow to
-    mirror (c4), so the oracle works through the batch in passes of `samples_per_pass` samples, each on tables compacted to
-    the rows that pass references (values recomputed from the counter-based generator, never read back from the device)."""
+    """Every output element of one full-size batch against the oracle, through every entry point bench.py times: dpi_plan_build +
+    dpi_lookup, dpi_forward (`value`), dpi_forward_host with the library defaults and with the staged output (`e2e`). The tables do
+    not fit on the host (c5) or are slow to mirror (c4), so the oracle works through the batch in passes of `samples_per_pass`
+    samples, each on tables compacted to the rows that pass references (values recomputed from the counter-based generator,
+    never read back from the device); each pass's reference is compared with all four blocks."""
     dt = harness.make_device_tables(cfg)
     batch = W.make_batch(cfg, dt.rows, cfg.seed)
     pooling = cfg.pooling_modes()
-    got = _run_gpu(cfg, dt, batch, pooling)
+    gots = {"plan_build + lookup": _run_gpu(cfg, dt, batch, pooling),
+            "forward": _via_forward(cfg, dt, batch, pooling),
+            "forward_host (auto)": _via_forward_host(cfg, dt, batch, pooling, 0),
+            "forward_host (staged out)": _via_forward_host(cfg, dt, batch, pooling, 1)}
     worst = 0.0
     for lo in range(0, cfg.B, samples_per_pass):
         samples = np.arange(lo, min(cfg.B, lo + samples_per_pass))
         sub = W.compact_subproblem(cfg, batch, samples)
         ref = oracle.lookup(sub.tables, W.DTYPE_CODE[cfg.dtype], len(samples), sub.indices, host_offsets(sub.lengths), pooling)
-        worst = max(worst, assert_outputs_match(got[samples], ref, sub.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out))
+        for name, got in gots.items():
+            try:
+                worst = max(worst, assert_outputs_match(got[samples], ref, sub.lengths, cfg.T, cfg.D, cfg.dtype, cfg.out))
+            except AssertionError as e:
+                raise AssertionError(f"{name}, samples {lo}..{samples[-1]}: {e}") from e
     del dt
     torch.cuda.empty_cache()
     return worst

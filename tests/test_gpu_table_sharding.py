@@ -40,26 +40,37 @@ def _worker(rank, world, port, dtype, out, B, q):
         dims = DIMS[dtype]
         T = len(dims)
         cfg = W.Config("tw", T, tuple(ROWS), max(dims), dtype, B, ("poisson", 5.0, 30, 0.1), ("zipf", 1.1), "sum", seed=6)
-        glob = W.make_batch(cfg, np.asarray(ROWS, np.int64), 9)
+        # three steps on three DIFFERENT global batches (a stale or half-overwritten block cannot pass for the current one)
+        globs = [W.make_batch(cfg, np.asarray(ROWS, np.int64), 9 + k) for k in range(3)]
         host_tables = W.mixed_dim_tables(cfg.seed, dims, ROWS, dtype)
         tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[out]
-        tw = sharding.TableWiseLookup(dims, ROWS, W.DTYPE_CODE[dtype], tdt, B, max(glob.N, 1), "cuda:0",
+        tw = sharding.TableWiseLookup(dims, ROWS, W.DTYPE_CODE[dtype], tdt, B, max(max(g.N for g in globs), 1), "cuda:0",
                                       out_dtype_code=W.DTYPE_CODE[out] if out != dtype else None)
         assert sorted(sum(tw.parts, [])) == list(range(T)) and tw.world == world
-        tw.out.local.fill_(float("nan"))
-        tw.out.barrier()            # every block is NaN-filled before anybody's kernel stores into it
-        local = sharding.table_shard_batch(glob, T, tw.mine)
+        tw.fill(float("nan"))       # every block is NaN-filled before anybody's kernel stores into it
         tables, ptrs = harness.tables_from_host_mixed([host_tables[t] for t in tw.mine], dtype)
-        ln = torch.from_numpy(local.lengths).cuda()
-        idx = torch.from_numpy(local.indices if local.N else np.zeros(1, np.int32)).cuda()
-        for _ in range(2):          # the second call reuses plan and mapped peer blocks
-            shard = sharding.table_wise_forward(tw, ln, idx, ptrs, pooling=POOL[tw.mine])
-        ref = oracle.lookup_general(host_tables, W.DTYPE_CODE[dtype], B, glob.indices,
-                                    host_offsets(glob.lengths).astype(np.int64), POOL)
         lo = rank * tw.rows_per_rank
         hi = min(B, lo + tw.rows_per_rank)
-        got = harness.out_to_f64(shard[: hi - lo])
-        assert_outputs_match_general(got, ref[lo:hi], glob.lengths.reshape(B, T)[lo:hi], dims, dtype, out)
+
+        def check(shard, glob):
+            ref = oracle.lookup_general(host_tables, W.DTYPE_CODE[dtype], B, glob.indices,
+                                        host_offsets(glob.lengths).astype(np.int64), POOL)
+            got = harness.out_to_f64(shard[: hi - lo])
+            assert_outputs_match_general(got, ref[lo:hi], glob.lengths.reshape(B, T)[lo:hi], dims, dtype, out)
+
+        prev = None
+        for glob in globs:          # later calls reuse plan and mapped peer blocks
+            local = sharding.table_shard_batch(glob, T, tw.mine)
+            ln = torch.from_numpy(local.lengths).cuda()
+            idx = torch.from_numpy(local.indices if local.N else np.zeros(1, np.int32)).cuda()
+            shard = sharding.table_wise_forward(tw, ln, idx, ptrs, pooling=POOL[tw.mine])
+            check(shard, glob)
+            # the previous step's block is still intact although every rank has stored a whole new step since (double
+            # buffering: a rank racing ahead writes the other block; sharding.TableWiseLookup docstring)
+            if prev is not None:
+                assert prev[0].data_ptr() != shard.data_ptr()
+                check(*prev)
+            prev = (shard, glob)
         launches = binding.launch_count()
         tw.close()
         q.put((rank, True, launches))
@@ -83,4 +94,4 @@ def test_two_processes_exchange_their_column_blocks_through_peer_stores(dtype, o
         assert p.exitcode == 0
     res = sorted(q.get(timeout=10) for _ in range(2))
     assert [r[1] for r in res] == [True, True], res
-    assert all(r[2] >= 4 for r in res)     # each rank launched its own planner + lookup twice
+    assert all(r[2] >= 6 for r in res)     # each rank launched its own planner + lookup three times
