@@ -247,6 +247,18 @@ def describe(cfg, rows, extra=None, R=R_BATCHES):
 # ----------------------------------------------------------------------------------------------------
 # CPU oracle legs
 # ----------------------------------------------------------------------------------------------------
+def synth_library():
+    """libdpi_synth.so (seeded table generator on the device) by path, or None when it has not been built."""
+    import ctypes
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_2606_21101_b200", "lib", "libdpi_synth.so")
+    if not os.path.exists(path):
+        return None
+    lib = ctypes.CDLL(path)
+    lib.dpi_synth_fill_table.restype = ctypes.c_int
+    lib.dpi_synth_fill_table.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int, ctypes.c_uint64, ctypes.c_void_p]
+    return lib
+
+
 def host_mirror(cfg, rows, budget_bytes):
     """Host copy of the tables for the CPU legs: the full tables when they fit the budget (c1-c4), else
     a ROW-SCALED mirror -- the first rows_s[t] rows of every table, indices taken modulo rows_s[t] (c5: 82 GB do not fit a
@@ -260,18 +272,23 @@ def host_mirror(cfg, rows, budget_bytes):
         cuda = torch.cuda.is_available()
     except Exception:
         cuda = False
-    if not cuda:
+    synth = synth_library() if cuda else None
+    if synth is None:   # tables generated on the host: keep that bounded
         budget_bytes = min(budget_bytes, 1 << 30)
     scale = min(1.0, budget_bytes / max(total, 1))
     rows_s = np.maximum(1, np.floor(rows * scale)).astype(np.int64) if scale < 1.0 else rows.copy()
     tables = []
-    if cuda:
+    if synth is not None:
+        # the seeded generator's device restatement (libdpi_synth.so: no method arithmetic), loaded directly -- this leg touches
+        # neither the product's binding nor libdpi.so; if the helper library has not been built the host generator is used
         import torch
-        from paper_2606_21101_b200 import binding, build, harness
-        build.build()
+        tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[cfg.dtype]
         for t in range(cfg.T):
-            buf = torch.empty((int(rows_s[t]), cfg.D), dtype=harness.TORCH_DTYPE[cfg.dtype], device="cuda")
-            binding.synth_fill_table(buf, buf.numel(), W.DTYPE_CODE[cfg.dtype], W.value_key(cfg.seed, t))
+            buf = torch.empty((int(rows_s[t]), cfg.D), dtype=tdt, device="cuda")
+            rc = synth.dpi_synth_fill_table(buf.data_ptr(), buf.numel(), W.DTYPE_CODE[cfg.dtype], W.value_key(cfg.seed, t),
+                                            torch.cuda.current_stream().cuda_stream)
+            if rc != 0:
+                raise SystemExit(f"bench.py: dpi_synth_fill_table failed with cudaError {rc}")
             h = buf.cpu()
             tables.append(h.view(torch.int16).numpy().view(np.uint16) if cfg.dtype == "bf16" else h.numpy())
             del buf
@@ -410,6 +427,32 @@ def link_floor(h2d_bytes: int, d2h_bytes: int, device: str, reps: int = 5) -> di
             "both_gbs": (h2d_bytes + d2h_bytes) / both / 1e6}
 
 
+def unique_rows(batch, T):
+    """Distinct (table, row) pairs one batch gathers: the entries of table t are those of bags g = b*T + t (sample-major)."""
+    lengths = np.asarray(batch.lengths, dtype=np.int64)
+    table_of_entry = np.repeat(np.tile(np.arange(T, dtype=np.int64), lengths.size // T), lengths)
+    idx = np.asarray(batch.indices, dtype=np.int64)
+    return int(np.unique(table_of_entry * (1 << 32) + idx).size) if idx.size else 0
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without torchrun: start the N ranks ourselves (one process per GPU, rendezvous on 127.0.0.1)
+    and pass their output through; rank 0 prints the one JSON line."""
+    import socket
+    import subprocess
+    if args.impl != "reference":
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) visible; refusing to report n_gpus={args.gpus}")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def run_ours(args):
     import torch
     from paper_2606_21101_b200 import binding, build, harness, sharding, workloads as W
@@ -534,8 +577,54 @@ def run_ours(args):
                     plan.lookup(dt.ptrs, b.indices, out, pooling=pooling, stream=stream)
                 ev[i][1].record(stream)
     barrier()
-    plan.set_option(binding.OPT_PDL, pdl_was)
     kernel_ms = [a.elapsed_time(b) for a, b in ev]
+    kernel_ms_source = "CUDA-event pair around each of %d plain stream launches" % n_k
+    plain_graph_ms = None
+    if graph is not None:
+        # A microsecond-scale kernel cannot be timed by an event pair around ONE stream launch: the pair measures launch
+        # latency (round 2 printed kernel times longer than the graph-replayed step that contains the kernel). For the
+        # graph-launched configs the kernel time is taken from graph replays instead: the step itself when it is ONE launch,
+        # else the step minus a graph of the planner launches alone. A graph of back-to-back PLAIN launches (PDL off, no overlap
+        # between consecutive kernels) is reported beside it.
+        def graph_ms(body):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                for i in range(n_k):
+                    body(batches[i % R], torch.cuda.current_stream())
+            g.replay()
+            barrier()
+            best = None
+            for _ in range(3):
+                a_, b2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                with torch.cuda.stream(stream):
+                    a_.record(stream)
+                    g.replay()
+                    b2.record(stream)
+                barrier()
+                t = a_.elapsed_time(b2) / n_k
+                best = t if best is None else min(best, t)
+            return best
+
+        def whole(b, s_):
+            if ablation:
+                plan.build(b.lengths, s_)
+                plan.lookup_input_first(dt.ptrs, b.indices, out, pooling=pooling, stream=s_)
+            else:
+                plan.forward(b.lengths, dt.ptrs, b.indices, out, pooling=pooling, stream=s_)
+
+        plain_graph_ms = graph_ms(whole)          # PDL off: consecutive kernels do not overlap
+        plan.set_option(binding.OPT_PDL, pdl_was)
+        step_graph_ms = total_ms / steps
+        if fused:
+            # one launch per step: the kernel IS the graph-replayed step (with PDL on, as timed, consecutive launches overlap by
+            # their prologue, so the step can be a little shorter than a plain back-to-back launch)
+            kernel_ms = [step_graph_ms]
+            kernel_ms_source = "the graph-replayed step itself (one launch per step, library-default PDL)"
+        else:
+            kernel_ms = [step_graph_ms - graph_ms(lambda b, s_: plan.build(b.lengths, s_))]
+            kernel_ms_source = ("graph-replayed step minus a graph of %d planner launches alone (best of 3 replays, / %d), "
+                                "library-default PDL" % (n_k, n_k))
+    plan.set_option(binding.OPT_PDL, pdl_was)
     # and the stream-launched step (no graph), for the graph-vs-stream comparison
     s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(stream):
@@ -556,6 +645,9 @@ def run_ours(args):
         max_lens.append(plan.stats(stream)[1])
     n_mean, s_mean = float(np.mean(Ns)), float(np.mean(Ss))
     bytes_step = W.algorithmic_bytes(cfg, cfg.G, n_mean, s_mean)
+    # north_star: "also shown with unique-row bytes" -- distinct (table, row) pairs a batch touches (np.unique per table on the
+    # host, after timing, mean over the rotating batches): the row bytes a perfect cache would fetch from HBM
+    uniq_rows = float(np.mean([unique_rows(b.host, cfg.T) for b in batches]))
 
     # ---- end to end through the host-buffer entry point ----------------------------------------------------
     e2e = None
@@ -610,13 +702,22 @@ def run_ours(args):
             variant = "planner + direct_kernel (DPI_OPT_MAX_BAG_HINT promise)"
     k_bytes = bytes_step["total"] if fused else bytes_step["lookup"]
     achieved = k_bytes / (k_ms * 1e-3) / 1e9
+    # the same launch counted with every distinct row once: algorithmic bytes minus the repeated row reads
+    uniq_bytes = k_bytes - (n_mean - uniq_rows) * cfg.row_bytes
+    step_ms = total_ms / steps
+    if k_ms > step_ms * 1.02 and not ablation:
+        raise SystemExit(f"bench.py: kernel time {k_ms:.5f} ms exceeds the step it is part of ({step_ms:.5f} ms): the kernel timing is broken")
     traffic, traffic_note = ncu_traffic(cfg.name, ncu_name)
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "frac_of_nominal_8000": achieved / 8000.0, "traffic": traffic,
                 "algorithmic_bytes_per_launch": k_bytes, "kernel_ms_avg": k_ms,
                 "kernel_ms_min": min(kernel_ms), "kernel_ms_median": statistics.median(kernel_ms),
-                "kernel_launches_timed": n_k, "kernel_share_of_step": k_ms / stream_step_ms}
+                "kernel_launches_timed": n_k, "kernel_ms_source": kernel_ms_source,
+                "kernel_ms_plain_launch_graph": plain_graph_ms,   # graph of back-to-back plain (PDL-off) launches of the step, / launches
+                "kernel_share_of_step": k_ms / (step_ms if graph is not None else stream_step_ms),
+                "unique_rows_per_launch": uniq_rows, "unique_row_bytes": uniq_bytes,
+                "unique_row_gbs": uniq_bytes / (k_ms * 1e-3) / 1e9, "unique_row_frac": uniq_bytes / (k_ms * 1e-3) / 1e9 / peak}
     if traffic_note:
         roofline["traffic_note"] = traffic_note
     cpu = None
@@ -749,6 +850,10 @@ def run_table_sharded(args):
 
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)   # does not return
+    if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus and args.shard != "tables":
+        raise SystemExit(f"bench.py: --gpus {args.gpus} disagrees with WORLD_SIZE={os.environ['WORLD_SIZE']}")
     if args.impl == "reference":
         run_reference(args)
     elif args.shard == "tables":

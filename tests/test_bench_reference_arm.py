@@ -47,3 +47,25 @@ def test_reference_arm_under_torchrun_two_ranks_prints_one_line():
     lines = _json_lines(r.stdout)
     assert len(lines) == 1
     _check(lines[0], 2)
+
+
+def test_bench_gpus_2_without_torchrun_launches_its_own_ranks():
+    """`python bench.py --gpus 2` started the way the driver starts the N = 1 bench (no torchrun, no WORLD_SIZE): bench.py
+    spawns the two ranks itself and rank 0 prints the one line with n_gpus = 2. The reference arm needs no GPU, so this runs
+    here; the CUDA arm takes the same spawn path and refuses loudly when fewer than N devices are visible."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, "bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "1",
+                        "--workload", "c1"], cwd=ROOT, capture_output=True, text=True, timeout=900, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = _json_lines(r.stdout)
+    assert len(lines) == 1
+    assert lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2 and lines[0]["config"]["workload"].startswith("c1")
+
+
+def test_bench_cuda_arm_refuses_more_gpus_than_visible():
+    import torch
+    n = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, "bench.py", "--gpus", str(n + 2), "--steps", "1"], cwd=ROOT, capture_output=True, text=True,
+                       timeout=300, env=env)
+    assert r.returncode != 0 and "refusing" in (r.stderr + r.stdout)
