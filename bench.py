@@ -9,7 +9,8 @@ batch of seeded synthetic input already resident in HBM; the timed loop rotates 
 default workload is BASELINE.json configs[4] (c5: 8 x 4e7 rows, D=64 fp32, B=65536, bags U{1..64}, uniform
 indices) -- the configuration the north_star's bandwidth target is quoted on; it fits one GPU (82 GB).
 Multi-GPU: the path shards by batch with no data-path collective (every rank holds all tables and its own
-batch): weak scaling, value = bags of all ranks / max-over-ranks device time.
+batch): weak scaling, value = bags of all ranks / max-over-ranks device time. `--gpus N` without torchrun
+(no WORLD_SIZE in the environment) starts the N ranks itself; the CUDA arm refuses if fewer than N devices are visible.
 
 Prints ONE JSON line (rank 0). `--impl reference` times the CPU oracle (oracle/) on a bounded sample.
 """
